@@ -1,0 +1,168 @@
+/*
+ * nrr_bm.h -- C ABI of the B200-native block-matching library (libnrr_bm.so).
+ *
+ * The data-parallel hot path of the physics-based non-rigid registration of arxiv/paper_2308_10868:
+ * variance-based block ("feature") selection in the pre-operative image and exhaustive NCC block matching
+ * against the intra-operative image.  Everything below runs in hand-written CUDA kernels for sm_100a; there
+ * is no CPU fallback: without a CUDA device every compute entry point returns NRR_E_CUDA.
+ *
+ * NAMES (BASELINE.json / SURVEY.md section 0).  The paper and this ABI use opposite image names:
+ *   "fixed"  = the paper's FLOATING / pre-operative image: blocks are selected and cut here
+ *              (section 3);
+ *   "moving" = the paper's REFERENCE / target / intra-operative image: the search window lives here
+ *              (listing PAPER.md:660-662, section 4.3 "search window sw in fixed image").
+ *
+ * LAYOUT.  A volume with dims = (nx, ny, nz) is a dense fp32 array, voxel (x,y,z) at (z*ny + y)*nx + x
+ * (x fastest).  Both volumes share dims (rigidly pre-aligned images on a common grid).
+ * All triples (dims, block, stride, window, block centres, displacements) are in (x, y, z) order.
+ *
+ * POINTERS.  In the device entry points every volume / array pointer is a DEVICE pointer owned by the
+ * caller (e.g. a torch tensor); dims/block/stride/window and out_n are HOST pointers.  In the *_host entry
+ * points every pointer is a HOST pointer.  `stream` is a cudaStream_t passed as void* (NULL = the legacy
+ * default stream).  The library never frees or retains caller pointers past the stream-ordered completion
+ * of the call; internal scratch is library-owned, allocated stream-ordered (cudaMallocAsync) and reused.
+ *
+ * ERRORS.  Every entry point returns NRR_OK (0) or a negative nrr_status; no exception crosses the ABI.
+ * nrr_bm_last_error() returns a thread-local message for the last nonzero return on this thread.
+ */
+#ifndef NRR_BM_H
+#define NRR_BM_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define NRR_BM_VERSION 100 /* 0.1.0 : major*10000 + minor*100 + patch */
+
+#if defined(__GNUC__)
+#define NRR_BM_API __attribute__((visibility("default")))
+#else
+#define NRR_BM_API
+#endif
+
+typedef enum nrr_status {
+    NRR_OK = 0,
+    NRR_E_NULL = -1,     /* a required pointer is NULL */
+    NRR_E_DIMS = -2,     /* a dimension is < 1, or the block is larger than the volume */
+    NRR_E_BLOCK = -3,    /* a block edge is < 1 or even (centres need odd edges; the paper parameterises
+                            blocks by a half size) */
+    NRR_E_STRIDE = -4,   /* a stride is < 1 */
+    NRR_E_WINDOW = -5,   /* a window half-range is < 0 */
+    NRR_E_FRAC = -6,     /* frac outside (0, 1] */
+    NRR_E_CAPACITY = -7, /* K > capacity; *out_n is still set to K, out_blocks holds the first `capacity` */
+    NRR_E_BOUNDS = -8,   /* a supplied block leaves the volume (validated on the device; reported by the
+                            synchronising host entry points and by nrr_bm_check_async_error) */
+    NRR_E_SMEM = -9,     /* block / window too large for the kernels' shared-memory or index limits */
+    NRR_E_CUDA = -10,    /* a CUDA runtime call failed (message in nrr_bm_last_error) */
+    NRR_E_ARG = -11      /* other invalid argument (n < 0, capacity < 0, ...) */
+} nrr_status;
+
+/*
+ * Variance-based block selection  --  PAPER.md:231-236 (section 3: registration points are where "the
+ * variability in the intensities in the surrounding region exceeds some threshold", identified "prior to
+ * the time-critical part") and PAPER.md:376 (section 4.1: "computes the variance within a block of size
+ * B_s", "selects F_s features with the highest variance", "0.5 + NFeatures x Fs blocks are selected").
+ *
+ * Candidates: the stride grid from origin 0 with blocks fully inside the volume, in ascending linear grid
+ * order (x fastest); a grid position is a candidate iff mask == NULL or mask[centre voxel] != 0; the
+ * population variance is taken over the whole block regardless of the mask.  With N candidates,
+ * K = floor(0.5 + N*frac) are kept: those of largest variance, ties to the lower candidate index.
+ *
+ *   fixed      [in]  device fp32 [nz][ny][nx]
+ *   dims       [in]  host int[3] (nx, ny, nz)
+ *   block      [in]  host int[3] full odd edge length per axis
+ *   stride     [in]  host int[3] grid stride per axis, >= 1
+ *   frac       [in]  selection fraction F_s in (0, 1]
+ *   mask       [in]  device uint8 [nz][ny][nx], or NULL (= every voxel)
+ *   out_blocks [out] device int32 [capacity][3]: block CENTRES (origin + (B-1)/2) of the kept candidates in
+ *                    ascending candidate index (a set with a canonical listing)
+ *   capacity   [in]  rows available in out_blocks / out_var
+ *   out_n      [out] HOST int: K.  The call synchronises `stream` once to return it.
+ *   out_var    [out] device double [capacity], or NULL: population variance of each kept block, same order
+ *   out_ncand  [out] HOST int, or NULL: N, the number of candidates
+ */
+NRR_BM_API int nrr_bm_select_blocks(const float *fixed, const int dims[3], const int block[3], const int stride[3],
+                         double frac, const unsigned char *mask, int *out_blocks, int capacity, int *out_n,
+                         double *out_var, int *out_ncand, void *stream);
+
+/*
+ * Exhaustive NCC block matching  --  PAPER.md:236-246 (section 3: for each registration point, the block
+ * displacement "that maximizes the intensity-based similarity metric", NCC equation) and the listing
+ * PAPER.md:659-667 (section 4.3: for each block, each candidate block in the window, similarity, maximum
+ * and its displacement).  Cost bound O(BxByBz x WxWyWz) per point.
+ *
+ * For block b with centre c and origin o = c - (B-1)/2, every displacement d with |d_a| <= window[a] whose
+ * block at o+d stays inside the moving volume is evaluated (others are skipped);
+ *     NCC(d) = sum (f - fbar)(m - mbar) / sqrt( sum (f - fbar)^2 * sum (m - mbar)^2 )
+ * over the B voxels of the fixed block at o and the moving block at o+d; a zero-variance block scores 0.
+ * out_disp[b] = the d of largest NCC (equal maxima: lowest linear candidate index
+ * ((dz+rz)(2ry+1) + (dy+ry))(2rx+1) + (dx+rx)), out_ncc[b] = that NCC.  fixed(p+v) ~ moving(p+d+v);
+ * units are voxels.  out_ncc is the confidence S of PAPER.md:263-264 in raw form.
+ *
+ *   fixed, moving [in]  device fp32 [nz][ny][nx]
+ *   blocks        [in]  device int32 [n][3] block centres (as written by nrr_bm_select_blocks)
+ *   n             [in]  number of blocks, >= 0
+ *   block         [in]  host int[3] full odd edge length per axis
+ *   window        [in]  host int[3] displacement half-range r per axis, >= 0; candidates = prod(2r+1)
+ *   out_disp      [out] device int32 [n][3]
+ *   out_ncc       [out] device fp32 [n]
+ * Asynchronous: kernels are enqueued on `stream` and the call returns.  A block that leaves the volume gets
+ * out_disp = (0,0,0), out_ncc = NaN and raises a sticky device flag that nrr_bm_check_async_error reports.
+ */
+NRR_BM_API int nrr_bm_match(const float *fixed, const float *moving, const int dims[3], const int *blocks, int n,
+                 const int block[3], const int window[3], int *out_disp, float *out_ncc, void *stream);
+
+/* Synchronises `stream` and returns NRR_E_BOUNDS if any nrr_bm_match enqueued on this thread since the last
+ * check saw a block leaving the volume (and clears the flag), NRR_E_CUDA on a CUDA error, else NRR_OK. */
+NRR_BM_API int nrr_bm_check_async_error(void *stream);
+
+/*
+ * Host-buffer forms (all pointers HOST memory; pinned memory makes the copies asynchronous).  They copy the
+ * inputs to the device, run the same kernels as the device forms, copy the results back and synchronise.
+ * nrr_bm_register_host = select + match of one volume pair in one call (both volumes uploaded once); this
+ * is the end-to-end call bench.py times.  out_var / out_ncand may be NULL.
+ */
+NRR_BM_API int nrr_bm_select_blocks_host(const float *fixed, const int dims[3], const int block[3], const int stride[3],
+                              double frac, const unsigned char *mask, int *out_blocks, int capacity,
+                              int *out_n, double *out_var, int *out_ncand);
+NRR_BM_API int nrr_bm_match_host(const float *fixed, const float *moving, const int dims[3], const int *blocks, int n,
+                      const int block[3], const int window[3], int *out_disp, float *out_ncc);
+NRR_BM_API int nrr_bm_register_host(const float *fixed, const float *moving, const int dims[3], const int block[3],
+                         const int stride[3], const int window[3], double frac, const unsigned char *mask,
+                         int *out_blocks, int capacity, int *out_n, int *out_disp, float *out_ncc);
+
+/*
+ * Instrumentation (no effect on results).
+ *  nrr_bm_profile_enable(1): every later select/match call on this thread brackets its phases with CUDA
+ *    events on the caller's stream.  nrr_bm_profile_read synchronises those events and returns the
+ *    accumulated milliseconds and call counts since the last read, then resets them:
+ *      ms[0] = selection kernels (statistics + radix select + compaction), ms[1] = moving-volume statistics
+ *      (per-candidate normalisers), ms[2] = matching kernel;  calls[i] = number of timed launches groups.
+ *  nrr_bm_launch_count(): kernels launched by this library on this thread since the last reset.
+ *  nrr_bm_match_info: which matching kernel a (block, window, dims) triple dispatches to.
+ *      info[0] = 1 fast register-tiled kernel / 0 generic kernel, info[1] = threads per CTA,
+ *      info[2] = dynamic shared memory bytes, info[3] = 1 if TMA staging is used, info[4] = candidates.
+ *  nrr_bm_fp32_peak: runs an FFMA-only microbenchmark on `stream`'s device and returns the measured
+ *      dense FP32 rate in TFLOP/s (the denominator context for the matching kernel's roofline).
+ */
+NRR_BM_API int nrr_bm_profile_enable(int on);
+NRR_BM_API int nrr_bm_profile_read(double ms[3], int calls[3]);
+NRR_BM_API long long nrr_bm_launch_count(int reset);
+NRR_BM_API int nrr_bm_match_info(const int dims[3], const int block[3], const int window[3], int info[5]);
+NRR_BM_API int nrr_bm_fp32_peak(double *out_tflops, void *stream);
+
+/* Tuning / experiment knobs (process-wide; results stay within the documented tolerances):
+ *   "tie_band"      FP32 candidates within this NCC distance of the FP32 maximum are re-scored in FP64
+ *                   (default 1e-4; 0 disables the re-score except for exact FP32 ties)
+ *   "force_generic" != 0: always use the generic matching kernel
+ *   "disable_tma"   != 0: stage shared memory with plain loads instead of TMA */
+NRR_BM_API int nrr_bm_set_option(const char *name, double value);
+
+NRR_BM_API const char *nrr_bm_last_error(void);
+NRR_BM_API const char *nrr_bm_status_string(int status);
+NRR_BM_API int nrr_bm_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NRR_BM_H */

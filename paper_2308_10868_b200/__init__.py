@@ -1,0 +1,11 @@
+"""B200-native block matching for physics-based non-rigid registration (arxiv/paper_2308_10868).
+
+The product is libnrr_bm.so (C ABI in include/nrr_bm.h, CUDA kernels in csrc/); this package is its thin
+Python binding.  Same names as the C entry points.
+"""
+from .binding import (  # noqa: F401
+    EXPORTS, LIB_PATH, NrrError, lib,
+    nrr_bm_check_async_error, nrr_bm_fp32_peak, nrr_bm_launch_count, nrr_bm_match, nrr_bm_match_host,
+    nrr_bm_match_info, nrr_bm_profile_enable, nrr_bm_profile_read, nrr_bm_register_host, nrr_bm_select_blocks,
+    nrr_bm_select_blocks_host, nrr_bm_set_option, nrr_bm_version,
+)

@@ -1,0 +1,267 @@
+"""Thin ctypes binding of libnrr_bm.so (include/nrr_bm.h): argument marshalling only.
+
+Every step of the path runs in the library's CUDA kernels.  PyTorch appears here only as the owner of
+device memory and streams.  There is no CPU fallback: if the library is missing or no CUDA device is
+present the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Sequence, Tuple
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libnrr_bm.so")
+
+NRR_OK = 0
+NRR_E_NULL, NRR_E_DIMS, NRR_E_BLOCK, NRR_E_STRIDE, NRR_E_WINDOW, NRR_E_FRAC = -1, -2, -3, -4, -5, -6
+NRR_E_CAPACITY, NRR_E_BOUNDS, NRR_E_SMEM, NRR_E_CUDA, NRR_E_ARG = -7, -8, -9, -10, -11
+
+EXPORTS = [
+    "nrr_bm_select_blocks", "nrr_bm_match", "nrr_bm_check_async_error",
+    "nrr_bm_select_blocks_host", "nrr_bm_match_host", "nrr_bm_register_host",
+    "nrr_bm_profile_enable", "nrr_bm_profile_read", "nrr_bm_launch_count", "nrr_bm_match_info",
+    "nrr_bm_fp32_peak", "nrr_bm_set_option", "nrr_bm_last_error", "nrr_bm_status_string", "nrr_bm_version",
+]
+
+
+class NrrError(RuntimeError):
+    def __init__(self, status: int, message: str):
+        super().__init__("%s (%d): %s" % (_status_name(status), status, message))
+        self.status = status
+
+
+_lib = None
+
+
+def lib() -> ctypes.CDLL:
+    """Loads libnrr_bm.so (built in-tree by paper_2308_10868_b200/build.py). Raises if it is missing."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError("libnrr_bm.so is not built: run `python -c 'import __graft_entry__ as g; g.build()'` "
+                          "or `python paper_2308_10868_b200/build.py` (there is no CPU fallback)")
+    L = ctypes.CDLL(LIB_PATH)
+    vp, ci, cd = ctypes.c_void_p, ctypes.c_int, ctypes.c_double
+    i3 = ctypes.POINTER(ctypes.c_int)
+    L.nrr_bm_select_blocks.restype = ci
+    L.nrr_bm_select_blocks.argtypes = [vp, i3, i3, i3, cd, vp, vp, ci, i3, vp, i3, vp]
+    L.nrr_bm_match.restype = ci
+    L.nrr_bm_match.argtypes = [vp, vp, i3, vp, ci, i3, i3, vp, vp, vp]
+    L.nrr_bm_check_async_error.restype = ci
+    L.nrr_bm_check_async_error.argtypes = [vp]
+    L.nrr_bm_select_blocks_host.restype = ci
+    L.nrr_bm_select_blocks_host.argtypes = [vp, i3, i3, i3, cd, vp, vp, ci, i3, vp, i3]
+    L.nrr_bm_match_host.restype = ci
+    L.nrr_bm_match_host.argtypes = [vp, vp, i3, vp, ci, i3, i3, vp, vp]
+    L.nrr_bm_register_host.restype = ci
+    L.nrr_bm_register_host.argtypes = [vp, vp, i3, i3, i3, i3, cd, vp, vp, ci, i3, vp, vp]
+    L.nrr_bm_profile_enable.restype = ci
+    L.nrr_bm_profile_enable.argtypes = [ci]
+    L.nrr_bm_profile_read.restype = ci
+    L.nrr_bm_profile_read.argtypes = [ctypes.POINTER(cd), i3]
+    L.nrr_bm_launch_count.restype = ctypes.c_longlong
+    L.nrr_bm_launch_count.argtypes = [ci]
+    L.nrr_bm_match_info.restype = ci
+    L.nrr_bm_match_info.argtypes = [i3, i3, i3, i3]
+    L.nrr_bm_fp32_peak.restype = ci
+    L.nrr_bm_fp32_peak.argtypes = [ctypes.POINTER(cd), vp]
+    L.nrr_bm_set_option.restype = ci
+    L.nrr_bm_set_option.argtypes = [ctypes.c_char_p, cd]
+    L.nrr_bm_last_error.restype = ctypes.c_char_p
+    L.nrr_bm_last_error.argtypes = []
+    L.nrr_bm_status_string.restype = ctypes.c_char_p
+    L.nrr_bm_status_string.argtypes = [ci]
+    L.nrr_bm_version.restype = ci
+    L.nrr_bm_version.argtypes = []
+    _lib = L
+    return L
+
+
+def _status_name(status: int) -> str:
+    try:
+        return lib().nrr_bm_status_string(int(status)).decode()
+    except Exception:  # pragma: no cover
+        return "NRR_E_?"
+
+
+def _check(status: int, allow: Sequence[int] = ()) -> int:
+    if status != NRR_OK and status not in allow:
+        raise NrrError(status, lib().nrr_bm_last_error().decode())
+    return status
+
+
+def _i3(t) -> ctypes.Array:
+    return (ctypes.c_int * 3)(int(t[0]), int(t[1]), int(t[2]))
+
+
+def _dims_of(vol) -> Tuple[int, int, int]:
+    nz, ny, nx = vol.shape
+    return (int(nx), int(ny), int(nz))
+
+
+def _stream_ptr(stream) -> int:
+    import torch
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return int(s.cuda_stream)
+
+
+def _dev(t, dtype, name):
+    import torch
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise TypeError("%s must be a CUDA tensor (no CPU fallback)" % name)
+    if t.dtype != dtype or not t.is_contiguous():
+        raise TypeError("%s must be a contiguous %s tensor" % (name, dtype))
+    return t
+
+
+# --------------------------------------------------------------------------------------------- device API
+def nrr_bm_select_blocks(fixed, block, stride, frac: float, mask=None, capacity: Optional[int] = None,
+                         want_var: bool = False, stream=None):
+    """Device form. fixed: CUDA fp32 [nz][ny][nx]; mask: CUDA uint8 same shape or None.
+    Returns (blocks int32 CUDA [K][3], K, N[, var float64 CUDA [K]])."""
+    import torch
+    fixed = _dev(fixed, torch.float32, "fixed")
+    dims = _dims_of(fixed)
+    if mask is not None:
+        mask = _dev(mask, torch.uint8, "mask")
+        if tuple(mask.shape) != tuple(fixed.shape):
+            raise ValueError("mask shape mismatch")
+    if capacity is None:
+        capacity = 1
+        for a in range(3):
+            capacity *= max(0, (dims[a] - int(block[a])) // max(1, int(stride[a])) + 1)
+        capacity = max(1, capacity)
+    out_blocks = torch.empty((capacity, 3), dtype=torch.int32, device=fixed.device)
+    out_var = torch.empty((capacity,), dtype=torch.float64, device=fixed.device) if want_var else None
+    n = ctypes.c_int(0)
+    ncand = ctypes.c_int(0)
+    with torch.cuda.device(fixed.device):
+        _check(lib().nrr_bm_select_blocks(fixed.data_ptr(), _i3(dims), _i3(block), _i3(stride), float(frac),
+                                          mask.data_ptr() if mask is not None else None, out_blocks.data_ptr(),
+                                          int(capacity), ctypes.byref(n), out_var.data_ptr() if want_var else None,
+                                          ctypes.byref(ncand), _stream_ptr(stream)))
+    k = n.value
+    if want_var:
+        return out_blocks[:k], k, ncand.value, out_var[:k]
+    return out_blocks[:k], k, ncand.value
+
+
+def nrr_bm_match(fixed, moving, blocks, block, window, out_disp=None, out_ncc=None, stream=None):
+    """Device form, asynchronous. Returns (disp int32 CUDA [n][3], ncc fp32 CUDA [n])."""
+    import torch
+    fixed = _dev(fixed, torch.float32, "fixed")
+    moving = _dev(moving, torch.float32, "moving")
+    if tuple(fixed.shape) != tuple(moving.shape):
+        raise ValueError("volume shape mismatch")
+    blocks = _dev(blocks, torch.int32, "blocks")
+    n = int(blocks.shape[0])
+    if out_disp is None:
+        out_disp = torch.empty((n, 3), dtype=torch.int32, device=fixed.device)
+    if out_ncc is None:
+        out_ncc = torch.empty((n,), dtype=torch.float32, device=fixed.device)
+    with torch.cuda.device(fixed.device):
+        _check(lib().nrr_bm_match(fixed.data_ptr(), moving.data_ptr(), _i3(_dims_of(fixed)), blocks.data_ptr(), n,
+                                  _i3(block), _i3(window), out_disp.data_ptr(), out_ncc.data_ptr(), _stream_ptr(stream)))
+    return out_disp, out_ncc
+
+
+def nrr_bm_check_async_error(stream=None) -> None:
+    _check(lib().nrr_bm_check_async_error(_stream_ptr(stream)))
+
+
+# --------------------------------------------------------------------------------------------- host API
+def _np(a, dtype, name):
+    if not isinstance(a, np.ndarray) or a.dtype != dtype or not a.flags["C_CONTIGUOUS"]:
+        raise TypeError("%s must be a C-contiguous numpy %s array" % (name, np.dtype(dtype).name))
+    return a
+
+
+def nrr_bm_select_blocks_host(fixed: np.ndarray, block, stride, frac: float, mask: Optional[np.ndarray] = None,
+                              capacity: Optional[int] = None):
+    fixed = _np(fixed, np.float32, "fixed")
+    dims = _dims_of(fixed)
+    if mask is not None:
+        mask = _np(mask, np.uint8, "mask")
+    if capacity is None:
+        capacity = max(1, int(np.prod([max(0, (dims[a] - block[a]) // stride[a] + 1) for a in range(3)])))
+    out_blocks = np.empty((capacity, 3), dtype=np.int32)
+    out_var = np.empty((capacity,), dtype=np.float64)
+    n, ncand = ctypes.c_int(0), ctypes.c_int(0)
+    _check(lib().nrr_bm_select_blocks_host(fixed.ctypes.data, _i3(dims), _i3(block), _i3(stride), float(frac),
+                                           mask.ctypes.data if mask is not None else None, out_blocks.ctypes.data,
+                                           int(capacity), ctypes.byref(n), out_var.ctypes.data, ctypes.byref(ncand)))
+    return out_blocks[:n.value], n.value, ncand.value, out_var[:n.value]
+
+
+def nrr_bm_match_host(fixed: np.ndarray, moving: np.ndarray, blocks: np.ndarray, block, window):
+    fixed = _np(fixed, np.float32, "fixed")
+    moving = _np(moving, np.float32, "moving")
+    blocks = _np(blocks, np.int32, "blocks")
+    n = int(blocks.shape[0])
+    disp = np.empty((n, 3), dtype=np.int32)
+    ncc = np.empty((n,), dtype=np.float32)
+    _check(lib().nrr_bm_match_host(fixed.ctypes.data, moving.ctypes.data, _i3(_dims_of(fixed)), blocks.ctypes.data, n,
+                                   _i3(block), _i3(window), disp.ctypes.data, ncc.ctypes.data))
+    return disp, ncc
+
+
+def nrr_bm_register_host(fixed, moving, block, stride, window, frac: float, mask=None, out_blocks=None,
+                         out_disp=None, out_ncc=None):
+    """select + match of one pair from HOST buffers (numpy arrays or pinned CPU torch tensors).
+    Returns (blocks [K][3], disp [K][3], ncc [K]) as views of the output buffers."""
+    def ptr(a):
+        return None if a is None else (a.ctypes.data if isinstance(a, np.ndarray) else a.data_ptr())
+    dims = _dims_of(fixed)
+    cap = int(np.prod([max(0, (dims[a] - block[a]) // stride[a] + 1) for a in range(3)]))
+    if out_blocks is None:
+        out_blocks = np.empty((cap, 3), dtype=np.int32)
+        out_disp = np.empty((cap, 3), dtype=np.int32)
+        out_ncc = np.empty((cap,), dtype=np.float32)
+    cap = int(out_blocks.shape[0])
+    n = ctypes.c_int(0)
+    _check(lib().nrr_bm_register_host(ptr(fixed), ptr(moving), _i3(dims), _i3(block), _i3(stride), _i3(window),
+                                      float(frac), ptr(mask), ptr(out_blocks), cap, ctypes.byref(n), ptr(out_disp),
+                                      ptr(out_ncc)))
+    k = n.value
+    return out_blocks[:k], out_disp[:k], out_ncc[:k]
+
+
+# --------------------------------------------------------------------------------------------- instrumentation
+def nrr_bm_profile_enable(on: bool) -> None:
+    _check(lib().nrr_bm_profile_enable(1 if on else 0))
+
+
+def nrr_bm_profile_read():
+    ms = (ctypes.c_double * 3)()
+    calls = (ctypes.c_int * 3)()
+    _check(lib().nrr_bm_profile_read(ms, calls))
+    return {"select_ms": ms[0], "moving_stats_ms": ms[1], "match_ms": ms[2],
+            "select_calls": calls[0], "moving_stats_calls": calls[1], "match_calls": calls[2]}
+
+
+def nrr_bm_launch_count(reset: bool = False) -> int:
+    return int(lib().nrr_bm_launch_count(1 if reset else 0))
+
+
+def nrr_bm_match_info(dims, block, window):
+    info = (ctypes.c_int * 5)()
+    _check(lib().nrr_bm_match_info(_i3(dims), _i3(block), _i3(window), info))
+    return {"fast": bool(info[0]), "threads": info[1], "smem_bytes": info[2], "tma": bool(info[3]), "candidates": info[4]}
+
+
+def nrr_bm_fp32_peak(stream=None) -> float:
+    out = ctypes.c_double(0.0)
+    _check(lib().nrr_bm_fp32_peak(ctypes.byref(out), _stream_ptr(stream)))
+    return out.value
+
+
+def nrr_bm_set_option(name: str, value: float) -> None:
+    _check(lib().nrr_bm_set_option(name.encode(), float(value)))
+
+
+def nrr_bm_version() -> int:
+    return int(lib().nrr_bm_version())

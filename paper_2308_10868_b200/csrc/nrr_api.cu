@@ -1,0 +1,430 @@
+// nrr_api.cu -- the extern "C" boundary of libnrr_bm.so (include/nrr_bm.h): argument validation, scratch
+// management, the host-buffer forms, instrumentation.  Every step of the path itself runs in the kernels of
+// nrr_select.cu / nrr_boxstat.cu / nrr_match.cu; nothing here computes on the CPU.
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <vector>
+
+#include "nrr_internal.cuh"
+
+namespace nrr {
+
+extern float g_tie_band;
+extern int g_force_generic;
+extern int g_disable_tma;
+
+namespace {
+
+thread_local char t_error[512] = "";
+thread_local long long t_launches = 0;
+thread_local int t_profile = 0;
+
+struct TimedSpan { int phase; cudaEvent_t e0, e1; };
+thread_local std::vector<TimedSpan> *t_spans = nullptr;
+
+thread_local unsigned int *t_err_flag = nullptr;      // device, sticky "a block left the volume"
+thread_local void *t_pinned = nullptr;                // small pinned staging buffer
+thread_local cudaStream_t t_host_stream = nullptr;    // stream of the *_host entry points
+thread_local bool t_pool_configured = false;
+
+constexpr size_t kPinnedBytes = 4096;
+
+int ensure_thread_state()
+{
+    if (!t_pool_configured) {
+        int dev = 0;
+        NRR_CUDA(cudaGetDevice(&dev));
+        cudaMemPool_t pool;
+        NRR_CUDA(cudaDeviceGetDefaultMemPool(&pool, dev));
+        unsigned long long keep = ~0ull;      // keep freed scratch cached in the pool: reuse without re-mapping
+        NRR_CUDA(cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep));
+        t_pool_configured = true;
+    }
+    if (!t_err_flag) {
+        NRR_CUDA(cudaMalloc((void **)&t_err_flag, sizeof(unsigned int)));
+        NRR_CUDA(cudaMemset(t_err_flag, 0, sizeof(unsigned int)));
+    }
+    if (!t_pinned) NRR_CUDA(cudaMallocHost(&t_pinned, kPinnedBytes));
+    return NRR_OK;
+}
+
+struct Span {      // brackets a phase with events when profiling is on
+    int phase;
+    cudaStream_t stream;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    Span(int p, cudaStream_t s) : phase(p), stream(s)
+    {
+        if (!t_profile) return;
+        if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) { e0 = e1 = nullptr; return; }
+        cudaEventRecord(e0, stream);
+    }
+    void stop()
+    {
+        if (!e0) return;
+        cudaEventRecord(e1, stream);
+        if (!t_spans) t_spans = new std::vector<TimedSpan>();
+        t_spans->push_back({phase, e0, e1});
+        e0 = e1 = nullptr;
+    }
+};
+
+int fail(int code, const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(t_error, sizeof(t_error), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+Int3 i3(const int v[3]) { return Int3{v[0], v[1], v[2]}; }
+
+int check_dims_block(const int dims[3], const int block[3])
+{
+    if (!dims || !block) return fail(NRR_E_NULL, "dims/block is NULL");
+    for (int a = 0; a < 3; ++a) {
+        if (dims[a] < 1) return fail(NRR_E_DIMS, "dims[%d] = %d < 1", a, dims[a]);
+        if (block[a] < 1 || (block[a] & 1) == 0)
+            return fail(NRR_E_BLOCK, "block[%d] = %d must be a positive odd edge length", a, block[a]);
+        if (block[a] > dims[a]) return fail(NRR_E_DIMS, "block[%d] = %d exceeds dims[%d] = %d", a, block[a], a, dims[a]);
+    }
+    return NRR_OK;
+}
+
+int check_select_args(const float *fixed, const int dims[3], const int block[3], const int stride[3], double frac,
+                      const int *out_blocks, int capacity, const int *out_n)
+{
+    if (!fixed || !out_n || !stride) return fail(NRR_E_NULL, "fixed/stride/out_n is NULL");
+    int rc = check_dims_block(dims, block);
+    if (rc) return rc;
+    for (int a = 0; a < 3; ++a)
+        if (stride[a] < 1) return fail(NRR_E_STRIDE, "stride[%d] = %d < 1", a, stride[a]);
+    if (!(frac > 0.0 && frac <= 1.0)) return fail(NRR_E_FRAC, "frac = %g outside (0, 1]", frac);
+    if (capacity < 0) return fail(NRR_E_ARG, "capacity = %d < 0", capacity);
+    if (capacity > 0 && !out_blocks) return fail(NRR_E_NULL, "out_blocks is NULL with capacity > 0");
+    return NRR_OK;
+}
+
+int check_match_args(const float *fixed, const float *moving, const int dims[3], const int *blocks, int n,
+                     const int block[3], const int window[3], const int *out_disp, const float *out_ncc)
+{
+    if (!fixed || !moving || !window) return fail(NRR_E_NULL, "fixed/moving/window is NULL");
+    int rc = check_dims_block(dims, block);
+    if (rc) return rc;
+    for (int a = 0; a < 3; ++a)
+        if (window[a] < 0) return fail(NRR_E_WINDOW, "window[%d] = %d < 0", a, window[a]);
+    if (n < 0) return fail(NRR_E_ARG, "n = %d < 0", n);
+    if (n > 0 && (!blocks || !out_disp || !out_ncc)) return fail(NRR_E_NULL, "blocks/out_disp/out_ncc is NULL with n > 0");
+    return NRR_OK;
+}
+
+Int3 grid_of(const int dims[3], const int block[3], const int stride[3])
+{
+    Int3 g;
+    g.x = (dims[0] - block[0]) / stride[0] + 1;
+    g.y = (dims[1] - block[1]) / stride[1] + 1;
+    g.z = (dims[2] - block[2]) / stride[2] + 1;
+    return g;
+}
+
+// Device select; returns K through *out_n after one synchronisation.
+int select_device(const float *fixed, const int dims[3], const int block[3], const int stride[3], double frac,
+                  const unsigned char *mask, int *out_blocks, int capacity, int *out_n, double *out_var,
+                  int *out_ncand, cudaStream_t stream)
+{
+    int rc = ensure_thread_state();
+    if (rc) return rc;
+    const Int3 g = grid_of(dims, block, stride);
+    const long long ngrid = (long long)g.x * g.y * g.z;
+    if (ngrid > 0x7fffffffll) return fail(NRR_E_DIMS, "stride grid has %lld positions (limit 2^31-1)", ngrid);
+    void *scratch = nullptr;
+    NRR_CUDA(cudaMallocAsync(&scratch, select_scratch_bytes(ngrid), stream));
+    SelectState *st = nullptr;
+    Span span(0, stream);
+    rc = select_enqueue(fixed, i3(dims), i3(block), i3(stride), g, frac, mask, out_blocks, capacity, out_var, scratch,
+                        &st, stream);
+    span.stop();
+    if (rc) { cudaFreeAsync(scratch, stream); return rc; }
+    SelectState *h = (SelectState *)t_pinned;
+    NRR_CUDA(cudaMemcpyAsync(h, st, sizeof(SelectState), cudaMemcpyDeviceToHost, stream));
+    NRR_CUDA(cudaFreeAsync(scratch, stream));
+    NRR_CUDA(cudaStreamSynchronize(stream));
+    *out_n = (int)h->k;
+    if (out_ncand) *out_ncand = (int)h->n_candidates;
+    if ((int)h->k > capacity)
+        return fail(NRR_E_CAPACITY, "K = %u selected blocks exceed capacity = %d", h->k, capacity);
+    return NRR_OK;
+}
+
+int match_device(const float *fixed, const float *moving, const int dims[3], const int *blocks, int n,
+                 const int block[3], const int window[3], int *out_disp, float *out_ncc, cudaStream_t stream)
+{
+    int rc = ensure_thread_state();
+    if (rc) return rc;
+    if (n == 0) return NRR_OK;
+    MatchPlan plan;
+    rc = match_plan(i3(dims), i3(block), i3(window), moving, fixed, &plan);
+    if (rc) return rc;
+    const size_t nvox = (size_t)dims[0] * dims[1] * dims[2];
+    float *inv_sd = nullptr;
+    NRR_CUDA(cudaMallocAsync((void **)&inv_sd, nvox * sizeof(float), stream));
+    Span s1(1, stream);
+    rc = boxstat_enqueue(moving, i3(dims), i3(block), inv_sd, stream);
+    s1.stop();
+    if (rc == NRR_OK) {
+        Span s2(2, stream);
+        rc = match_enqueue(fixed, moving, inv_sd, i3(dims), blocks, n, i3(block), i3(window), out_disp, out_ncc,
+                           t_err_flag, stream);
+        s2.stop();
+    }
+    cudaError_t e = cudaFreeAsync(inv_sd, stream);
+    if (rc == NRR_OK && e != cudaSuccess) return cuda_fail(e, "cudaFreeAsync");
+    return rc;
+}
+
+int check_async(cudaStream_t stream)
+{
+    int rc = ensure_thread_state();
+    if (rc) return rc;
+    unsigned int *h = (unsigned int *)((char *)t_pinned + 1024);
+    NRR_CUDA(cudaMemcpyAsync(h, t_err_flag, sizeof(unsigned int), cudaMemcpyDeviceToHost, stream));
+    NRR_CUDA(cudaMemsetAsync(t_err_flag, 0, sizeof(unsigned int), stream));
+    NRR_CUDA(cudaStreamSynchronize(stream));
+    if (*h) return fail(NRR_E_BOUNDS, "a supplied block leaves the volume");
+    return NRR_OK;
+}
+
+int host_stream(cudaStream_t *s)
+{
+    if (!t_host_stream) NRR_CUDA(cudaStreamCreateWithFlags(&t_host_stream, cudaStreamNonBlocking));
+    *s = t_host_stream;
+    return NRR_OK;
+}
+
+struct DevBuf {     // stream-ordered device buffer released on scope exit
+    void *p = nullptr;
+    cudaStream_t s;
+    explicit DevBuf(cudaStream_t st) : s(st) {}
+    ~DevBuf() { if (p) cudaFreeAsync(p, s); }
+    cudaError_t alloc(size_t bytes) { return cudaMallocAsync(&p, bytes ? bytes : 1, s); }
+    cudaError_t upload(const void *h, size_t bytes)
+    {
+        cudaError_t e = alloc(bytes);
+        if (e != cudaSuccess) return e;
+        return cudaMemcpyAsync(p, h, bytes, cudaMemcpyHostToDevice, s);
+    }
+};
+
+}  // namespace
+
+void set_error(const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(t_error, sizeof(t_error), fmt, ap);
+    va_end(ap);
+}
+
+int cuda_fail(cudaError_t e, const char *what)
+{
+    snprintf(t_error, sizeof(t_error), "CUDA error %d (%s) in %s", (int)e, cudaGetErrorString(e), what);
+    return NRR_E_CUDA;
+}
+
+void count_launch(int n) { t_launches += n; }
+
+}  // namespace nrr
+
+using namespace nrr;
+
+extern "C" {
+
+int nrr_bm_select_blocks(const float *fixed, const int dims[3], const int block[3], const int stride[3], double frac,
+                         const unsigned char *mask, int *out_blocks, int capacity, int *out_n, double *out_var,
+                         int *out_ncand, void *stream)
+{
+    int rc = check_select_args(fixed, dims, block, stride, frac, out_blocks, capacity, out_n);
+    if (rc) return rc;
+    return select_device(fixed, dims, block, stride, frac, mask, out_blocks, capacity, out_n, out_var, out_ncand,
+                         (cudaStream_t)stream);
+}
+
+int nrr_bm_match(const float *fixed, const float *moving, const int dims[3], const int *blocks, int n,
+                 const int block[3], const int window[3], int *out_disp, float *out_ncc, void *stream)
+{
+    int rc = check_match_args(fixed, moving, dims, blocks, n, block, window, out_disp, out_ncc);
+    if (rc) return rc;
+    return match_device(fixed, moving, dims, blocks, n, block, window, out_disp, out_ncc, (cudaStream_t)stream);
+}
+
+int nrr_bm_check_async_error(void *stream) { return check_async((cudaStream_t)stream); }
+
+int nrr_bm_select_blocks_host(const float *fixed, const int dims[3], const int block[3], const int stride[3],
+                              double frac, const unsigned char *mask, int *out_blocks, int capacity, int *out_n,
+                              double *out_var, int *out_ncand)
+{
+    int rc = check_select_args(fixed, dims, block, stride, frac, out_blocks, capacity, out_n);
+    if (rc) return rc;
+    cudaStream_t s;
+    if ((rc = host_stream(&s))) return rc;
+    const size_t nvox = (size_t)dims[0] * dims[1] * dims[2];
+    DevBuf d_fixed(s), d_mask(s), d_blocks(s), d_var(s);
+    NRR_CUDA(d_fixed.upload(fixed, nvox * sizeof(float)));
+    if (mask) NRR_CUDA(d_mask.upload(mask, nvox));
+    NRR_CUDA(d_blocks.alloc((size_t)capacity * 3 * sizeof(int)));
+    if (out_var) NRR_CUDA(d_var.alloc((size_t)capacity * sizeof(double)));
+    rc = select_device((const float *)d_fixed.p, dims, block, stride, frac, (const unsigned char *)d_mask.p,
+                       (int *)d_blocks.p, capacity, out_n, (double *)d_var.p, out_ncand, s);
+    if (rc != NRR_OK && rc != NRR_E_CAPACITY) return rc;
+    const size_t k = (size_t)(*out_n < capacity ? *out_n : capacity);
+    NRR_CUDA(cudaMemcpyAsync(out_blocks, d_blocks.p, k * 3 * sizeof(int), cudaMemcpyDeviceToHost, s));
+    if (out_var) NRR_CUDA(cudaMemcpyAsync(out_var, d_var.p, k * sizeof(double), cudaMemcpyDeviceToHost, s));
+    NRR_CUDA(cudaStreamSynchronize(s));
+    return rc;
+}
+
+int nrr_bm_match_host(const float *fixed, const float *moving, const int dims[3], const int *blocks, int n,
+                      const int block[3], const int window[3], int *out_disp, float *out_ncc)
+{
+    int rc = check_match_args(fixed, moving, dims, blocks, n, block, window, out_disp, out_ncc);
+    if (rc) return rc;
+    if (n == 0) return NRR_OK;
+    cudaStream_t s;
+    if ((rc = host_stream(&s))) return rc;
+    const size_t nvox = (size_t)dims[0] * dims[1] * dims[2];
+    DevBuf d_fixed(s), d_moving(s), d_blocks(s), d_disp(s), d_ncc(s);
+    NRR_CUDA(d_fixed.upload(fixed, nvox * sizeof(float)));
+    NRR_CUDA(d_moving.upload(moving, nvox * sizeof(float)));
+    NRR_CUDA(d_blocks.upload(blocks, (size_t)n * 3 * sizeof(int)));
+    NRR_CUDA(d_disp.alloc((size_t)n * 3 * sizeof(int)));
+    NRR_CUDA(d_ncc.alloc((size_t)n * sizeof(float)));
+    rc = match_device((const float *)d_fixed.p, (const float *)d_moving.p, dims, (const int *)d_blocks.p, n, block,
+                      window, (int *)d_disp.p, (float *)d_ncc.p, s);
+    if (rc) return rc;
+    NRR_CUDA(cudaMemcpyAsync(out_disp, d_disp.p, (size_t)n * 3 * sizeof(int), cudaMemcpyDeviceToHost, s));
+    NRR_CUDA(cudaMemcpyAsync(out_ncc, d_ncc.p, (size_t)n * sizeof(float), cudaMemcpyDeviceToHost, s));
+    return check_async(s);
+}
+
+int nrr_bm_register_host(const float *fixed, const float *moving, const int dims[3], const int block[3],
+                         const int stride[3], const int window[3], double frac, const unsigned char *mask,
+                         int *out_blocks, int capacity, int *out_n, int *out_disp, float *out_ncc)
+{
+    int rc = check_select_args(fixed, dims, block, stride, frac, out_blocks, capacity, out_n);
+    if (rc) return rc;
+    if (!moving || !window) return fail(NRR_E_NULL, "moving/window is NULL");
+    for (int a = 0; a < 3; ++a)
+        if (window[a] < 0) return fail(NRR_E_WINDOW, "window[%d] = %d < 0", a, window[a]);
+    if (capacity > 0 && (!out_disp || !out_ncc)) return fail(NRR_E_NULL, "out_disp/out_ncc is NULL with capacity > 0");
+    cudaStream_t s;
+    if ((rc = host_stream(&s))) return rc;
+    const size_t nvox = (size_t)dims[0] * dims[1] * dims[2];
+    DevBuf d_fixed(s), d_moving(s), d_mask(s), d_blocks(s), d_disp(s), d_ncc(s);
+    NRR_CUDA(d_fixed.upload(fixed, nvox * sizeof(float)));
+    if (mask) NRR_CUDA(d_mask.upload(mask, nvox));
+    NRR_CUDA(d_moving.upload(moving, nvox * sizeof(float)));      // overlaps the selection kernels' queueing
+    NRR_CUDA(d_blocks.alloc((size_t)capacity * 3 * sizeof(int)));
+    rc = select_device((const float *)d_fixed.p, dims, block, stride, frac, (const unsigned char *)d_mask.p,
+                       (int *)d_blocks.p, capacity, out_n, nullptr, nullptr, s);
+    if (rc) return rc;
+    const int n = *out_n;
+    if (n == 0) return NRR_OK;
+    NRR_CUDA(d_disp.alloc((size_t)n * 3 * sizeof(int)));
+    NRR_CUDA(d_ncc.alloc((size_t)n * sizeof(float)));
+    rc = match_device((const float *)d_fixed.p, (const float *)d_moving.p, dims, (const int *)d_blocks.p, n, block,
+                      window, (int *)d_disp.p, (float *)d_ncc.p, s);
+    if (rc) return rc;
+    NRR_CUDA(cudaMemcpyAsync(out_blocks, d_blocks.p, (size_t)n * 3 * sizeof(int), cudaMemcpyDeviceToHost, s));
+    NRR_CUDA(cudaMemcpyAsync(out_disp, d_disp.p, (size_t)n * 3 * sizeof(int), cudaMemcpyDeviceToHost, s));
+    NRR_CUDA(cudaMemcpyAsync(out_ncc, d_ncc.p, (size_t)n * sizeof(float), cudaMemcpyDeviceToHost, s));
+    return check_async(s);
+}
+
+int nrr_bm_profile_enable(int on)
+{
+    t_profile = on ? 1 : 0;
+    return NRR_OK;
+}
+
+int nrr_bm_profile_read(double ms[3], int calls[3])
+{
+    if (!ms || !calls) return fail(NRR_E_NULL, "ms/calls is NULL");
+    for (int i = 0; i < 3; ++i) { ms[i] = 0.0; calls[i] = 0; }
+    if (!t_spans) return NRR_OK;
+    int rc = NRR_OK;
+    for (TimedSpan &sp : *t_spans) {
+        float t = 0.f;
+        cudaError_t e = cudaEventSynchronize(sp.e1);
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&t, sp.e0, sp.e1);
+        if (e != cudaSuccess) rc = cuda_fail(e, "profile events");
+        else if (sp.phase >= 0 && sp.phase < 3) { ms[sp.phase] += (double)t; calls[sp.phase] += 1; }
+        cudaEventDestroy(sp.e0);
+        cudaEventDestroy(sp.e1);
+    }
+    t_spans->clear();
+    return rc;
+}
+
+long long nrr_bm_launch_count(int reset)
+{
+    long long v = t_launches;
+    if (reset) t_launches = 0;
+    return v;
+}
+
+int nrr_bm_match_info(const int dims[3], const int block[3], const int window[3], int info[5])
+{
+    if (!info || !window) return fail(NRR_E_NULL, "info/window is NULL");
+    int rc = check_dims_block(dims, block);
+    if (rc) return rc;
+    for (int a = 0; a < 3; ++a)
+        if (window[a] < 0) return fail(NRR_E_WINDOW, "window[%d] = %d < 0", a, window[a]);
+    MatchPlan plan;
+    memset(&plan, 0, sizeof(plan));
+    rc = match_plan(i3(dims), i3(block), i3(window), nullptr, nullptr, &plan);
+    if (rc) return rc;
+    info[0] = plan.fast; info[1] = plan.threads; info[2] = plan.smem_bytes; info[3] = plan.tma; info[4] = plan.candidates;
+    return NRR_OK;
+}
+
+int nrr_bm_fp32_peak(double *out_tflops, void *stream)
+{
+    if (!out_tflops) return fail(NRR_E_NULL, "out_tflops is NULL");
+    return fp32_peak_measure(out_tflops, (cudaStream_t)stream);
+}
+
+int nrr_bm_set_option(const char *name, double value)
+{
+    if (!name) return fail(NRR_E_NULL, "name is NULL");
+    if (!strcmp(name, "tie_band")) { g_tie_band = (float)value; return NRR_OK; }
+    if (!strcmp(name, "force_generic")) { g_force_generic = value != 0.0; return NRR_OK; }
+    if (!strcmp(name, "disable_tma")) { g_disable_tma = value != 0.0; return NRR_OK; }
+    return fail(NRR_E_ARG, "unknown option '%s'", name);
+}
+
+const char *nrr_bm_last_error(void) { return t_error; }
+
+const char *nrr_bm_status_string(int status)
+{
+    switch (status) {
+    case NRR_OK: return "NRR_OK";
+    case NRR_E_NULL: return "NRR_E_NULL";
+    case NRR_E_DIMS: return "NRR_E_DIMS";
+    case NRR_E_BLOCK: return "NRR_E_BLOCK";
+    case NRR_E_STRIDE: return "NRR_E_STRIDE";
+    case NRR_E_WINDOW: return "NRR_E_WINDOW";
+    case NRR_E_FRAC: return "NRR_E_FRAC";
+    case NRR_E_CAPACITY: return "NRR_E_CAPACITY";
+    case NRR_E_BOUNDS: return "NRR_E_BOUNDS";
+    case NRR_E_SMEM: return "NRR_E_SMEM";
+    case NRR_E_CUDA: return "NRR_E_CUDA";
+    case NRR_E_ARG: return "NRR_E_ARG";
+    default: return "NRR_E_UNKNOWN";
+    }
+}
+
+int nrr_bm_version(void) { return NRR_BM_VERSION; }
+
+}  // extern "C"

@@ -1,0 +1,72 @@
+// nrr_internal.cuh -- declarations shared by the translation units of libnrr_bm.so (CUDA path only).
+// Nothing here is shared with oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/nrr_bm.h"
+
+namespace nrr {
+
+struct Int3 { int x, y, z; };
+
+// ---- error plumbing (nrr_api.cu) --------------------------------------------------------------------
+void set_error(const char *fmt, ...);
+int cuda_fail(cudaError_t e, const char *what);   // records the message, returns NRR_E_CUDA
+void count_launch(int n = 1);
+
+#define NRR_CUDA(call)                                              \
+    do {                                                            \
+        cudaError_t e__ = (call);                                   \
+        if (e__ != cudaSuccess) return ::nrr::cuda_fail(e__, #call); \
+    } while (0)
+
+#define NRR_LAUNCH_CHECK(what)                                        \
+    do {                                                              \
+        cudaError_t e__ = cudaGetLastError();                         \
+        if (e__ != cudaSuccess) return ::nrr::cuda_fail(e__, what);   \
+        ::nrr::count_launch();                                        \
+    } while (0)
+
+// ---- selection (nrr_select.cu) ----------------------------------------------------------------------
+// Device-side state of one selection call; lives in library scratch.
+struct SelectState {
+    unsigned long long prefix;      // radix-select: key bits decided so far
+    unsigned long long mask;        // which bits of prefix are decided
+    unsigned int n_candidates;      // N: in-mask grid positions
+    unsigned int k;                 // K = floor(0.5 + N*frac)
+    unsigned int k_remaining;       // still to take inside the current prefix bucket
+    unsigned int ticket[8];         // last-CTA-done counters, one per kernel of the sequence
+    unsigned int total_selected;    // written by the compaction scan (== K)
+};
+
+size_t select_scratch_bytes(long long ngrid);
+// Enqueues the whole selection sequence. `scratch` must hold select_scratch_bytes(ngrid) bytes.
+int select_enqueue(const float *fixed, Int3 dims, Int3 block, Int3 stride, Int3 grid, double frac,
+                   const unsigned char *mask, int *out_blocks, int capacity, double *out_var,
+                   void *scratch, SelectState **state_out, cudaStream_t stream);
+
+// ---- moving-volume statistics (nrr_boxstat.cu) ------------------------------------------------------
+// inv_sd[p] = 1/sqrt(sum over the block with ORIGIN p of (m - mean)^2), 0 for zero-variance blocks,
+// for every origin p whose block fits in the volume; other entries are left untouched.
+int boxstat_enqueue(const float *moving, Int3 dims, Int3 block, float *inv_sd, cudaStream_t stream);
+
+// ---- matching (nrr_match.cu) ------------------------------------------------------------------------
+struct MatchPlan {
+    int fast;          // 1: register-tiled kernel, 0: generic kernel
+    int threads;
+    int smem_bytes;
+    int tma;           // 1: TMA staging
+    int candidates;
+};
+int match_plan(Int3 dims, Int3 block, Int3 window, const void *moving_ptr, const void *fixed_ptr,
+               MatchPlan *plan);
+int match_enqueue(const float *fixed, const float *moving, const float *inv_sd, Int3 dims, const int *blocks,
+                  int n, Int3 block, Int3 window, int *out_disp, float *out_ncc, unsigned int *err_flag,
+                  cudaStream_t stream);
+
+// ---- FFMA microbenchmark (nrr_fma_peak.cu) ----------------------------------------------------------
+int fp32_peak_measure(double *out_tflops, cudaStream_t stream);
+
+}  // namespace nrr

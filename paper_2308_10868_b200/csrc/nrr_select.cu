@@ -1,0 +1,366 @@
+// nrr_select.cu -- variance-based block selection on the device.
+//
+//   S1  block statistics : one thread per stride-grid position, two-pass population variance in IEEE
+//                          double with explicitly rounded (never contracted) operations, summed in
+//                          x-fastest order ("computes the variance within a block").
+//   S2  count            : K = floor(0.5 + N*frac) on the device with the same rounded operations
+//                          ("0.5 + NFeatures x Fs blocks are selected").
+//   S3  top-K            : most-significant-digit radix select over the 64-bit variance keys (6 passes of
+//                          11/11/11/11/11/9 bits) -> threshold T and the number of T-valued ties to keep
+//                          (lowest candidate index first), then an order-preserving compaction that emits
+//                          block centres in ascending candidate index.
+//
+// No CTA ever waits for another: every multi-CTA step ends with the "last CTA done" ticket pattern, so the
+// sequence cannot deadlock whatever the grid size.  All launches go to one stream; the caller synchronises
+// once to read K.
+#include "nrr_internal.cuh"
+
+namespace nrr {
+
+namespace {
+
+constexpr int kRadixBins = 2048;
+constexpr int kNumPasses = 6;
+__constant__ int c_shift[kNumPasses] = {53, 42, 31, 20, 9, 0};
+__constant__ int c_width[kNumPasses] = {11, 11, 11, 11, 11, 9};
+
+constexpr int kStatsThreads = 128;
+constexpr int kScanThreads = 256;
+constexpr int kItemsPerThread = 8;
+constexpr int kChunk = kScanThreads * kItemsPerThread;   // grid positions per CTA in the radix / compaction kernels
+
+// Monotone map variance -> unsigned key. Out-of-mask positions carry var = -1 and map to key 0, below every
+// candidate (a candidate's key is >= 1), so they can never be taken while K <= N.
+__device__ __forceinline__ unsigned long long key_of(double var)
+{
+    return var < 0.0 ? 0ull : (unsigned long long)__double_as_longlong(var) + 1ull;
+}
+
+__device__ __forceinline__ unsigned int digit_of(unsigned long long key, int pass)
+{
+    return (unsigned int)(key >> c_shift[pass]) & ((1u << c_width[pass]) - 1u);
+}
+
+// Block-wide: the calling CTA (all threads) picks the radix digit of pass `pass` that contains the
+// k_remaining-th largest key of the current prefix bucket, from the global histogram `hist`.
+__device__ void pick_digit(const unsigned int *hist, SelectState *st, int pass)
+{
+    __shared__ unsigned int s_warp[32];
+    __shared__ unsigned int s_found_bin, s_found_cum;
+    const int nbins = 1 << c_width[pass];
+    const int T = blockDim.x;
+    const int per = (nbins + T - 1) / T;
+    const int tid = threadIdx.x;
+    const unsigned int k = st->k_remaining;
+    // thread t owns the descending bins  top - t*per - i,  i in [0, per)
+    unsigned int local = 0;
+    for (int i = 0; i < per; ++i) {
+        int bin = nbins - 1 - (tid * per + i);
+        if (bin >= 0) local += __ldcg(hist + bin);
+    }
+    // inclusive scan of `local` over the CTA
+    unsigned int incl = local;
+    const int lane = tid & 31, warp = tid >> 5;
+    for (int o = 1; o < 32; o <<= 1) {
+        unsigned int v = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += v;
+    }
+    if (lane == 31) s_warp[warp] = incl;
+    if (tid == 0) { s_found_bin = (unsigned int)(nbins - 1); s_found_cum = 0; }
+    __syncthreads();
+    unsigned int base = 0;
+    for (int w = 0; w < warp; ++w) base += s_warp[w];
+    incl += base;
+    const unsigned int excl = incl - local;
+    if (k > 0 && excl < k && k <= incl) {
+        unsigned int cum = excl;
+        for (int i = 0; i < per; ++i) {
+            int bin = nbins - 1 - (tid * per + i);
+            if (bin < 0) break;
+            unsigned int c = __ldcg(hist + bin);
+            if (cum + c >= k) { s_found_bin = (unsigned int)bin; s_found_cum = cum; break; }
+            cum += c;
+        }
+    }
+    __syncthreads();
+    if (tid == 0) {
+        st->prefix |= (unsigned long long)s_found_bin << c_shift[pass];
+        st->mask |= (unsigned long long)((1u << c_width[pass]) - 1u) << c_shift[pass];
+        st->k_remaining = k - s_found_cum;
+    }
+}
+
+// Adds the CTA's shared histogram into the global one, then returns true in the last CTA to finish.
+__device__ bool flush_hist_and_ticket(unsigned int *s_hist, unsigned int *g_hist, unsigned int *ticket)
+{
+    __shared__ bool s_last;
+    __syncthreads();
+    for (int b = threadIdx.x; b < kRadixBins; b += blockDim.x) {
+        unsigned int c = s_hist[b];
+        if (c) atomicAdd(g_hist + b, c);
+    }
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) s_last = (atomicAdd(ticket, 1u) == gridDim.x - 1);
+    __syncthreads();
+    if (s_last) __threadfence();
+    return s_last;
+}
+
+// S1 + S2 + radix pass 0.
+__global__ void __launch_bounds__(kStatsThreads)
+stats_kernel(const float *__restrict__ fixed, Int3 dims, Int3 block, Int3 stride, Int3 grid, long long ngrid,
+             double frac, const unsigned char *__restrict__ mask, double *__restrict__ var,
+             unsigned int *hist0, SelectState *st)
+{
+    __shared__ unsigned int s_hist[kRadixBins];
+    for (int b = threadIdx.x; b < kRadixBins; b += kStatsThreads) s_hist[b] = 0;
+    __syncthreads();
+
+    const long long g = (long long)blockIdx.x * kStatsThreads + threadIdx.x;
+    bool in = false;
+    if (g < ngrid) {
+        const int i = (int)(g % grid.x);
+        const int j = (int)((g / grid.x) % grid.y);
+        const int k = (int)(g / ((long long)grid.x * grid.y));
+        const int ox = i * stride.x, oy = j * stride.y, oz = k * stride.z;
+        const int cx = ox + (block.x - 1) / 2, cy = oy + (block.y - 1) / 2, cz = oz + (block.z - 1) / 2;
+        in = (mask == nullptr) || mask[((size_t)cz * dims.y + cy) * dims.x + cx] != 0;
+        double v = -1.0;
+        if (in) {
+            const double nvox = (double)((long long)block.x * block.y * block.z);
+            double s = 0.0;
+            for (int z = 0; z < block.z; ++z)
+                for (int y = 0; y < block.y; ++y) {
+                    const float *row = fixed + ((size_t)(oz + z) * dims.y + (oy + y)) * dims.x + ox;
+                    for (int x = 0; x < block.x; ++x) s = __dadd_rn(s, (double)__ldg(row + x));
+                }
+            const double mean = __ddiv_rn(s, nvox);
+            double q = 0.0;
+            for (int z = 0; z < block.z; ++z)
+                for (int y = 0; y < block.y; ++y) {
+                    const float *row = fixed + ((size_t)(oz + z) * dims.y + (oy + y)) * dims.x + ox;
+                    for (int x = 0; x < block.x; ++x) {
+                        const double d = __dsub_rn((double)__ldg(row + x), mean);
+                        q = __dadd_rn(q, __dmul_rn(d, d));
+                    }
+                }
+            v = __ddiv_rn(q, nvox);
+            atomicAdd(&s_hist[digit_of(key_of(v), 0)], 1u);
+        }
+        var[g] = v;
+    }
+    const int cnt = __syncthreads_count(in ? 1 : 0);
+    if (threadIdx.x == 0 && cnt) atomicAdd(&st->n_candidates, (unsigned int)cnt);
+
+    if (flush_hist_and_ticket(s_hist, hist0, &st->ticket[0])) {
+        if (threadIdx.x == 0) {
+            const unsigned int n = *((volatile unsigned int *)&st->n_candidates);
+            // K = floor(0.5 + N*frac), product and sum rounded separately
+            double kd = floor(__dadd_rn(0.5, __dmul_rn((double)n, frac)));
+            unsigned int kk = kd <= 0.0 ? 0u : (kd >= (double)n ? n : (unsigned int)kd);
+            st->k = kk;
+            st->k_remaining = kk;
+            st->prefix = 0ull;
+            st->mask = 0ull;
+        }
+        __syncthreads();
+        pick_digit(hist0, st, 0);
+    }
+}
+
+// Radix passes 1..5: histogram of the next digit over the keys that match the decided prefix.
+__global__ void __launch_bounds__(kScanThreads)
+radix_pass_kernel(const double *__restrict__ var, long long ngrid, unsigned int *hist, SelectState *st, int pass)
+{
+    __shared__ unsigned int s_hist[kRadixBins];
+    for (int b = threadIdx.x; b < kRadixBins; b += kScanThreads) s_hist[b] = 0;
+    __syncthreads();
+    const unsigned long long prefix = st->prefix, mask = st->mask;
+    const long long base = (long long)blockIdx.x * kChunk;
+#pragma unroll
+    for (int i = 0; i < kItemsPerThread; ++i) {
+        const long long g = base + (long long)i * kScanThreads + threadIdx.x;
+        if (g < ngrid) {
+            const unsigned long long key = key_of(var[g]);
+            if ((key & mask) == prefix) atomicAdd(&s_hist[digit_of(key, pass)], 1u);
+        }
+    }
+    if (flush_hist_and_ticket(s_hist, hist, &st->ticket[pass])) pick_digit(hist, st, pass);
+}
+
+// Packs (#key > T, #key == T) of a run of grid positions into one 64-bit word so one scan carries both.
+__device__ __forceinline__ unsigned long long pack_counts(unsigned int gt, unsigned int eq)
+{
+    return ((unsigned long long)gt << 32) | eq;
+}
+
+__device__ unsigned long long block_exclusive_scan_u64(unsigned long long v, unsigned long long *total)
+{
+    __shared__ unsigned long long s_w[32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+    unsigned long long incl = v;
+    for (int o = 1; o < 32; o <<= 1) {
+        unsigned long long t = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += t;
+    }
+    __syncthreads();   // protect s_w against a previous use
+    if (lane == 31) s_w[warp] = incl;
+    __syncthreads();
+    unsigned long long base = 0, tot = 0;
+    for (int w = 0; w < nwarp; ++w) {
+        if (w < warp) base += s_w[w];
+        tot += s_w[w];
+    }
+    if (total) *total = tot;
+    return base + incl - v;
+}
+
+// Per-CTA counts of keys above / equal to the threshold; the last CTA turns them into exclusive offsets.
+__global__ void __launch_bounds__(kScanThreads)
+count_kernel(const double *__restrict__ var, long long ngrid, unsigned long long *cta_counts,
+             unsigned long long *cta_offsets, SelectState *st)
+{
+    const unsigned long long T = st->prefix;
+    const long long base = (long long)blockIdx.x * kChunk + (long long)threadIdx.x * kItemsPerThread;
+    unsigned int gt = 0, eq = 0;
+#pragma unroll
+    for (int i = 0; i < kItemsPerThread; ++i) {
+        const long long g = base + i;
+        if (g < ngrid) {
+            const unsigned long long key = key_of(var[g]);
+            gt += key > T;
+            eq += key == T;
+        }
+    }
+    unsigned long long tot;
+    block_exclusive_scan_u64(pack_counts(gt, eq), &tot);
+    __shared__ bool s_last;
+    if (threadIdx.x == 0) {
+        cta_counts[blockIdx.x] = tot;
+        __threadfence();
+        s_last = (atomicAdd(&st->ticket[6], 1u) == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    // exclusive scan over all CTA totals, kScanThreads at a time
+    __shared__ unsigned long long s_carry;
+    if (threadIdx.x == 0) s_carry = 0;
+    __syncthreads();
+    for (unsigned int start = 0; start < gridDim.x; start += kScanThreads) {
+        const unsigned int c = start + threadIdx.x;
+        const unsigned long long v = c < gridDim.x ? __ldcg(cta_counts + c) : 0ull;
+        unsigned long long t;
+        const unsigned long long ex = block_exclusive_scan_u64(v, &t);
+        const unsigned long long carry = s_carry;
+        if (c < gridDim.x) cta_offsets[c] = carry + ex;
+        __syncthreads();
+        if (threadIdx.x == 0) s_carry = carry + t;
+        __syncthreads();
+    }
+}
+
+// Order-preserving compaction: position of a kept candidate = #(key > T before it) + min(#(key == T before
+// it), ties), and a T-valued candidate is kept iff fewer than `ties` T-valued candidates precede it.
+__global__ void __launch_bounds__(kScanThreads)
+compact_kernel(const double *__restrict__ var, long long ngrid, Int3 block, Int3 stride, Int3 grid,
+               const unsigned long long *__restrict__ cta_offsets, const SelectState *st,
+               int *__restrict__ out_blocks, double *__restrict__ out_var, int capacity)
+{
+    const unsigned int K = st->k;
+    if (K == 0) return;
+    const unsigned long long T = st->prefix;
+    const unsigned int ties = st->k_remaining;
+    const long long base = (long long)blockIdx.x * kChunk + (long long)threadIdx.x * kItemsPerThread;
+    unsigned long long keys[kItemsPerThread];
+    unsigned int gt = 0, eq = 0;
+#pragma unroll
+    for (int i = 0; i < kItemsPerThread; ++i) {
+        const long long g = base + i;
+        keys[i] = g < ngrid ? key_of(var[g]) : 0ull;
+        gt += keys[i] > T;
+        eq += (keys[i] == T) && (g < ngrid);
+    }
+    const unsigned long long ex = block_exclusive_scan_u64(pack_counts(gt, eq), nullptr) + cta_offsets[blockIdx.x];
+    unsigned int gt_before = (unsigned int)(ex >> 32), eq_before = (unsigned int)(ex & 0xffffffffu);
+#pragma unroll
+    for (int i = 0; i < kItemsPerThread; ++i) {
+        const long long g = base + i;
+        if (g >= ngrid) break;
+        const bool is_gt = keys[i] > T, is_eq = keys[i] == T;
+        if (is_gt || (is_eq && eq_before < ties)) {
+            const unsigned int pos = gt_before + (eq_before < ties ? eq_before : ties);
+            if (pos < (unsigned int)capacity) {
+                const int gi = (int)(g % grid.x);
+                const int gj = (int)((g / grid.x) % grid.y);
+                const int gk = (int)(g / ((long long)grid.x * grid.y));
+                out_blocks[3 * (size_t)pos + 0] = gi * stride.x + (block.x - 1) / 2;
+                out_blocks[3 * (size_t)pos + 1] = gj * stride.y + (block.y - 1) / 2;
+                out_blocks[3 * (size_t)pos + 2] = gk * stride.z + (block.z - 1) / 2;
+                if (out_var) out_var[pos] = var[g];
+            }
+        }
+        gt_before += is_gt;
+        eq_before += is_eq;
+    }
+}
+
+struct ScratchLayout {
+    size_t state, hist, var, counts, offsets, total;
+};
+
+ScratchLayout layout(long long ngrid)
+{
+    ScratchLayout L;
+    const size_t nchunks = (size_t)((ngrid + kChunk - 1) / kChunk) + 1;
+    size_t off = 0;
+    L.state = off;   off += 256;                                            // SelectState (zeroed per call)
+    L.hist = off;    off += sizeof(unsigned int) * kRadixBins * kNumPasses; // zeroed per call
+    L.var = off;     off += sizeof(double) * (size_t)(ngrid > 0 ? ngrid : 1);
+    L.counts = off;  off += sizeof(unsigned long long) * nchunks;
+    L.offsets = off; off += sizeof(unsigned long long) * nchunks;
+    L.total = off;
+    return L;
+}
+
+}  // namespace
+
+size_t select_scratch_bytes(long long ngrid) { return layout(ngrid).total; }
+
+int select_enqueue(const float *fixed, Int3 dims, Int3 block, Int3 stride, Int3 grid, double frac,
+                   const unsigned char *mask, int *out_blocks, int capacity, double *out_var, void *scratch,
+                   SelectState **state_out, cudaStream_t stream)
+{
+    static_assert(sizeof(SelectState) <= 256, "SelectState must fit its scratch slot");
+    const long long ngrid = (long long)grid.x * grid.y * grid.z;
+    const ScratchLayout L = layout(ngrid);
+    char *base = (char *)scratch;
+    SelectState *st = (SelectState *)(base + L.state);
+    unsigned int *hist = (unsigned int *)(base + L.hist);
+    double *var = (double *)(base + L.var);
+    unsigned long long *counts = (unsigned long long *)(base + L.counts);
+    unsigned long long *offsets = (unsigned long long *)(base + L.offsets);
+    *state_out = st;
+
+    NRR_CUDA(cudaMemsetAsync(base, 0, L.var, stream));   // state + histograms
+    if (ngrid == 0) return NRR_OK;
+
+    const unsigned int stats_ctas = (unsigned int)((ngrid + kStatsThreads - 1) / kStatsThreads);
+    stats_kernel<<<stats_ctas, kStatsThreads, 0, stream>>>(fixed, dims, block, stride, grid, ngrid, frac, mask,
+                                                           var, hist, st);
+    NRR_LAUNCH_CHECK("stats_kernel");
+    const unsigned int chunks = (unsigned int)((ngrid + kChunk - 1) / kChunk);
+    for (int pass = 1; pass < kNumPasses; ++pass) {
+        radix_pass_kernel<<<chunks, kScanThreads, 0, stream>>>(var, ngrid, hist + (size_t)pass * kRadixBins, st, pass);
+        NRR_LAUNCH_CHECK("radix_pass_kernel");
+    }
+    count_kernel<<<chunks, kScanThreads, 0, stream>>>(var, ngrid, counts, offsets, st);
+    NRR_LAUNCH_CHECK("count_kernel");
+    compact_kernel<<<chunks, kScanThreads, 0, stream>>>(var, ngrid, block, stride, grid, offsets, st, out_blocks,
+                                                        out_var, capacity);
+    NRR_LAUNCH_CHECK("compact_kernel");
+    return NRR_OK;
+}
+
+}  // namespace nrr

@@ -1,0 +1,276 @@
+"""GPU parity tests (-m gpu): the CUDA path, called through the C ABI, against the CPU oracle, element by
+element on the same seeded inputs.  Sizes span several tiles and ragged tails; the BASELINE.json configs run
+at full size (config 4 and the 32-setting batch on sampled blocks the oracle computes one by one)."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+import oracle                                    # noqa: E402  (test infrastructure)
+import paper_2308_10868_b200 as nrr             # noqa: E402  (product)
+from nrr_inputs import CONFIGS, batch_settings, make_pair, spherical_mask   # noqa: E402
+from _parity import assert_match_parity, assert_select_parity               # noqa: E402
+
+
+def _cuda(a):
+    return None if a is None else torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _smooth(dims, seed, sigma=1.5):
+    from scipy import ndimage
+    nx, ny, nz = dims
+    v = ndimage.gaussian_filter(np.random.default_rng(seed).standard_normal((nz, ny, nx)), sigma, mode="reflect")
+    return ((v - v.min()) / (v.max() - v.min()) * 1000.0).astype(np.float32)
+
+
+def _shift_noise(vol, s, noise, seed):
+    nz, ny, nx = vol.shape
+    iz = np.clip(np.arange(nz) - s[2], 0, nz - 1)
+    iy = np.clip(np.arange(ny) - s[1], 0, ny - 1)
+    ix = np.clip(np.arange(nx) - s[0], 0, nx - 1)
+    m = vol[np.ix_(iz, iy, ix)].astype(np.float64)
+    m = m + np.random.default_rng(seed).normal(0, noise, size=m.shape)
+    return np.ascontiguousarray(m, dtype=np.float32)
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _require_cuda():
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    nrr.lib()      # fails loudly if libnrr_bm.so is missing: there is no fallback
+    yield
+
+
+_pairs = {}
+
+
+def pair(name):
+    if name not in _pairs:
+        _pairs[name] = make_pair(CONFIGS[name])
+    return _pairs[name]
+
+
+# ------------------------------------------------------------------------------------------- selection
+@pytest.mark.parametrize("dims,block,stride,frac,mask_r", [
+    ((41, 37, 29), (5, 5, 5), (5, 5, 5), 0.30, None),
+    ((41, 37, 29), (7, 7, 7), (5, 5, 5), 0.25, 15.0),
+    ((41, 37, 29), (3, 5, 7), (4, 3, 2), 0.50, 15.0),
+    ((41, 37, 29), (9, 9, 9), (6, 6, 6), 1.00, None),
+    ((64, 50, 33), (5, 5, 5), (1, 1, 1), 0.05, 20.0),       # dense grid: many chunks, ragged tail
+    ((130, 3, 3), (3, 3, 3), (1, 1, 1), 0.10, None),         # degenerate thin volume
+    ((9, 9, 9), (9, 9, 9), (1, 1, 1), 1.00, None),           # a single candidate
+])
+def test_select_parity_small(dims, block, stride, frac, mask_r):
+    vol = _smooth(dims, 100 + dims[0])
+    mask = None if mask_r is None else spherical_mask(dims, mask_r)
+    ora = oracle.select(vol, block, stride, frac, mask)
+    blocks, n, ncand, var = nrr.nrr_bm_select_blocks(_cuda(vol), block, stride, frac, _cuda(mask), want_var=True)
+    assert_select_parity(blocks.cpu().numpy(), n, ncand, ora, var.cpu().numpy())
+
+
+def test_select_uniform_image_and_exact_ties():
+    vol = np.full((12, 15, 20), 42.0, dtype=np.float32)
+    ora = oracle.select(vol, (3, 3, 3), (3, 3, 3), 0.25)
+    blocks, n, ncand, var = nrr.nrr_bm_select_blocks(_cuda(vol), (3, 3, 3), (3, 3, 3), 0.25, want_var=True)
+    assert_select_parity(blocks.cpu().numpy(), n, ncand, ora, var.cpu().numpy())
+    vol2 = np.zeros((6, 6, 18), dtype=np.float32)
+    pat = np.arange(27, dtype=np.float32).reshape(3, 3, 3)
+    vol2[0:3, 0:3, 3:6] = pat
+    vol2[3:6, 3:6, 12:15] = pat
+    for frac in (1.0 / 24.0, 2.0 / 24.0, 3.0 / 24.0):
+        ora = oracle.select(vol2, (3, 3, 3), (3, 3, 3), frac)
+        blocks, n, ncand = nrr.nrr_bm_select_blocks(_cuda(vol2), (3, 3, 3), (3, 3, 3), frac)
+        assert_select_parity(blocks.cpu().numpy(), n, ncand, ora)
+
+
+def test_select_mask_excluding_everything_and_capacity_error():
+    vol = _smooth((20, 20, 20), 7)
+    mask = np.zeros_like(vol, dtype=np.uint8)
+    blocks, n, ncand = nrr.nrr_bm_select_blocks(_cuda(vol), (5, 5, 5), (5, 5, 5), 0.5, _cuda(mask))
+    assert n == 0 and ncand == 0 and blocks.shape[0] == 0
+    with pytest.raises(nrr.NrrError) as ei:
+        nrr.nrr_bm_select_blocks(_cuda(vol), (5, 5, 5), (5, 5, 5), 0.5, capacity=3)
+    assert ei.value.status == -7
+
+
+@pytest.mark.parametrize("name", ["tiny", "intraop", "fullres", "highres"])
+def test_select_parity_configs(name):
+    cfg = CONFIGS[name]
+    fixed, _, mask = pair(name)
+    ora = oracle.select(fixed, cfg.block, cfg.stride, cfg.frac, mask)
+    blocks, n, ncand, var = nrr.nrr_bm_select_blocks(_cuda(fixed), cfg.block, cfg.stride, cfg.frac, _cuda(mask), want_var=True)
+    assert_select_parity(blocks.cpu().numpy(), n, ncand, ora, var.cpu().numpy())
+    print("%s: N=%d K=%d oracle K/K+1 variance margin %.3g" % (name, ncand, n, ora["margin"]))
+
+
+# ------------------------------------------------------------------------------------------- matching
+def _match_case(dims, block, window, shift, noise, seed, stride=None, frac=1.0, expect_fast=None):
+    vol = _smooth(dims, seed)
+    mov = _shift_noise(vol, shift, noise, seed + 1)
+    sel = oracle.select(vol, block, stride or block, frac)
+    ora = oracle.match(vol, mov, sel["centres"], block, window)
+    info = nrr.nrr_bm_match_info(dims, block, window)
+    if expect_fast is not None:
+        assert info["fast"] == expect_fast, info
+    disp, ncc = nrr.nrr_bm_match(_cuda(vol), _cuda(mov), _cuda(sel["centres"]), block, window)
+    nrr.nrr_bm_check_async_error()
+    return assert_match_parity(disp.cpu().numpy(), ncc.cpu().numpy(), ora, label=str((dims, block, window))), len(sel["centres"])
+
+
+@pytest.mark.parametrize("dims,block,window,fast", [
+    ((40, 36, 24), (5, 5, 5), (3, 3, 3), True),      # nx % 4 == 0: TMA staging; every grid block incl. borders
+    ((41, 37, 29), (5, 5, 5), (3, 3, 3), True),      # nx % 4 != 0: plain-load staging
+    ((48, 40, 30), (7, 7, 7), (5, 5, 3), True),      # config-2 shape of window
+    ((45, 43, 31), (7, 7, 7), (5, 5, 5), True),
+    ((44, 40, 36), (9, 9, 9), (3, 3, 2), True),
+    ((40, 40, 40), (11, 11, 11), (3, 3, 3), True),
+    ((36, 32, 28), (5, 5, 5), (7, 7, 1), True),
+    ((40, 36, 24), (3, 5, 3), (2, 1, 3), False),     # anisotropic: generic kernel
+    ((33, 31, 29), (7, 7, 7), (4, 4, 4), False),     # window without a fast instantiation
+    ((30, 30, 30), (5, 5, 5), (0, 0, 0), False),     # single candidate
+])
+def test_match_parity_small(dims, block, window, fast):
+    exempt, n = _match_case(dims, block, window, (1, -1, 1), 20.0, 200 + dims[0], expect_fast=fast)
+    print("%s %s %s: %d blocks, %d exempt" % (dims, block, window, n, exempt))
+
+
+def test_match_generic_equals_fast_kernel():
+    dims, block, window = (48, 44, 40), (7, 7, 7), (5, 5, 5)
+    vol = _smooth(dims, 31)
+    mov = _shift_noise(vol, (2, 1, -2), 25.0, 32)
+    sel = oracle.select(vol, block, (5, 5, 5), 0.5)
+    c = _cuda(sel["centres"])
+    d1, n1 = nrr.nrr_bm_match(_cuda(vol), _cuda(mov), c, block, window)
+    nrr.nrr_bm_set_option("force_generic", 1)
+    try:
+        d2, n2 = nrr.nrr_bm_match(_cuda(vol), _cuda(mov), c, block, window)
+    finally:
+        nrr.nrr_bm_set_option("force_generic", 0)
+    nrr.nrr_bm_set_option("disable_tma", 1)
+    try:
+        d3, n3 = nrr.nrr_bm_match(_cuda(vol), _cuda(mov), c, block, window)
+    finally:
+        nrr.nrr_bm_set_option("disable_tma", 0)
+    ora = oracle.match(vol, mov, sel["centres"], block, window)
+    for d, n_, lab in ((d1, n1, "fast+tma"), (d2, n2, "generic"), (d3, n3, "fast, plain staging")):
+        assert_match_parity(d.cpu().numpy(), n_.cpu().numpy(), ora, label=lab)
+    assert torch.equal(d1, d3) and torch.equal(n1, n3)      # staging path must not change a bit
+
+
+def test_match_largest_fast_instantiation():
+    dims, block, window = (64, 60, 56), (11, 11, 11), (9, 9, 9)
+    vol = _smooth(dims, 41, sigma=2.0)
+    mov = _shift_noise(vol, (4, -6, 5), 15.0, 42)
+    sel = oracle.select(vol, block, (9, 9, 9), 0.4)
+    ora = oracle.match(vol, mov, sel["centres"], block, window)
+    assert nrr.nrr_bm_match_info(dims, block, window)["fast"]
+    disp, ncc = nrr.nrr_bm_match(_cuda(vol), _cuda(mov), _cuda(sel["centres"]), block, window)
+    assert_match_parity(disp.cpu().numpy(), ncc.cpu().numpy(), ora)
+
+
+def test_match_exact_ties_and_constant_regions():
+    # period-2 volume along x: dx = -2, 0, +2 are bit-identical candidates -> lowest linear index wins
+    base = np.random.default_rng(15).uniform(0, 1000, size=(9, 9, 2)).astype(np.float32)
+    vol = np.ascontiguousarray(np.tile(base, (1, 1, 8)))
+    centres = np.asarray([[8, 4, 4], [6, 4, 4]], dtype=np.int32)
+    ora = oracle.match(vol, vol, centres, (3, 3, 3), (2, 0, 0))
+    disp, ncc = nrr.nrr_bm_match(_cuda(vol), _cuda(vol), _cuda(centres), (3, 3, 3), (2, 0, 0))
+    assert disp.cpu().numpy().tolist() == ora["disp"].tolist() == [[-2, 0, 0], [-2, 0, 0]]
+    np.testing.assert_allclose(ncc.cpu().numpy(), ora["ncc"], atol=1e-6)
+    # constant moving volume / constant fixed block: NCC := 0 everywhere, index 0 wins (reading Q12)
+    vol = _smooth((24, 24, 16), 16)
+    const = np.full_like(vol, 123.0)
+    centres = np.asarray([[12, 12, 8]], dtype=np.int32)
+    for f, m in ((vol, const), (const, vol)):
+        for block, window in (((5, 5, 5), (3, 3, 3)), ((5, 5, 5), (2, 2, 2))):
+            ora = oracle.match(f, m, centres, block, window)
+            disp, ncc = nrr.nrr_bm_match(_cuda(f), _cuda(m), _cuda(centres), block, window)
+            assert disp.cpu().numpy().tolist() == ora["disp"].tolist()
+            assert ncc.cpu().numpy().tolist() == [0.0]
+
+
+def test_match_zero_blocks_and_bounds_flag():
+    vol = _smooth((24, 24, 16), 17)
+    empty = torch.empty((0, 3), dtype=torch.int32, device="cuda")
+    disp, ncc = nrr.nrr_bm_match(_cuda(vol), _cuda(vol), empty, (5, 5, 5), (3, 3, 3))
+    assert disp.shape == (0, 3) and ncc.shape == (0,)
+    nrr.nrr_bm_check_async_error()
+    bad = np.asarray([[12, 12, 8], [1, 12, 8]], dtype=np.int32)        # second block leaves the volume
+    disp, ncc = nrr.nrr_bm_match(_cuda(vol), _cuda(vol), _cuda(bad), (5, 5, 5), (3, 3, 3))
+    with pytest.raises(nrr.NrrError) as ei:
+        nrr.nrr_bm_check_async_error()
+    assert ei.value.status == -8
+    assert disp.cpu().numpy()[0].tolist() == [0, 0, 0] and np.isnan(ncc.cpu().numpy()[1])
+    nrr.nrr_bm_check_async_error()                                       # flag was cleared
+
+
+def test_host_forms_equal_device_forms():
+    cfg = CONFIGS["tiny"]
+    fixed, moving, mask = pair("tiny")
+    blocks, n, ncand = nrr.nrr_bm_select_blocks(_cuda(fixed), cfg.block, cfg.stride, cfg.frac)
+    disp, ncc = nrr.nrr_bm_match(_cuda(fixed), _cuda(moving), blocks, cfg.block, cfg.window)
+    hb, hn, hc, hv = nrr.nrr_bm_select_blocks_host(fixed, cfg.block, cfg.stride, cfg.frac)
+    assert hn == n and hc == ncand and np.array_equal(hb, blocks.cpu().numpy())
+    hd, hs = nrr.nrr_bm_match_host(fixed, moving, hb, cfg.block, cfg.window)
+    assert np.array_equal(hd, disp.cpu().numpy()) and np.array_equal(hs, ncc.cpu().numpy())
+    rb, rd, rs = nrr.nrr_bm_register_host(fixed, moving, cfg.block, cfg.stride, cfg.window, cfg.frac)
+    assert np.array_equal(rb, hb) and np.array_equal(rd, hd) and np.array_equal(rs, hs)
+
+
+@pytest.mark.parametrize("name", ["tiny", "intraop", "fullres"])
+def test_match_parity_configs_full(name):
+    """BASELINE.json configs 1-3 at full size, every selected block, in the launch configuration bench.py uses."""
+    cfg = CONFIGS[name]
+    fixed, moving, mask = pair(name)
+    blocks, n, ncand = nrr.nrr_bm_select_blocks(_cuda(fixed), cfg.block, cfg.stride, cfg.frac, _cuda(mask))
+    disp, ncc = nrr.nrr_bm_match(_cuda(fixed), _cuda(moving), blocks, cfg.block, cfg.window)
+    nrr.nrr_bm_check_async_error()
+    ora = oracle.match(fixed, moving, blocks.cpu().numpy(), cfg.block, cfg.window)
+    exempt = assert_match_parity(disp.cpu().numpy(), ncc.cpu().numpy(), ora, label=name)
+    err = np.abs(ncc.cpu().numpy().astype(np.float64) - ora["ncc"])
+    print("%s: %d blocks, %d inside the 1e-5 tie band (%d differ), max |dNCC| %.3g" % (
+        name, n, int((ora["gap"] < 1e-5).sum()), exempt, err.max()))
+    if name == "tiny":      # exact recovery of the constructed translation
+        inside = np.all((blocks.cpu().numpy() - 2 + np.asarray(cfg.shift) >= np.maximum(cfg.shift, 0)) &
+                        (blocks.cpu().numpy() + 3 + np.asarray(cfg.shift) <= np.asarray(cfg.dims) + np.minimum(cfg.shift, 0)), axis=1)
+        assert np.all(disp.cpu().numpy()[inside] == np.asarray(cfg.shift))
+
+
+def test_match_parity_highres_sampled():
+    """Config 4 (512x512x176, 9^3, +-7): the full launch on the GPU, 400 sampled blocks on the oracle."""
+    cfg = CONFIGS["highres"]
+    fixed, moving, mask = pair("highres")
+    blocks, n, ncand = nrr.nrr_bm_select_blocks(_cuda(fixed), cfg.block, cfg.stride, cfg.frac)
+    assert (ncand, n) == (197568, 39514)
+    disp, ncc = nrr.nrr_bm_match(_cuda(fixed), _cuda(moving), blocks, cfg.block, cfg.window)
+    nrr.nrr_bm_check_async_error()
+    idx = np.unique(np.concatenate([np.arange(40), np.arange(n - 40, n),
+                                    np.random.default_rng(5).choice(n, 320, replace=False)]))
+    ora = oracle.match(fixed, moving, blocks.cpu().numpy()[idx], cfg.block, cfg.window)
+    exempt = assert_match_parity(disp.cpu().numpy()[idx], ncc.cpu().numpy()[idx], ora, label="highres")
+    print("highres: %d blocks on the GPU, %d checked, %d exempt" % (n, len(idx), exempt))
+    # properties that hold at any size
+    d = disp.cpu().numpy()
+    assert np.all(np.abs(d) <= np.asarray(cfg.window))
+    s = ncc.cpu().numpy()
+    assert np.all(np.isfinite(s)) and np.all(s <= 1.0 + 1e-5) and np.all(s >= -1.0 - 1e-5)
+
+
+def test_match_parity_batch_sampled():
+    """Config 5: 32 settings on the fullres pair; per setting the selection is checked in full and 48 sampled
+    blocks are checked against the oracle."""
+    cfg = CONFIGS["fullres"]
+    fixed, moving, mask = pair("fullres")
+    f, m, k = _cuda(fixed), _cuda(moving), _cuda(mask)
+    total_exempt = 0
+    for si, st in enumerate(batch_settings()):
+        ora_sel = oracle.select(fixed, st.block, st.stride, st.frac, mask)
+        blocks, n, ncand = nrr.nrr_bm_select_blocks(f, st.block, st.stride, st.frac, k)
+        assert_select_parity(blocks.cpu().numpy(), n, ncand, ora_sel)
+        disp, ncc = nrr.nrr_bm_match(f, m, blocks, st.block, st.window)
+        idx = np.sort(np.random.default_rng(1000 + si).choice(n, 48, replace=False))
+        ora = oracle.match(fixed, moving, ora_sel["centres"][idx], st.block, st.window)
+        total_exempt += assert_match_parity(disp.cpu().numpy()[idx], ncc.cpu().numpy()[idx], ora, label=str(st))
+    nrr.nrr_bm_check_async_error()
+    print("batch: 32 settings, %d exempt blocks among the samples" % total_exempt)
