@@ -6,8 +6,11 @@
 // moving volume by nrr_boxstat.cu.  (PAPER.md:243-246 equation; listing PAPER.md:659-667.)
 //
 // FAST KERNEL (cubic block B in {5,7,9,11}, window (R,R,rz) with R in {3,5,7,9}):
-//   M1  stage   : the fixed block and the union of the window's moving voxels arrive in shared memory by TMA
-//                 (one cp.async.bulk.tensor each; out-of-volume voxels are zero-filled by the hardware).
+//   M1  stage   : the union of the window's moving voxels arrives in shared memory by ONE TMA tensor copy
+//                 (cp.async.bulk.tensor.3d; out-of-volume voxels are zero-filled by the hardware).  TMA needs
+//                 a 16-byte aligned inner start coordinate (measured on B200: an unaligned x start raises an
+//                 illegal-instruction fault), so the box starts at x rounded down to a multiple of 4 and each
+//                 row is then shifted left by the 0..3 floats of slack, in place, with vector loads/stores.
 //                 The union rows have a pitch of 4*odd floats and each z-plane holds W + 8k rows, so the
 //                 LDS.128 row loads of a quarter-warp touch eight distinct 16-byte bank groups.
 //   M3  cross   : one thread per candidate ROW (dy,dz): the W = 2R+1 candidates along x live in registers;
@@ -207,9 +210,29 @@ __device__ void write_bounds_error(int b, int *out_disp, float *out_ncc, unsigne
 }
 
 // ------------------------------------------------------------------------------------------ fast kernel
+// row[k] = row[k + S] for k < UX, in place, one thread per row: whole row to registers, then vector stores.
+template <int S, int UX, int PITCH>
+__device__ __forceinline__ void shift_row_left(float *row)
+{
+    constexpr int NL = (UX + S + 3) / 4;        // vectors holding the shifted source
+    constexpr int NS = (UX + 3) / 4;            // vectors written
+    static_assert(NL * 4 <= PITCH, "row pitch too small for the alignment slack");
+    float t[NL * 4 + 4];
+#pragma unroll
+    for (int q = 0; q < NL; ++q) {
+        const float4 v = *reinterpret_cast<const float4 *>(row + 4 * q);
+        t[4 * q + 0] = v.x; t[4 * q + 1] = v.y; t[4 * q + 2] = v.z; t[4 * q + 3] = v.w;
+    }
+#pragma unroll
+    for (int k = NL * 4; k < NL * 4 + 4; ++k) t[k] = 0.f;
+#pragma unroll
+    for (int q = 0; q < NS; ++q)
+        *reinterpret_cast<float4 *>(row + 4 * q) = make_float4(t[4 * q + S], t[4 * q + 1 + S], t[4 * q + 2 + S], t[4 * q + 3 + S]);
+}
+
 constexpr int pitch_for(int ux)
 {
-    int p = (ux + 3) / 4 * 4;
+    int p = (ux + 3 + 3) / 4 * 4;               // room for the 0..3 floats of TMA alignment slack
     return ((p / 4) % 2 == 0) ? p + 4 : p;      // 4 * odd
 }
 
@@ -229,7 +252,7 @@ struct FastCfg {
 };
 
 struct FastSmem {      // tail of the dynamic shared memory, after the union and the fixed block
-    uint64_t bar_fixed, bar_union;
+    uint64_t bar_union;
     double red[32];
     float am_v[32];
     int am_i[32];
@@ -260,8 +283,7 @@ inline size_t fast_smem_bytes(int rz)
 constexpr int kFastMaxThreads = 512;
 
 template <int B, int R>
-__global__ void __launch_bounds__(kFastMaxThreads) match_rows_kernel(const __grid_constant__ CUtensorMap tm_moving,
-                                  const __grid_constant__ CUtensorMap tm_fixed, int use_tma,
+__global__ void __launch_bounds__(kFastMaxThreads) match_rows_kernel(const __grid_constant__ CUtensorMap tm_moving, int use_tma,
                                   const float *__restrict__ fixed, const float *__restrict__ moving,
                                   const float *__restrict__ inv_sd, Int3 dims, const int *__restrict__ blocks,
                                   int rz, float tie_band, int *__restrict__ out_disp, float *__restrict__ out_ncc,
@@ -290,34 +312,32 @@ __global__ void __launch_bounds__(kFastMaxThreads) match_rows_kernel(const __gri
     const int nrows = W * WZ;
 
     // ---- M1: stage the fixed block and the window union
+    const int x0 = ox - R;
+    const int x0a = x0 & ~3;                  // floor to a multiple of 4 (two's complement), TMA alignment
+    const int xoff = x0 - x0a;                // 0..3 floats of slack at the start of every staged row
     if (use_tma) {
         if (tid == 0) {
-            mbar_init(&sm->bar_fixed, 1);
             mbar_init(&sm->bar_union, 1);
             mbar_fence_init();
-            mbar_arrive_expect_tx(&sm->bar_fixed, (uint32_t)(sizeof(float) * B * B * FP));
-            tma_load_3d(s_fixed, &tm_fixed, ox, oy, oz, &sm->bar_fixed);
             mbar_arrive_expect_tx(&sm->bar_union, (uint32_t)(sizeof(float) * (size_t)UZ * PROWS * PITCH));
-            tma_load_3d(s_union, &tm_moving, ox - R, oy - R, oz - rz, &sm->bar_union);
+            tma_load_3d(s_union, &tm_moving, x0a, oy - R, oz - rz, &sm->bar_union);
         }
-        __syncthreads();                      // barrier initialisation visible before anyone waits
-        mbar_wait(&sm->bar_fixed, 0);
     } else {
-        for (int i = tid; i < B * B * B; i += blockDim.x) {
-            const int z = i / (B * B), r = i % (B * B), y = r / B, x = r % B;
-            s_fixed[(z * B + y) * FP + x] = __ldg(fixed + ((size_t)(oz + z) * dims.y + (oy + y)) * dims.x + ox + x);
-        }
         const int ux = C::UX;
         for (int i = tid; i < UZ * ux * ux; i += blockDim.x) {
             const int z = i / (ux * ux), r = i % (ux * ux), y = r / ux, x = r % ux;
-            const int gx = ox - R + x, gy = oy - R + y, gz = oz - rz + z;
+            const int gx = x0 + x, gy = oy - R + y, gz = oz - rz + z;
             float v = 0.f;
             if (gx >= 0 && gx < dims.x && gy >= 0 && gy < dims.y && gz >= 0 && gz < dims.z)
                 v = __ldg(moving + ((size_t)gz * dims.y + gy) * dims.x + gx);
             s_union[((size_t)z * PROWS + y) * PITCH + x] = v;
         }
-        __syncthreads();
     }
+    for (int i = tid; i < B * B * B; i += blockDim.x) {
+        const int z = i / (B * B), r = i % (B * B), y = r / B, x = r % B;
+        s_fixed[(z * B + y) * FP + x] = __ldg(fixed + ((size_t)(oz + z) * dims.y + (oy + y)) * dims.x + ox + x);
+    }
+    __syncthreads();                          // fixed block staged; barrier initialisation visible
 
     // ---- centre the fixed block in place: mean and SS in FP64, f' stored in FP32
     {
@@ -354,7 +374,19 @@ __global__ void __launch_bounds__(kFastMaxThreads) match_rows_kernel(const __gri
         isd[j] = (row_ok && px >= 0 && px + B <= dims.x) ? __ldg(inv_sd + ((size_t)pz * dims.y + py) * dims.x + px) : -1.f;
     }
 
-    if (use_tma) mbar_wait(&sm->bar_union, 0);
+    if (use_tma) {
+        mbar_wait(&sm->bar_union, 0);
+        if (xoff != 0) {                      // uniform over the CTA
+            const int nstaged = UZ * C::UX;   // rows that are read later: (z, y < UX)
+            for (int r = tid; r < nstaged; r += blockDim.x) {
+                float *row = s_union + ((size_t)(r / C::UX) * PROWS + (r % C::UX)) * PITCH;
+                if (xoff == 1) shift_row_left<1, C::UX, PITCH>(row);
+                else if (xoff == 2) shift_row_left<2, C::UX, PITCH>(row);
+                else shift_row_left<3, C::UX, PITCH>(row);
+            }
+        }
+        __syncthreads();
+    }
 
     // ---- M3: cross terms
     float acc[W];
@@ -533,11 +565,11 @@ bool make_volume_map(CUtensorMap *map, const float *vol, Int3 dims, int bx, int 
               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-bool tma_eligible(Int3 dims, const void *moving, const void *fixed, int box_z)
+bool tma_eligible(Int3 dims, const void *moving, int box_z)
 {
     if (g_disable_tma) return false;
     if (dims.x % 4 != 0) return false;                                   // global strides must be multiples of 16 B
-    if (((uintptr_t)moving & 15) || ((uintptr_t)fixed & 15)) return false;
+    if ((uintptr_t)moving & 15) return false;
     if (box_z > 256) return false;
     return encode_tiled_fn() != nullptr;
 }
@@ -550,7 +582,7 @@ int launch_fast(const float *fixed, const float *moving, const float *inv_sd, In
     const int nrows = C::W * (2 * rz + 1);
     const int threads = (nrows + 31) / 32 * 32;
     const size_t smem = fast_smem_bytes<B, R>(rz);
-    const bool tma = tma_eligible(dims, moving, fixed, B + 2 * rz);
+    const bool tma = tma_eligible(dims, moving, B + 2 * rz);
     if (plan_only) {
         plan_only->fast = 1;
         plan_only->threads = threads;
@@ -558,20 +590,17 @@ int launch_fast(const float *fixed, const float *moving, const float *inv_sd, In
         plan_only->tma = tma ? 1 : 0;
         return NRR_OK;
     }
-    CUtensorMap tm_m, tm_f;
+    CUtensorMap tm_m;
     memset(&tm_m, 0, sizeof(tm_m));
-    memset(&tm_f, 0, sizeof(tm_f));
     int use_tma = 0;
-    if (tma && make_volume_map(&tm_m, moving, dims, C::PITCH, C::PROWS, B + 2 * rz) &&
-        make_volume_map(&tm_f, fixed, dims, C::FP, B, B))
-        use_tma = 1;
+    if (tma && make_volume_map(&tm_m, moving, dims, C::PITCH, C::PROWS, B + 2 * rz)) use_tma = 1;
     auto kern = match_rows_kernel<B, R>;
     static int configured_smem = 0;     // per instantiation
     if ((int)smem > configured_smem) {
         NRR_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         configured_smem = (int)smem;
     }
-    kern<<<n, threads, smem, stream>>>(tm_m, tm_f, use_tma, fixed, moving, inv_sd, dims, blocks, rz, g_tie_band,
+    kern<<<n, threads, smem, stream>>>(tm_m, use_tma, fixed, moving, inv_sd, dims, blocks, rz, g_tie_band,
                                        out_disp, out_ncc, err_flag);
     NRR_LAUNCH_CHECK("match_rows_kernel");
     return NRR_OK;
