@@ -14,6 +14,8 @@ namespace nrr {
 extern float g_tie_band;
 extern int g_force_generic;
 extern int g_disable_tma;
+extern int g_force_rows;
+extern int g_pair_g;
 
 namespace {
 
@@ -401,6 +403,8 @@ int nrr_bm_set_option(const char *name, double value)
     if (!strcmp(name, "tie_band")) { g_tie_band = (float)value; return NRR_OK; }
     if (!strcmp(name, "force_generic")) { g_force_generic = value != 0.0; return NRR_OK; }
     if (!strcmp(name, "disable_tma")) { g_disable_tma = value != 0.0; return NRR_OK; }
+    if (!strcmp(name, "force_rows")) { g_force_rows = value != 0.0; return NRR_OK; }
+    if (!strcmp(name, "pair_blocks_per_cta")) { g_pair_g = (int)value; return NRR_OK; }
     return fail(NRR_E_ARG, "unknown option '%s'", name);
 }
 

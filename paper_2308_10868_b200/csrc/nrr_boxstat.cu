@@ -26,7 +26,7 @@ constexpr int kThreads = TX * TY;
 __global__ void __launch_bounds__(kThreads)
 boxstat_kernel(const float *__restrict__ vol, Int3 dims, Int3 block, float *__restrict__ inv_sd)
 {
-    extern __shared__ __align__(16) unsigned char s_dyn[];
+    NRR_DYN_SMEM(s_dyn);
     // carve: row sums (double2) | ring (double2) | plane tile (float)
     const int HX = TX + block.x - 1, HY = TY + block.y - 1;
     double2 *s_row = (double2 *)s_dyn;                       // [HY][TX]
@@ -112,7 +112,7 @@ int boxstat_enqueue(const float *moving, Int3 dims, Int3 block, float *inv_sd, c
         set_error("volume too large for the moving-volume statistics grid");
         return NRR_E_DIMS;
     }
-    boxstat_kernel<<<grid, kThreads, smem, stream>>>(moving, dims, block, inv_sd);
+    NRR_LAUNCH(boxstat_kernel, grid, kThreads, smem, stream, moving, dims, block, inv_sd);
     NRR_LAUNCH_CHECK("boxstat_kernel");
     return NRR_OK;
 }

@@ -7,6 +7,14 @@
 
 #include "../../include/nrr_bm.h"
 
+// Kernel launch and dynamic shared memory go through two macros so that the test suite can compile these
+// sources as plain C++ against tests/cuda_emul (a fiber-per-thread emulation used by the CPU tests only;
+// NRR_EMUL is never defined when the product library is built).
+#ifndef NRR_EMUL
+#define NRR_LAUNCH(kern, grid, block, smem, stream, ...) (kern)<<<(grid), (block), (smem), (stream)>>>(__VA_ARGS__)
+#define NRR_DYN_SMEM(name) extern __shared__ __align__(128) unsigned char name[]
+#endif
+
 namespace nrr {
 
 struct Int3 { int x, y, z; };
@@ -54,17 +62,23 @@ int boxstat_enqueue(const float *moving, Int3 dims, Int3 block, float *inv_sd, c
 
 // ---- matching (nrr_match.cu) ------------------------------------------------------------------------
 struct MatchPlan {
-    int fast;          // 1: register-tiled kernel, 0: generic kernel
+    int fast;          // 2: pair kernel (two candidate rows per thread), 1: one row per thread, 0: generic kernel
     int threads;
     int smem_bytes;
     int tma;           // 1: TMA staging
     int candidates;
+    int blocks_per_cta;
 };
 int match_plan(Int3 dims, Int3 block, Int3 window, const void *moving_ptr, const void *fixed_ptr,
                MatchPlan *plan);
 int match_enqueue(const float *fixed, const float *moving, const float *inv_sd, Int3 dims, const int *blocks,
                   int n, Int3 block, Int3 window, int *out_disp, float *out_ncc, unsigned int *err_flag,
                   cudaStream_t stream);
+
+// nrr_match_pair.cu: tries the pair kernel; *handled tells whether it took the call.
+int match_pair_dispatch(const float *fixed, const float *moving, const float *inv_sd, Int3 dims, const int *blocks,
+                        int n, Int3 block, Int3 window, int *out_disp, float *out_ncc, unsigned int *err_flag,
+                        cudaStream_t stream, MatchPlan *plan_only, bool *handled);
 
 // ---- FFMA microbenchmark (nrr_fma_peak.cu) ----------------------------------------------------------
 int fp32_peak_measure(double *out_tflops, cudaStream_t stream);

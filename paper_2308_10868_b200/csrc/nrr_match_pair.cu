@@ -1,0 +1,699 @@
+// nrr_match_pair.cu -- the register-tiled matching kernel for cubic blocks.
+//
+// NCC's numerator over the centred fixed block f' = f - fbar is num(d) = sum_v f'(v) * m(o + d + v)
+// (sum f' = 0, so the moving mean drops out); NCC(d) = num(d) * inv_sd_m(o + d) * inv_sd_f with inv_sd_m
+// precomputed per block origin of the moving volume (nrr_boxstat.cu).  PAPER.md:243-246 (NCC equation),
+// listing PAPER.md:659-667 (for each block, for each candidate in the window, similarity, maximum).
+//
+// Two kernels per nrr_bm_match call:
+//
+//  prep_kernel<B>      one warp per block: FP64 mean and sum of squares of the fixed block, then one RECORD per
+//                      block in global scratch, laid out exactly as the matching kernel wants it in shared
+//                      memory: the centred block f' as rows of FP floats, a PAIR TABLE holding, for the planes
+//                      zr = 1..B-1, the interleaved pairs (f'[zr][vy][vx], f'[zr-1][vy][vx]), and a header
+//                      with 1/sqrt(SS_f).  Blocks that leave the volume are flagged here.
+//
+//  match_pair_kernel<B,R>  one CTA per group of G consecutive blocks.
+//    M1 stage   : one elected warp issues, per block, ONE TMA tensor copy of the window union of the moving
+//                 volume (cp.async.bulk.tensor.3d, out-of-volume voxels zero-filled by the hardware) and one
+//                 bulk copy of the G records; a single mbarrier collects the bytes.  TMA needs a 16-byte
+//                 aligned inner start coordinate on B200 (an unaligned x start raises an illegal-instruction
+//                 fault), so the box starts at x rounded down to a multiple of 4 and every staged row is
+//                 shifted left in place by its block's 0..3 floats of slack.
+//    M3 cross   : a thread owns TWO candidate rows that are adjacent in z, (dy, 2p) and (dy, 2p+1), W = 2R+1
+//                 candidates each, as W packed accumulator pairs.  Every moving row it loads (LDS.128) feeds
+//                 both rows: plane zr of the union meets fixed plane zr for the first row and zr-1 for the
+//                 second, so one FFMA2 (fma.rn.f32x2: scalar moving voxel x pair of fixed voxels from the pair
+//                 table) does two useful FMAs per issue slot and halves the shared-memory traffic per FMA.
+//                 The two end planes touch one row only and use plain FFMA on one half of the pair.  The
+//                 odd plane of candidates (dz = 2rz) is handled by separate warps with one row per thread.
+//                 Which lane takes which (block, dy, p) comes from a host-built table that packs the tasks of
+//                 the G blocks into full warps and keeps the LDS.128 of each quarter-warp on distinct banks.
+//    M4 argmax  : NCC in registers; per-block maximum through a warp reduction and one 64-bit shared atomicMax
+//                 on (ordered NCC bits, ~index), i.e. lowest linear candidate index among equal maxima; every
+//                 candidate within tie_band of the FP32 maximum is re-scored in FP64 (two-pass, raw voxels)
+//                 and the decision is taken on the FP64 values.
+//    M5 write   : out_disp, out_ncc.
+#include <cuda.h>
+#include <math.h>
+#include <string.h>
+
+#include <map>
+#include <mutex>
+#include <vector>
+
+#include "nrr_match_common.cuh"
+
+namespace nrr {
+
+extern float g_tie_band;
+int g_pair_g = 0;             // experiment knob: force the number of blocks per CTA (0 = planner's choice)
+
+namespace {
+
+typedef unsigned long long u64;
+
+constexpr int kGMax = 8;
+constexpr int kPairMaxThreads = 512;
+
+template <int B, int R>
+struct PairCfg {
+    static constexpr int W = 2 * R + 1;                 // candidates per row
+    static constexpr int UX = B + 2 * R;                // union extent in x and y
+    static constexpr int PITCH = pitch_for(UX);         // floats per staged row: 4 * odd, >= UX + 3
+    static constexpr int NV = (UX + 3) / 4;             // LDS.128 per moving row
+    static constexpr int FP = (B + 3) / 4 * 4;          // floats per row of the plain centred block
+    static constexpr int NF = FP / 4;
+    static constexpr int FPP = (2 * B + 3) / 4 * 4;     // floats per row of the pair table
+    static constexpr int NFP = FPP / 4;
+    static constexpr int PLAIN_FLOATS = B * B * FP;
+    static constexpr int PAIR_FLOATS = (B - 1) * B * FPP;
+    static constexpr int HDR_FLOATS = 4;                // isd_f, valid, 0, 0
+    static constexpr int REC_FLOATS = PLAIN_FLOATS + PAIR_FLOATS + HDR_FLOATS;
+    static constexpr int REC_BYTES = REC_FLOATS * 4;
+    static_assert(REC_BYTES % 16 == 0, "records are moved by 16-byte bulk copies");
+    static_assert(PITCH >= NV * 4, "row pitch must cover the vector loads");
+};
+
+struct PairCtrl {              // tail of the dynamic shared memory
+    uint64_t bar;
+    u64 best[kGMax];           // (ordered NCC bits << 32) | ~index
+    int4 org[kGMax];           // block origin (x, y, z), w = 1 if the block is inside the volume
+    int count[kGMax];          // near ties besides the FP32 best
+    TieScratch ts;
+};
+
+// ------------------------------------------------------------------------------------------ PTX helpers
+#ifdef NRR_EMUL
+__device__ __forceinline__ void bulk_load(void *dst, const void *src, uint32_t bytes, uint64_t *bar) { emul::bulk_load(dst, src, bytes, bar); }
+__device__ __forceinline__ void fma2s(u64 &acc, float m, u64 f)
+{
+    float a[2], b[2];
+    memcpy(a, &acc, 8);
+    memcpy(b, &f, 8);
+    a[0] = fmaf(m, b[0], a[0]);
+    a[1] = fmaf(m, b[1], a[1]);
+    memcpy(&acc, a, 8);
+}
+__device__ __forceinline__ void fma_lo(u64 &acc, float x, float y)
+{
+    float a[2];
+    memcpy(a, &acc, 8);
+    a[0] = fmaf(x, y, a[0]);
+    memcpy(&acc, a, 8);
+}
+__device__ __forceinline__ void fma_hi(u64 &acc, float x, float y)
+{
+    float a[2];
+    memcpy(a, &acc, 8);
+    a[1] = fmaf(x, y, a[1]);
+    memcpy(&acc, a, 8);
+}
+#else
+__device__ __forceinline__ void bulk_load(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+// (acc.lo, acc.hi) += m * (f.lo, f.hi): SASS FFMA2 with a scalar-broadcast operand
+__device__ __forceinline__ void fma2s(u64 &acc, float m, u64 f)
+{
+    u64 mm;
+    asm("mov.b64 %0, {%1, %1};" : "=l"(mm) : "f"(m));
+    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc) : "l"(mm), "l"(f));
+}
+__device__ __forceinline__ void fma_lo(u64 &acc, float a, float b)
+{
+    asm("{\n\t.reg .f32 lo, hi;\n\tmov.b64 {lo, hi}, %0;\n\tfma.rn.f32 lo, %1, %2, lo;\n\tmov.b64 %0, {lo, hi};\n\t}"
+        : "+l"(acc) : "f"(a), "f"(b));
+}
+__device__ __forceinline__ void fma_hi(u64 &acc, float a, float b)
+{
+    asm("{\n\t.reg .f32 lo, hi;\n\tmov.b64 {lo, hi}, %0;\n\tfma.rn.f32 hi, %1, %2, hi;\n\tmov.b64 %0, {lo, hi};\n\t}"
+        : "+l"(acc) : "f"(a), "f"(b));
+}
+#endif
+__device__ __forceinline__ uint32_t order_bits(float v)      // monotone float -> unsigned, never 0 for |v| <= 1
+{
+    const uint32_t b = __float_as_uint(v + 0.f);              // -0 -> +0
+    return (b & 0x80000000u) ? ~b : (b | 0x80000000u);
+}
+__device__ __forceinline__ float unorder_bits(uint32_t k)
+{
+    return __uint_as_float((k & 0x80000000u) ? (k & 0x7fffffffu) : ~k);
+}
+
+// ------------------------------------------------------------------------------------------ prep kernel
+constexpr int kPrepWarps = 4;
+
+template <int B, int R>
+__global__ void __launch_bounds__(kPrepWarps * 32)
+prep_kernel(const float *__restrict__ fixed, Int3 dims, const int *__restrict__ blocks, int n,
+            float *__restrict__ records, int *__restrict__ out_disp, float *__restrict__ out_ncc,
+            unsigned int *err_flag)
+{
+    using C = PairCfg<B, R>;
+    constexpr int NVOX = B * B * B;
+    __shared__ float s_f[kPrepWarps][NVOX];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int b = blockIdx.x * kPrepWarps + warp;
+    if (b >= n) return;
+    float *rec = records + (size_t)b * C::REC_FLOATS;
+    float *hdr = rec + C::PLAIN_FLOATS + C::PAIR_FLOATS;
+    const int ox = blocks[3 * (size_t)b + 0] - (B - 1) / 2;
+    const int oy = blocks[3 * (size_t)b + 1] - (B - 1) / 2;
+    const int oz = blocks[3 * (size_t)b + 2] - (B - 1) / 2;
+    if (!block_in_volume(dims, Int3{B, B, B}, ox, oy, oz)) {      // uniform over the warp
+        if (lane == 0) {
+            out_disp[3 * (size_t)b + 0] = 0;
+            out_disp[3 * (size_t)b + 1] = 0;
+            out_disp[3 * (size_t)b + 2] = 0;
+            out_ncc[b] = __int_as_float(0x7fc00000);
+            atomicOr(err_flag, 1u);
+        }
+        for (int i = lane; i < C::REC_FLOATS; i += 32) rec[i] = 0.f;      // header: isd_f = 0, valid = 0
+        return;
+    }
+    float *f = s_f[warp];
+    double s = 0.0;
+    for (int i = lane; i < NVOX; i += 32) {
+        const int z = i / (B * B), r = i % (B * B), y = r / B, x = r % B;
+        const float v = __ldg(fixed + ((size_t)(oz + z) * dims.y + (oy + y)) * dims.x + ox + x);
+        f[i] = v;
+        s += (double)v;
+    }
+    const double mean = warp_sum(s) / (double)NVOX;
+    double q = 0.0;
+    for (int i = lane; i < NVOX; i += 32) {
+        const double d = (double)f[i] - mean;
+        f[i] = (float)d;
+        q += d * d;
+    }
+    const double ssf = warp_sum(q);
+    __syncwarp();
+    // plain centred block: rows of FP floats, zero padded
+    for (int i = lane; i < C::PLAIN_FLOATS; i += 32) {
+        const int zy = i / C::FP, x = i % C::FP;
+        rec[i] = x < B ? f[zy * B + x] : 0.f;
+    }
+    // pair table: for zr = 1..B-1 and every (vy, vx): (f'[zr][vy][vx], f'[zr-1][vy][vx])
+    float *pt = rec + C::PLAIN_FLOATS;
+    for (int i = lane; i < C::PAIR_FLOATS; i += 32) {
+        const int row = i / C::FPP, k = i % C::FPP;         // row = (zr-1)*B + vy
+        const int zr = row / B + 1, vy = row % B, vx = k >> 1, h = k & 1;
+        pt[i] = vx < B ? f[((zr - h) * B + vy) * B + vx] : 0.f;
+    }
+    if (lane == 0) {
+        hdr[0] = ssf == 0.0 ? 0.f : (float)(1.0 / sqrt(ssf));
+        hdr[1] = 1.f;
+        hdr[2] = 0.f;
+        hdr[3] = 0.f;
+    }
+}
+
+// ------------------------------------------------------------------------------------------ main loops
+template <int NV>
+__device__ __forceinline__ void load_row(float (&m)[NV * 4], const float *p)
+{
+#pragma unroll
+    for (int q = 0; q < NV; ++q) {
+        const float4 v = *reinterpret_cast<const float4 *>(p + 4 * q);
+        m[4 * q + 0] = v.x; m[4 * q + 1] = v.y; m[4 * q + 2] = v.z; m[4 * q + 3] = v.w;
+    }
+}
+
+// Two candidate rows per thread: row A at union plane offset 0, row B one plane further.
+// urow = first moving row of A; rec = this block's record; ra/rb receive the raw numerators.
+template <int B, int R>
+__device__ __forceinline__ void pair_rows(const float *urow, const float *rec, float (&ra)[2 * R + 1], float (&rb)[2 * R + 1])
+{
+    using C = PairCfg<B, R>;
+    constexpr int W = C::W, PITCH = C::PITCH, PLANE = C::UX * C::PITCH;
+    u64 acc[W];
+#pragma unroll
+    for (int j = 0; j < W; ++j) acc[j] = 0ull;
+    // plane 0: row A only, fixed plane 0
+#pragma unroll 1
+    for (int vy = 0; vy < B; ++vy) {
+        float m[C::NV * 4], f[C::FP];
+        load_row<C::NV>(m, urow + vy * PITCH);
+        load_row<C::NF>(f, rec + vy * C::FP);
+#pragma unroll
+        for (int vx = 0; vx < B; ++vx)
+#pragma unroll
+            for (int j = 0; j < W; ++j) fma_lo(acc[j], f[vx], m[j + vx]);
+    }
+    // planes 1..B-1: both rows, (f'[zr], f'[zr-1]) pairs
+    const float *pt = rec + C::PLAIN_FLOATS;
+#pragma unroll 1
+    for (int zr = 1; zr < B; ++zr) {
+        const float *up = urow + zr * PLANE;
+        const float *fp = pt + (zr - 1) * B * C::FPP;
+#pragma unroll 1
+        for (int vy = 0; vy < B; ++vy) {
+            float m[C::NV * 4];
+            u64 f[C::NFP * 2];
+            load_row<C::NV>(m, up + vy * PITCH);
+#pragma unroll
+            for (int q = 0; q < C::NFP; ++q) {
+                const ulonglong2 v = *reinterpret_cast<const ulonglong2 *>(fp + vy * C::FPP + 4 * q);
+                f[2 * q] = v.x; f[2 * q + 1] = v.y;
+            }
+#pragma unroll
+            for (int vx = 0; vx < B; ++vx)
+#pragma unroll
+                for (int j = 0; j < W; ++j) fma2s(acc[j], m[j + vx], f[vx]);
+        }
+    }
+    // plane B: row B only, fixed plane B-1
+    {
+        const float *up = urow + B * PLANE;
+        const float *fp = rec + (B - 1) * B * C::FP;
+#pragma unroll 1
+        for (int vy = 0; vy < B; ++vy) {
+            float m[C::NV * 4], f[C::FP];
+            load_row<C::NV>(m, up + vy * PITCH);
+            load_row<C::NF>(f, fp + vy * C::FP);
+#pragma unroll
+            for (int vx = 0; vx < B; ++vx)
+#pragma unroll
+                for (int j = 0; j < W; ++j) fma_hi(acc[j], f[vx], m[j + vx]);
+        }
+    }
+#pragma unroll
+    for (int j = 0; j < W; ++j) {
+        ra[j] = __uint_as_float((uint32_t)(acc[j] & 0xffffffffull));
+        rb[j] = __uint_as_float((uint32_t)(acc[j] >> 32));
+    }
+}
+
+// One candidate row per thread (the odd last plane of candidates).
+template <int B, int R>
+__device__ __forceinline__ void single_row(const float *urow, const float *rec, float (&ra)[2 * R + 1])
+{
+    using C = PairCfg<B, R>;
+    constexpr int W = C::W, PITCH = C::PITCH, PLANE = C::UX * C::PITCH;
+#pragma unroll
+    for (int j = 0; j < W; ++j) ra[j] = 0.f;
+#pragma unroll 1
+    for (int vz = 0; vz < B; ++vz) {
+        const float *up = urow + vz * PLANE;
+        const float *fp = rec + vz * B * C::FP;
+#pragma unroll 1
+        for (int vy = 0; vy < B; ++vy) {
+            float m[C::NV * 4], f[C::FP];
+            load_row<C::NV>(m, up + vy * PITCH);
+            load_row<C::NF>(f, fp + vy * C::FP);
+#pragma unroll
+            for (int vx = 0; vx < B; ++vx)
+#pragma unroll
+                for (int j = 0; j < W; ++j) ra[j] = fmaf(f[vx], m[j + vx], ra[j]);
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------ the kernel
+struct PairArgs {
+    const float *fixed, *moving, *inv_sd, *records;
+    const int *blocks;
+    const uint32_t *task_tab;      // [threads]: valid << 31 | g << 16 | dy << 8 | p
+    int *out_disp;
+    float *out_ncc;
+    Int3 dims;
+    int n, rz, G, n_pair_warps;
+    int union_stride;              // bytes between the unions of consecutive blocks of a CTA (multiple of 128)
+    float tie_band;
+};
+
+template <int B, int R>
+__global__ void __launch_bounds__(kPairMaxThreads, 1)
+match_pair_kernel(const __grid_constant__ CUtensorMap tm_moving, const PairArgs a)
+{
+    using C = PairCfg<B, R>;
+    constexpr int W = C::W, PITCH = C::PITCH, UX = C::UX, PLANE = C::UX * C::PITCH;
+    NRR_DYN_SMEM(s_raw);
+    unsigned char *s_base = s_raw + ((128u - (smem_u32(s_raw) & 127u)) & 127u);
+    unsigned char *s_unions = s_base;
+    float *s_recs = (float *)(s_base + (size_t)a.G * a.union_stride);
+    PairCtrl *ctrl = (PairCtrl *)((unsigned char *)s_recs + (size_t)a.G * C::REC_BYTES);
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int b0 = blockIdx.x * a.G;
+    const int gact = min(a.G, a.n - b0);
+    const int rz = a.rz, WZ = 2 * rz + 1, UZ = B + 2 * rz;
+    const Int3 dims = a.dims;
+    const uint32_t union_bytes = (uint32_t)(sizeof(float) * UZ * UX * PITCH);
+
+    // ---- M1: stage. Warp 0: lane g owns block b0 + g.
+    if (warp == 0) {
+        if (lane == 0) {
+            mbar_init(&ctrl->bar, 1);
+            mbar_fence_init();
+        }
+        int ox = 0, oy = 0, oz = 0, ok = 0;
+        if (lane < gact) {
+            ox = a.blocks[3 * (size_t)(b0 + lane) + 0] - (B - 1) / 2;
+            oy = a.blocks[3 * (size_t)(b0 + lane) + 1] - (B - 1) / 2;
+            oz = a.blocks[3 * (size_t)(b0 + lane) + 2] - (B - 1) / 2;
+            ok = block_in_volume(dims, Int3{B, B, B}, ox, oy, oz) ? 1 : 0;
+        }
+        if (lane < kGMax) {
+            ctrl->org[lane] = make_int4(ox, oy, oz, ok);
+            ctrl->best[lane] = 0ull;
+            ctrl->count[lane] = 0;
+        }
+        const unsigned okmask = __ballot_sync(0xffffffffu, ok);
+        __syncwarp();
+        if (lane == 0)
+            mbar_arrive_expect_tx(&ctrl->bar, (uint32_t)__popc(okmask) * union_bytes + (uint32_t)gact * C::REC_BYTES);
+        __syncwarp();
+        if (ok) tma_load_3d(s_unions + (size_t)lane * a.union_stride, &tm_moving, (ox - R) & ~3, oy - R, oz - rz, &ctrl->bar);
+        if (lane == 0) bulk_load(s_recs, a.records + (size_t)b0 * C::REC_FLOATS, (uint32_t)gact * C::REC_BYTES, &ctrl->bar);
+    }
+    // this lane's task
+    const uint32_t task = a.task_tab[tid];
+    const int g = (task >> 16) & 0xff, dyi = (task >> 8) & 0xff, p = task & 0xff;
+    const bool is_pair = warp < a.n_pair_warps;
+    const int dzA = is_pair ? 2 * p : WZ - 1;
+    __syncthreads();                                   // org[] and the barrier are visible
+    const int4 org = ctrl->org[g < gact ? g : 0];
+    const bool active = (task >> 31) && g < gact && org.w;
+
+    mbar_wait(&ctrl->bar, 0);
+    // ---- undo the TMA alignment slack: shift every staged row left by its block's 0..3 floats
+    {
+        const int rows_per_block = UZ * UX;
+        for (int r = tid; r < gact * rows_per_block; r += blockDim.x) {
+            const int gg = r / rows_per_block, rr = r - gg * rows_per_block;
+            const int4 o = ctrl->org[gg];
+            const int xoff = (o.x - R) & 3;
+            float *row = (float *)(s_unions + (size_t)gg * a.union_stride) + (size_t)rr * PITCH;
+            if (!o.w || xoff == 0) continue;
+            if (xoff == 1) shift_row_left<1, UX, PITCH>(row);
+            else if (xoff == 2) shift_row_left<2, UX, PITCH>(row);
+            else shift_row_left<3, UX, PITCH>(row);
+        }
+    }
+    __syncthreads();
+
+    // ---- M3: cross terms
+    float ra[W], rb[W];
+    const float *urow = (const float *)(s_unions + (size_t)g * a.union_stride) + (size_t)dzA * PLANE + dyi * PITCH;
+    const float *rec = s_recs + (size_t)g * C::REC_FLOATS;
+    if (is_pair) {
+        if (active) pair_rows<B, R>(urow, rec, ra, rb);
+    } else {
+        if (active) single_row<B, R>(urow, rec, ra);
+    }
+
+    // ---- M4: NCC and the per-block arg-max
+    float bv = -INFINITY;
+    int bi = 0x7fffffff;
+    if (active) {
+        const float isd_f = rec[C::PLAIN_FLOATS + C::PAIR_FLOATS];
+        const int py = org.y + dyi - R;
+        const bool y_ok = py >= 0 && py + B <= dims.y;
+        const int jlo = max(0, R - org.x), jhi = min(W - 1, dims.x - B - org.x + R);      // valid j range
+        {
+            const int pz = org.z + dzA - rz;
+            const bool row_ok = y_ok && pz >= 0 && pz + B <= dims.z;
+            const float *ip = a.inv_sd + ((size_t)pz * dims.y + py) * dims.x + org.x - R;
+#pragma unroll
+            for (int j = 0; j < W; ++j) {
+                const bool ok = row_ok && j >= jlo && j <= jhi;
+                const float v = ok ? ra[j] * __ldg(ip + j) * isd_f : -INFINITY;
+                ra[j] = v;
+                if (v > bv) { bv = v; bi = (dzA * W + dyi) * W + j; }
+            }
+        }
+        if (is_pair) {
+            const int pz = org.z + dzA + 1 - rz;
+            const bool row_ok = y_ok && pz >= 0 && pz + B <= dims.z;
+            const float *ip = a.inv_sd + ((size_t)pz * dims.y + py) * dims.x + org.x - R;
+#pragma unroll
+            for (int j = 0; j < W; ++j) {
+                const bool ok = row_ok && j >= jlo && j <= jhi;
+                const float v = ok ? rb[j] * __ldg(ip + j) * isd_f : -INFINITY;
+                rb[j] = v;
+                if (v > bv) { bv = v; bi = ((dzA + 1) * W + dyi) * W + j; }
+            }
+        }
+    }
+    {
+        const bool have = bi != 0x7fffffff;
+        const uint32_t khi = have ? order_bits(bv) : 0u, klo = have ? 0xffffffffu - (uint32_t)bi : 0u;
+        const int gq = active ? g : 0x7fffffff;
+        const int gmin = __reduce_min_sync(0xffffffffu, gq);
+        const int gmax = __reduce_max_sync(0xffffffffu, active ? g : -1);
+        for (int gg = gmin; gg <= gmax; ++gg) {          // warp-uniform bounds; empty when no lane is active
+            const uint32_t mh = __reduce_max_sync(0xffffffffu, (active && g == gg) ? khi : 0u);
+            const uint32_t ml = __reduce_max_sync(0xffffffffu, (active && g == gg && khi == mh) ? klo : 0u);
+            if (lane == 0 && mh) atomicMax(&ctrl->best[gg], ((u64)mh << 32) | ml);
+        }
+    }
+    __syncthreads();
+
+    // ---- near ties: the unions are dead now, their storage holds the per-block lists
+    if (active) {
+        const u64 best = ctrl->best[g];
+        const float thr = unorder_bits((uint32_t)(best >> 32)) - a.tie_band;
+        const int big = (int)(0xffffffffu - (uint32_t)best);
+        int *s_list = (int *)(s_unions + (size_t)g * a.union_stride);
+#pragma unroll
+        for (int j = 0; j < W; ++j) {
+            const int idx = (dzA * W + dyi) * W + j;
+            if (ra[j] >= thr && idx != big) s_list[atomicAdd(&ctrl->count[g], 1)] = idx;
+        }
+        if (is_pair) {
+#pragma unroll
+            for (int j = 0; j < W; ++j) {
+                const int idx = ((dzA + 1) * W + dyi) * W + j;
+                if (rb[j] >= thr && idx != big) s_list[atomicAdd(&ctrl->count[g], 1)] = idx;
+            }
+        }
+    }
+    __syncthreads();
+
+    // ---- M5: write, with the FP64 photo finish where needed
+    const Int3 block = {B, B, B}, window = {R, R, rz};
+    for (int gg = 0; gg < gact; ++gg) {
+        const int4 o = ctrl->org[gg];
+        if (!o.w) continue;                              // flagged by the prep kernel
+        const u64 best = ctrl->best[gg];
+        const int big = (int)(0xffffffffu - (uint32_t)best);
+        const int cnt = ctrl->count[gg];
+        if (cnt == 0) {
+            if (tid == 0) write_result(big, unorder_bits((uint32_t)(best >> 32)), window, b0 + gg, a.out_disp, a.out_ncc);
+            continue;
+        }
+        if (tid == 0) { ctrl->ts.count = cnt; ctrl->ts.best_i = big; }
+        __syncthreads();
+        rescore_and_write(a.fixed, a.moving, dims, block, window, o.x, o.y, o.z,
+                          (const int *)(s_unions + (size_t)gg * a.union_stride), &ctrl->ts, b0 + gg, a.out_disp, a.out_ncc);
+        __syncthreads();
+    }
+}
+
+// ------------------------------------------------------------------------------------------ host side
+struct PairGeom {
+    int G, n_pair_warps, n_single_warps, threads;
+    int pair_lanes_per_block, single_lanes_per_block;
+    int union_stride;
+    size_t smem;
+    double efficiency;          // useful candidate rows / issued row slots
+    int ctas_per_sm;
+};
+
+constexpr size_t kMaxSmemPerCta = 227 * 1024, kSmemPerSm = 228 * 1024;
+
+template <int B, int R>
+bool pair_geometry(int rz, int G, PairGeom *out)
+{
+    using C = PairCfg<B, R>;
+    const int WZ = 2 * rz + 1, UZ = B + 2 * rz, NP = WZ / 2;
+    PairGeom g;
+    g.G = G;
+    g.pair_lanes_per_block = (C::W * NP + 7) / 8 * 8;
+    g.single_lanes_per_block = (C::W + 7) / 8 * 8;
+    g.n_pair_warps = (G * g.pair_lanes_per_block + 31) / 32;
+    g.n_single_warps = (G * g.single_lanes_per_block + 31) / 32;
+    g.threads = (g.n_pair_warps + g.n_single_warps) * 32;
+    g.union_stride = (int)align_up(sizeof(float) * (size_t)UZ * C::UX * C::PITCH, 128);
+    g.smem = (size_t)G * g.union_stride + (size_t)G * C::REC_BYTES + align_up(sizeof(PairCtrl), 16) + 128;
+    if (g.threads > kPairMaxThreads || g.smem > kMaxSmemPerCta) return false;
+    g.efficiency = (double)G * C::W * WZ / 32.0 / (2.0 * g.n_pair_warps + g.n_single_warps);
+    const int by_smem = (int)(kSmemPerSm / (g.smem + 1024));
+    const int by_regs = 65536 / (g.threads * 112);
+    g.ctas_per_sm = by_smem < by_regs ? by_smem : by_regs;
+    if (g.ctas_per_sm < 1) g.ctas_per_sm = 1;
+    *out = g;
+    return true;
+}
+
+template <int B, int R>
+bool pair_plan(int rz, PairGeom *best)
+{
+    bool found = false;
+    double best_score = 0.0;
+    for (int G = 1; G <= kGMax; ++G) {
+        if (g_pair_g && G != g_pair_g) continue;
+        PairGeom g;
+        if (!pair_geometry<B, R>(rz, G, &g)) continue;
+        // a lone CTA per SM cannot overlap its staging with another CTA's arithmetic
+        const double score = g.efficiency * (g.ctas_per_sm >= 2 ? 1.0 : 0.85);
+        if (!found || score > best_score + 1e-9) { found = true; best_score = score; *best = g; }
+    }
+    return found;
+}
+
+// Lane -> task table.  Tasks of block g fill the lane segment [g*L, (g+1)*L); inside it they are grouped into
+// quarter-warps so that the eight LDS.128 row addresses of a quarter fall on distinct 16-byte bank groups
+// where the counts allow it (address of a task, in 16-byte units: P4*dy + PLANE4*dz, PLANE4 = P4*UX).
+void place_tasks(std::vector<uint32_t> &tab, int lane0, int lanes, int g, const std::vector<int> &dy,
+                 const std::vector<int> &p, const std::vector<int> &residue)
+{
+    const int ngroups = lanes / 8;
+    std::vector<std::vector<int>> grp(ngroups);
+    std::vector<std::vector<int>> by_res(8);
+    for (size_t t = 0; t < dy.size(); ++t) by_res[residue[t]].push_back((int)t);
+    std::vector<int> order = {0, 1, 2, 3, 4, 5, 6, 7};
+    for (int i = 0; i < 8; ++i)
+        for (int j = i + 1; j < 8; ++j)
+            if (by_res[order[j]].size() > by_res[order[i]].size()) { int t = order[i]; order[i] = order[j]; order[j] = t; }
+    for (int oi = 0; oi < 8; ++oi) {
+        const int r = order[oi];
+        for (int t : by_res[r]) {
+            int pick = -1, pick_same = 0;
+            size_t pick_load = 0;
+            for (int k = 0; k < ngroups; ++k) {
+                if (grp[k].size() >= 8) continue;
+                int same = 0;
+                for (int u : grp[k]) same += residue[u] == r;
+                if (pick < 0 || same < pick_same || (same == pick_same && grp[k].size() < pick_load)) {
+                    pick = k; pick_same = same; pick_load = grp[k].size();
+                }
+            }
+            grp[pick].push_back(t);
+        }
+    }
+    for (int k = 0; k < ngroups; ++k)
+        for (size_t s = 0; s < grp[k].size(); ++s) {
+            const int t = grp[k][s];
+            tab[lane0 + 8 * k + (int)s] = 0x80000000u | ((uint32_t)g << 16) | ((uint32_t)dy[t] << 8) | (uint32_t)p[t];
+        }
+}
+
+template <int B, int R>
+std::vector<uint32_t> build_task_table(int rz, const PairGeom &g)
+{
+    using C = PairCfg<B, R>;
+    const int WZ = 2 * rz + 1, NP = WZ / 2, P4 = C::PITCH / 4, PLANE4 = P4 * C::UX;
+    std::vector<uint32_t> tab((size_t)g.threads, 0u);
+    for (int blk = 0; blk < g.G; ++blk) {
+        std::vector<int> dy, p, res;
+        for (int pp = 0; pp < NP; ++pp)
+            for (int d = 0; d < C::W; ++d) { dy.push_back(d); p.push_back(pp); res.push_back((P4 * d + PLANE4 * 2 * pp) & 7); }
+        place_tasks(tab, blk * g.pair_lanes_per_block, g.pair_lanes_per_block, blk, dy, p, res);
+        dy.clear(); p.clear(); res.clear();
+        for (int d = 0; d < C::W; ++d) { dy.push_back(d); p.push_back(0); res.push_back((P4 * d + PLANE4 * (WZ - 1)) & 7); }
+        place_tasks(tab, g.n_pair_warps * 32 + blk * g.single_lanes_per_block, g.single_lanes_per_block, blk, dy, p, res);
+    }
+    return tab;
+}
+
+std::mutex g_tab_mutex;
+std::map<long long, uint32_t *> g_tab_cache;      // (device, B, R, rz, G) -> device table
+
+template <int B, int R>
+int task_table_device(int rz, const PairGeom &g, cudaStream_t stream, const uint32_t **out)
+{
+    int dev = 0;
+    NRR_CUDA(cudaGetDevice(&dev));
+    const long long key = ((((long long)dev * 32 + B) * 32 + R) * 512 + rz) * 16 + g.G;
+    std::lock_guard<std::mutex> lock(g_tab_mutex);
+    auto it = g_tab_cache.find(key);
+    if (it != g_tab_cache.end()) { *out = it->second; return NRR_OK; }
+    const std::vector<uint32_t> tab = build_task_table<B, R>(rz, g);
+    uint32_t *d = nullptr;
+    NRR_CUDA(cudaMalloc((void **)&d, tab.size() * sizeof(uint32_t)));
+    // pageable source: the copy is staged before the call returns, so `tab` may go out of scope
+    NRR_CUDA(cudaMemcpyAsync(d, tab.data(), tab.size() * sizeof(uint32_t), cudaMemcpyHostToDevice, stream));
+    NRR_CUDA(cudaStreamSynchronize(stream));
+    g_tab_cache[key] = d;
+    *out = d;
+    return NRR_OK;
+}
+
+template <int B, int R>
+int launch_pair(const float *fixed, const float *moving, const float *inv_sd, Int3 dims, const int *blocks, int n,
+                int rz, int *out_disp, float *out_ncc, unsigned int *err_flag, cudaStream_t stream,
+                MatchPlan *plan_only, bool *handled)
+{
+    using C = PairCfg<B, R>;
+    *handled = false;
+    PairGeom g;
+    if (!pair_plan<B, R>(rz, &g)) return NRR_OK;
+    if (plan_only) {
+        if (!tma_eligible(dims, moving, B + 2 * rz) && moving) return NRR_OK;
+        *handled = true;
+        plan_only->fast = 2;
+        plan_only->threads = g.threads;
+        plan_only->smem_bytes = (int)g.smem;
+        plan_only->tma = 1;
+        plan_only->blocks_per_cta = g.G;
+        return NRR_OK;
+    }
+    if (!tma_eligible(dims, moving, B + 2 * rz)) return NRR_OK;
+    CUtensorMap tm_m;
+    memset(&tm_m, 0, sizeof(tm_m));
+    if (!make_volume_map(&tm_m, moving, dims, C::PITCH, C::UX, B + 2 * rz)) return NRR_OK;
+    *handled = true;
+    const uint32_t *tab = nullptr;
+    int rc = task_table_device<B, R>(rz, g, stream, &tab);
+    if (rc) return rc;
+    float *records = nullptr;
+    NRR_CUDA(cudaMallocAsync((void **)&records, (size_t)n * C::REC_BYTES, stream));
+    auto prep = prep_kernel<B, R>;
+    NRR_LAUNCH(prep, (n + kPrepWarps - 1) / kPrepWarps, kPrepWarps * 32, 0, stream, fixed, dims, blocks, n, records,
+               out_disp, out_ncc, err_flag);
+    NRR_LAUNCH_CHECK("prep_kernel");
+    auto kern = match_pair_kernel<B, R>;
+    static size_t configured_smem = 0;     // per instantiation
+    if (g.smem > configured_smem) {
+        NRR_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem));
+        configured_smem = g.smem;
+    }
+    PairArgs a;
+    a.fixed = fixed; a.moving = moving; a.inv_sd = inv_sd; a.records = records; a.blocks = blocks; a.task_tab = tab;
+    a.out_disp = out_disp; a.out_ncc = out_ncc; a.dims = dims; a.n = n; a.rz = rz; a.G = g.G;
+    a.n_pair_warps = g.n_pair_warps; a.union_stride = g.union_stride; a.tie_band = g_tie_band;
+    NRR_LAUNCH(kern, (n + g.G - 1) / g.G, g.threads, g.smem, stream, tm_m, a);
+    NRR_LAUNCH_CHECK("match_pair_kernel");
+    NRR_CUDA(cudaFreeAsync(records, stream));
+    return NRR_OK;
+}
+
+}  // namespace
+
+// Tries the pair kernel; *handled tells whether it took the call (cubic block 5/7/9/11, in-plane window
+// 3/5/7/9 equal in x and y, TMA-eligible volume).
+int match_pair_dispatch(const float *fixed, const float *moving, const float *inv_sd, Int3 dims, const int *blocks, int n,
+                        Int3 block, Int3 window, int *out_disp, float *out_ncc, unsigned int *err_flag,
+                        cudaStream_t stream, MatchPlan *plan_only, bool *handled)
+{
+    *handled = false;
+    if (!(block.x == block.y && block.y == block.z && window.x == window.y)) return NRR_OK;
+#define NRR_PAIR(BB, RR)                                                                                           \
+    if (block.x == BB && window.x == RR)                                                                           \
+        return launch_pair<BB, RR>(fixed, moving, inv_sd, dims, blocks, n, window.z, out_disp, out_ncc, err_flag, \
+                                   stream, plan_only, handled);
+    NRR_PAIR(5, 3) NRR_PAIR(5, 5) NRR_PAIR(5, 7) NRR_PAIR(5, 9)
+    NRR_PAIR(7, 3) NRR_PAIR(7, 5) NRR_PAIR(7, 7) NRR_PAIR(7, 9)
+    NRR_PAIR(9, 3) NRR_PAIR(9, 5) NRR_PAIR(9, 7) NRR_PAIR(9, 9)
+    NRR_PAIR(11, 3) NRR_PAIR(11, 5) NRR_PAIR(11, 7) NRR_PAIR(11, 9)
+#undef NRR_PAIR
+    return NRR_OK;
+}
+
+}  // namespace nrr

@@ -347,18 +347,18 @@ int select_enqueue(const float *fixed, Int3 dims, Int3 block, Int3 stride, Int3 
     if (ngrid == 0) return NRR_OK;
 
     const unsigned int stats_ctas = (unsigned int)((ngrid + kStatsThreads - 1) / kStatsThreads);
-    stats_kernel<<<stats_ctas, kStatsThreads, 0, stream>>>(fixed, dims, block, stride, grid, ngrid, frac, mask,
-                                                           var, hist, st);
+    NRR_LAUNCH(stats_kernel, stats_ctas, kStatsThreads, 0, stream, fixed, dims, block, stride, grid, ngrid, frac, mask,
+               var, hist, st);
     NRR_LAUNCH_CHECK("stats_kernel");
     const unsigned int chunks = (unsigned int)((ngrid + kChunk - 1) / kChunk);
     for (int pass = 1; pass < kNumPasses; ++pass) {
-        radix_pass_kernel<<<chunks, kScanThreads, 0, stream>>>(var, ngrid, hist + (size_t)pass * kRadixBins, st, pass);
+        NRR_LAUNCH(radix_pass_kernel, chunks, kScanThreads, 0, stream, var, ngrid, hist + (size_t)pass * kRadixBins, st, pass);
         NRR_LAUNCH_CHECK("radix_pass_kernel");
     }
-    count_kernel<<<chunks, kScanThreads, 0, stream>>>(var, ngrid, counts, offsets, st);
+    NRR_LAUNCH(count_kernel, chunks, kScanThreads, 0, stream, var, ngrid, counts, offsets, st);
     NRR_LAUNCH_CHECK("count_kernel");
-    compact_kernel<<<chunks, kScanThreads, 0, stream>>>(var, ngrid, block, stride, grid, offsets, st, out_blocks,
-                                                        out_var, capacity);
+    NRR_LAUNCH(compact_kernel, chunks, kScanThreads, 0, stream, var, ngrid, block, stride, grid, offsets, st, out_blocks,
+               out_var, capacity);
     NRR_LAUNCH_CHECK("compact_kernel");
     return NRR_OK;
 }

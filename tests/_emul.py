@@ -1,0 +1,72 @@
+"""TEST INFRASTRUCTURE ONLY: ctypes access to tests/cuda_emul/libnrr_bm_emul.so, the product's .cu sources
+compiled as plain C++ against a fiber-per-thread CUDA emulation (see tests/cuda_emul/include/cuda_runtime.h).
+It exercises the kernels' logic on the CPU through the same C-ABI host entry points; it is not a product path
+(the package never loads it, and without a CUDA device the product library returns NRR_E_CUDA)."""
+import ctypes
+import importlib.util
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        spec = importlib.util.spec_from_file_location("build_emul", os.path.join(_HERE, "cuda_emul", "build_emul.py"))
+        mod = importlib.util.module_from_spec(spec)
+        spec.loader.exec_module(mod)
+        L = ctypes.CDLL(mod.build())
+        L.nrr_bm_last_error.restype = ctypes.c_char_p
+        L.nrr_bm_set_option.argtypes = [ctypes.c_char_p, ctypes.c_double]
+        vp, ci, cd = ctypes.c_void_p, ctypes.c_int, ctypes.c_double
+        i3 = ctypes.POINTER(ctypes.c_int)
+        L.nrr_bm_select_blocks_host.argtypes = [vp, i3, i3, i3, cd, vp, vp, ci, ctypes.POINTER(ci), vp, ctypes.POINTER(ci)]
+        L.nrr_bm_match_host.argtypes = [vp, vp, i3, vp, ci, i3, i3, vp, vp]
+        L.nrr_bm_match_info.argtypes = [i3, i3, i3, i3]
+        _lib = L
+    return _lib
+
+
+def _i3(t):
+    return (ctypes.c_int * 3)(int(t[0]), int(t[1]), int(t[2]))
+
+
+def _check(rc):
+    if rc != 0:
+        raise RuntimeError("emulated libnrr_bm status %d: %s" % (rc, lib().nrr_bm_last_error().decode()))
+
+
+def set_option(name, value):
+    _check(lib().nrr_bm_set_option(name.encode(), float(value)))
+
+
+def match_info(dims, block, window):
+    info = (ctypes.c_int * 6)()
+    _check(lib().nrr_bm_match_info(_i3(dims), _i3(block), _i3(window), info))
+    return {"kernel": info[0], "threads": info[1], "smem_bytes": info[2], "tma": info[3], "candidates": info[4]}
+
+
+def select(fixed, block, stride, frac, mask=None):
+    nz, ny, nx = fixed.shape
+    cap = max(1, int(np.prod([max(0, ((nx, ny, nz)[a] - block[a]) // stride[a] + 1) for a in range(3)])))
+    blocks = np.empty((cap, 3), np.int32)
+    var = np.empty((cap,), np.float64)
+    n, ncand = ctypes.c_int(0), ctypes.c_int(0)
+    _check(lib().nrr_bm_select_blocks_host(fixed.ctypes.data, _i3((nx, ny, nz)), _i3(block), _i3(stride), float(frac),
+                                           None if mask is None else mask.ctypes.data, blocks.ctypes.data, cap,
+                                           ctypes.byref(n), var.ctypes.data, ctypes.byref(ncand)))
+    return blocks[:n.value], n.value, ncand.value, var[:n.value]
+
+
+def match(fixed, moving, blocks, block, window):
+    nz, ny, nx = fixed.shape
+    blocks = np.ascontiguousarray(blocks, np.int32)
+    n = blocks.shape[0]
+    disp = np.empty((n, 3), np.int32)
+    ncc = np.empty((n,), np.float32)
+    _check(lib().nrr_bm_match_host(fixed.ctypes.data, moving.ctypes.data, _i3((nx, ny, nz)), blocks.ctypes.data, n,
+                                   _i3(block), _i3(window), disp.ctypes.data, ncc.ctypes.data))
+    return disp, ncc

@@ -80,7 +80,7 @@ def test_match_info_dispatch_table(nrr):
         for r in (3, 5, 7, 9):
             info = nrr.nrr_bm_match_info((256, 256, 124), (b, b, b), (r, r, r))
             assert info["fast"] and info["candidates"] == (2 * r + 1) ** 3
-            assert info["threads"] % 32 == 0 and info["threads"] >= (2 * r + 1) ** 2
+            assert info["threads"] % 32 == 0 and 32 <= info["threads"] <= 512
             assert info["smem_bytes"] <= 227 * 1024
     assert nrr.nrr_bm_match_info((256, 256, 60), (7, 7, 7), (5, 5, 3))["fast"]
     assert not nrr.nrr_bm_match_info((256, 256, 60), (7, 5, 7), (5, 5, 3))["fast"]

@@ -1,0 +1,122 @@
+"""CPU tests (-m "not gpu") of the CUDA kernels' LOGIC: the product's .cu sources compiled as plain C++ against
+the fiber-per-thread emulation under tests/cuda_emul, called through the C-ABI host entry points and compared
+with the oracle under the same acceptance rules as the GPU parity tests (tests/_parity.py).  This catches index,
+layout, barrier and tie-rule mistakes without a GPU; it says nothing about hardware behaviour or speed, which the
+-m gpu tests and bench.py cover."""
+import numpy as np
+import pytest
+
+import oracle
+import _emul
+from nrr_inputs import CONFIGS, make_pair, spherical_mask
+from _parity import assert_match_parity, assert_select_parity
+
+
+def _smooth(dims, seed, sigma=1.5):
+    from scipy import ndimage
+    nx, ny, nz = dims
+    v = ndimage.gaussian_filter(np.random.default_rng(seed).standard_normal((nz, ny, nx)), sigma, mode="reflect")
+    return ((v - v.min()) / (v.max() - v.min()) * 1000.0).astype(np.float32)
+
+
+def _shift_noise(vol, s, noise, seed):
+    nz, ny, nx = vol.shape
+    iz = np.clip(np.arange(nz) - s[2], 0, nz - 1)
+    iy = np.clip(np.arange(ny) - s[1], 0, ny - 1)
+    ix = np.clip(np.arange(nx) - s[0], 0, nx - 1)
+    m = vol[np.ix_(iz, iy, ix)].astype(np.float64) + np.random.default_rng(seed).normal(0, noise, size=vol.shape)
+    return np.ascontiguousarray(m, dtype=np.float32)
+
+
+@pytest.fixture(autouse=True)
+def _default_options():
+    for name, v in (("force_rows", 0), ("force_generic", 0), ("disable_tma", 0), ("pair_blocks_per_cta", 0), ("tie_band", 1e-4)):
+        _emul.set_option(name, v)
+    yield
+
+
+@pytest.mark.parametrize("dims,block,stride,frac,mask_r", [
+    ((41, 37, 29), (5, 5, 5), (5, 5, 5), 0.30, None),
+    ((41, 37, 29), (7, 7, 7), (5, 5, 5), 0.25, 15.0),
+    ((41, 37, 29), (3, 5, 7), (4, 3, 2), 0.50, 15.0),
+    ((130, 3, 3), (3, 3, 3), (1, 1, 1), 0.10, None),
+    ((9, 9, 9), (9, 9, 9), (1, 1, 1), 1.00, None),
+])
+def test_emulated_selection_matches_the_oracle(dims, block, stride, frac, mask_r):
+    vol = _smooth(dims, 100 + dims[0])
+    mask = None if mask_r is None else spherical_mask(dims, mask_r)
+    ora = oracle.select(vol, block, stride, frac, mask)
+    blocks, n, ncand, var = _emul.select(vol, block, stride, frac, mask)
+    assert_select_parity(blocks, n, ncand, ora, var)
+
+
+def test_emulated_tiny_config_all_three_matching_kernels():
+    cfg = CONFIGS["tiny"]
+    fixed, moving, mask = make_pair(cfg)
+    ora = oracle.select(fixed, cfg.block, cfg.stride, cfg.frac, mask)
+    blocks, n, ncand, var = _emul.select(fixed, cfg.block, cfg.stride, cfg.frac, mask)
+    assert_select_parity(blocks, n, ncand, ora, var)
+    om = oracle.match(fixed, moving, ora["centres"], cfg.block, cfg.window)
+    dims = fixed.shape[::-1]
+    for opts, kernel in ((dict(), 2), (dict(force_rows=1), 1), (dict(force_generic=1), 0)):
+        for k, v in opts.items():
+            _emul.set_option(k, v)
+        assert _emul.match_info(dims, cfg.block, cfg.window)["kernel"] == kernel
+        disp, ncc = _emul.match(fixed, moving, blocks, cfg.block, cfg.window)
+        assert_match_parity(disp, ncc, om, "tiny kernel %d" % kernel)
+        for k in opts:
+            _emul.set_option(k, 0)
+
+
+def _grid_blocks(dims, block, stride):
+    """Every stride-grid block, borders included (their windows leave the volume: skip rule)."""
+    axes = [np.arange(0, dims[a] - block[a] + 1, stride[a]) + (block[a] - 1) // 2 for a in range(3)]
+    zz, yy, xx = np.meshgrid(axes[2], axes[1], axes[0], indexing="ij")
+    return np.stack([xx.ravel(), yy.ravel(), zz.ravel()], axis=1).astype(np.int32)
+
+
+@pytest.mark.parametrize("dims,b,r,rz,stride,g", [
+    ((28, 26, 22), 5, 3, 3, (7, 7, 8), 0),        # W = 7: 3 pairs + the odd plane
+    ((32, 30, 26), 7, 5, 5, (9, 11, 9), 0),       # the config-3 shape (block 7, window 5); planner's G
+    ((32, 30, 26), 7, 5, 5, (9, 11, 9), 3),       # a group size that leaves a partial last CTA
+    ((32, 30, 24), 7, 5, 3, (12, 11, 8), 0),      # the config-2 shape: anisotropic window (5,5,3)
+    ((36, 34, 30), 9, 7, 7, (13, 12, 10), 0),     # the config-4 shape
+    ((28, 28, 24), 5, 5, 0, (11, 11, 9), 0),      # rz = 0: only the single-row warps work
+    ((32, 30, 30), 11, 3, 3, (10, 9, 9), 0),
+])
+def test_emulated_pair_kernel_matches_the_oracle(dims, b, r, rz, stride, g):
+    fixed = _smooth(dims, 7 + b + r)
+    moving = _shift_noise(fixed, (1, -2, 1), 8.0, 11)
+    block, window = (b, b, b), (r, r, rz)
+    blocks = _grid_blocks(dims, block, stride)
+    _emul.set_option("pair_blocks_per_cta", g)
+    assert _emul.match_info(dims, block, window)["kernel"] == 2
+    om = oracle.match(fixed, moving, blocks, block, window)
+    disp, ncc = _emul.match(fixed, moving, blocks, block, window)
+    assert_match_parity(disp, ncc, om, "pair %s" % (dims,))
+    _emul.set_option("force_rows", 1)                      # the one-row-per-thread kernel on the same input
+    disp, ncc = _emul.match(fixed, moving, blocks, block, window)
+    assert_match_parity(disp, ncc, om, "rows %s" % (dims,))
+
+
+def test_emulated_degenerate_inputs():
+    """Constant regions (zero variance: NCC := 0, lowest index wins), exact ties, blocks that leave the volume."""
+    dims = (24, 24, 20)
+    fixed = _smooth(dims, 3)
+    fixed[:, :, :12] = 500.0                               # constant half: zero-variance fixed blocks and candidates
+    moving = fixed.copy()
+    moving[10:, :, :] = _shift_noise(fixed, (1, 0, 0), 5.0, 5)[10:, :, :]
+    block, window = (5, 5, 5), (3, 3, 3)
+    blocks = _grid_blocks(dims, block, (6, 6, 5))
+    om = oracle.match(fixed, moving, blocks, block, window)
+    for opts in (dict(), dict(force_rows=1), dict(force_generic=1)):
+        for k, v in opts.items():
+            _emul.set_option(k, v)
+        disp, ncc = _emul.match(fixed, moving, blocks, block, window)
+        assert_match_parity(disp, ncc, om, "degenerate %s" % (opts,))
+        for k in opts:
+            _emul.set_option(k, 0)
+    bad = blocks.copy()
+    bad[1] = (1, 2, 2)                                     # origin (-1, 0, 0): leaves the volume
+    with pytest.raises(RuntimeError, match="leaves the volume"):
+        _emul.match(fixed, moving, bad, block, window)
