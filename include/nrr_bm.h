@@ -112,6 +112,20 @@ NRR_BM_API int nrr_bm_select_blocks(const float *fixed, const int dims[3], const
 NRR_BM_API int nrr_bm_match(const float *fixed, const float *moving, const int dims[3], const int *blocks, int n,
                  const int block[3], const int window[3], int *out_disp, float *out_ncc, void *stream);
 
+/*
+ * Per-candidate normalisers of the moving volume (row M2 of the hot path; nrr_bm_match runs this itself,
+ * the entry point exposes it for tests and for callers that match one moving volume against many block lists).
+ * For every block ORIGIN p whose block fits in the volume,
+ *     out_inv_sd[p] = 1 / sqrt( sum over the block at p of (m - mean)^2 ),   0 for a zero-variance block,
+ * i.e. the moving-image factor of NCC's denominator; entries whose block would leave the
+ * volume are left untouched.  Sums are accumulated in FP64; the result is rounded to fp32.
+ *   moving      [in]  device fp32 [nz][ny][nx]        out_inv_sd [out] device fp32 [nz][ny][nx]
+ * Asynchronous on `stream`.  nrr_bm_moving_stats_host: same with HOST buffers, synchronises.
+ */
+NRR_BM_API int nrr_bm_moving_stats(const float *moving, const int dims[3], const int block[3], float *out_inv_sd,
+                        void *stream);
+NRR_BM_API int nrr_bm_moving_stats_host(const float *moving, const int dims[3], const int block[3], float *out_inv_sd);
+
 /* Synchronises `stream` and returns NRR_E_BOUNDS if any nrr_bm_match enqueued on this thread since the last
  * check saw a block leaving the volume (and clears the flag), NRR_E_CUDA on a CUDA error, else NRR_OK. */
 NRR_BM_API int nrr_bm_check_async_error(void *stream);

@@ -20,7 +20,7 @@ NRR_E_NULL, NRR_E_DIMS, NRR_E_BLOCK, NRR_E_STRIDE, NRR_E_WINDOW, NRR_E_FRAC = -1
 NRR_E_CAPACITY, NRR_E_BOUNDS, NRR_E_SMEM, NRR_E_CUDA, NRR_E_ARG = -7, -8, -9, -10, -11
 
 EXPORTS = [
-    "nrr_bm_select_blocks", "nrr_bm_match", "nrr_bm_check_async_error",
+    "nrr_bm_select_blocks", "nrr_bm_match", "nrr_bm_check_async_error", "nrr_bm_moving_stats", "nrr_bm_moving_stats_host",
     "nrr_bm_select_blocks_host", "nrr_bm_match_host", "nrr_bm_register_host",
     "nrr_bm_profile_enable", "nrr_bm_profile_read", "nrr_bm_launch_count", "nrr_bm_match_info",
     "nrr_bm_fp32_peak", "nrr_bm_set_option", "nrr_bm_last_error", "nrr_bm_status_string", "nrr_bm_version",
@@ -51,6 +51,10 @@ def lib() -> ctypes.CDLL:
     L.nrr_bm_select_blocks.argtypes = [vp, i3, i3, i3, cd, vp, vp, ci, i3, vp, i3, vp]
     L.nrr_bm_match.restype = ci
     L.nrr_bm_match.argtypes = [vp, vp, i3, vp, ci, i3, i3, vp, vp, vp]
+    L.nrr_bm_moving_stats.restype = ci
+    L.nrr_bm_moving_stats.argtypes = [vp, i3, i3, vp, vp]
+    L.nrr_bm_moving_stats_host.restype = ci
+    L.nrr_bm_moving_stats_host.argtypes = [vp, i3, i3, vp]
     L.nrr_bm_check_async_error.restype = ci
     L.nrr_bm_check_async_error.argtypes = [vp]
     L.nrr_bm_select_blocks_host.restype = ci
@@ -167,6 +171,19 @@ def nrr_bm_match(fixed, moving, blocks, block, window, out_disp=None, out_ncc=No
         _check(lib().nrr_bm_match(fixed.data_ptr(), moving.data_ptr(), _i3(_dims_of(fixed)), blocks.data_ptr(), n,
                                   _i3(block), _i3(window), out_disp.data_ptr(), out_ncc.data_ptr(), _stream_ptr(stream)))
     return out_disp, out_ncc
+
+
+def nrr_bm_moving_stats(moving, block, out_inv_sd=None, stream=None):
+    """Device form, asynchronous. Returns inv_sd fp32 CUDA [nz][ny][nx] (entries whose block leaves the volume untouched)."""
+    import torch
+    moving = _dev(moving, torch.float32, "moving")
+    if out_inv_sd is None:
+        out_inv_sd = torch.zeros_like(moving)
+    out_inv_sd = _dev(out_inv_sd, torch.float32, "out_inv_sd")
+    with torch.cuda.device(moving.device):
+        _check(lib().nrr_bm_moving_stats(moving.data_ptr(), _i3(_dims_of(moving)), _i3(block), out_inv_sd.data_ptr(),
+                                         _stream_ptr(stream)))
+    return out_inv_sd
 
 
 def nrr_bm_check_async_error(stream=None) -> None:

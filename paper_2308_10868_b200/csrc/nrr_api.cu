@@ -16,6 +16,8 @@ extern int g_force_generic;
 extern int g_disable_tma;
 extern int g_force_rows;
 extern int g_pair_g;
+extern int g_boxstat_generic;
+extern int g_select_generic;
 
 namespace {
 
@@ -261,6 +263,34 @@ int nrr_bm_match(const float *fixed, const float *moving, const int dims[3], con
     return match_device(fixed, moving, dims, blocks, n, block, window, out_disp, out_ncc, (cudaStream_t)stream);
 }
 
+int nrr_bm_moving_stats(const float *moving, const int dims[3], const int block[3], float *out_inv_sd, void *stream)
+{
+    if (!moving || !out_inv_sd) return fail(NRR_E_NULL, "moving/out_inv_sd is NULL");
+    int rc = check_dims_block(dims, block);
+    if (rc) return rc;
+    if ((rc = ensure_thread_state())) return rc;
+    return boxstat_enqueue(moving, i3(dims), i3(block), out_inv_sd, (cudaStream_t)stream);
+}
+
+int nrr_bm_moving_stats_host(const float *moving, const int dims[3], const int block[3], float *out_inv_sd)
+{
+    if (!moving || !out_inv_sd) return fail(NRR_E_NULL, "moving/out_inv_sd is NULL");
+    int rc = check_dims_block(dims, block);
+    if (rc) return rc;
+    if ((rc = ensure_thread_state())) return rc;
+    cudaStream_t s;
+    if ((rc = host_stream(&s))) return rc;
+    const size_t nvox = (size_t)dims[0] * dims[1] * dims[2];
+    DevBuf d_moving(s), d_out(s);
+    NRR_CUDA(d_moving.upload(moving, nvox * sizeof(float)));
+    NRR_CUDA(d_out.upload(out_inv_sd, nvox * sizeof(float)));      // untouched entries keep the caller's values
+    rc = boxstat_enqueue((const float *)d_moving.p, i3(dims), i3(block), (float *)d_out.p, s);
+    if (rc) return rc;
+    NRR_CUDA(cudaMemcpyAsync(out_inv_sd, d_out.p, nvox * sizeof(float), cudaMemcpyDeviceToHost, s));
+    NRR_CUDA(cudaStreamSynchronize(s));
+    return NRR_OK;
+}
+
 int nrr_bm_check_async_error(void *stream) { return check_async((cudaStream_t)stream); }
 
 int nrr_bm_select_blocks_host(const float *fixed, const int dims[3], const int block[3], const int stride[3],
@@ -403,6 +433,8 @@ int nrr_bm_set_option(const char *name, double value)
     if (!strcmp(name, "tie_band")) { g_tie_band = (float)value; return NRR_OK; }
     if (!strcmp(name, "force_generic")) { g_force_generic = value != 0.0; return NRR_OK; }
     if (!strcmp(name, "disable_tma")) { g_disable_tma = value != 0.0; return NRR_OK; }
+    if (!strcmp(name, "select_generic")) { g_select_generic = value != 0.0; return NRR_OK; }
+    if (!strcmp(name, "boxstat_generic")) { g_boxstat_generic = value != 0.0; return NRR_OK; }
     if (!strcmp(name, "force_rows")) { g_force_rows = value != 0.0; return NRR_OK; }
     if (!strcmp(name, "pair_blocks_per_cta")) { g_pair_g = (int)value; return NRR_OK; }
     return fail(NRR_E_ARG, "unknown option '%s'", name);

@@ -18,6 +18,8 @@
 
 namespace nrr {
 
+int g_boxstat_generic = 0;      // != 0: always use the generic (any block shape) kernel
+
 namespace {
 
 constexpr int TX = 32, TY = 8, ZCHUNK = 32;
@@ -93,12 +95,173 @@ boxstat_kernel(const float *__restrict__ vol, Int3 dims, Int3 block, float *__re
     }
 }
 
+
+// ------------------------------------------------------------------------------------------ sliding kernel
+// Cubic blocks B in {5,7,9,11}.  One CTA owns a TX x TY tile of ORIGINS and marches over a chunk of z.
+//   z : every thread owns NCOL input columns (x,y) of the haloed tile and keeps, per column, the running FP64
+//       sums of m and m^2 over the last B planes (the plane that leaves the window is read again: an L2 hit);
+//   x : the z-summed plane goes to shared memory; a thread per (row, 8 origins) slides the B-wide window;
+//   y : a thread per (column, TY/2 origins) slides along y and writes inv_sd, coalesced along x.
+// O(1) FP64 additions per voxel and axis; traffic: each input plane is read once per CTA column (halo
+// (TX+B-1)(TY+B-1)/(TX TY)), each origin written once.
+template <int B>
+struct SlideCfg {
+    static constexpr int NT = 256;
+    static constexpr int TX = 64;
+    static constexpr int TY = B <= 7 ? 18 : (B == 9 ? 16 : 14);
+    static constexpr int HX = TX + B - 1, HY = TY + B - 1;
+    static constexpr int NCOL = (HX * HY + NT - 1) / NT;
+    static constexpr int ZP = HX | 1;            // pitch of s_z rows, in double2 (odd: conflict-free column walks)
+    static constexpr int RP = HY | 1;            // pitch of s_row columns, in double2
+    static constexpr int XS = 8;                 // origins per x-pass thread
+    static constexpr int YS = TY / 2;            // origins per y-pass thread
+    static constexpr size_t SMEM = sizeof(double2) * ((size_t)HY * ZP + (size_t)TX * RP);
+    static_assert(HY * (TX / XS) <= NT && TX * 2 <= NT, "pass tasks must fit the CTA");
+};
+
+template <int B>
+__global__ void __launch_bounds__(256, 2)
+boxstat_slide_kernel(const float *__restrict__ vol, Int3 dims, int zchunk, float *__restrict__ inv_sd)
+{
+    using C = SlideCfg<B>;
+    constexpr int TX = C::TX, TY = C::TY, HX = C::HX, HY = C::HY, NCOL = C::NCOL, ZP = C::ZP, RP = C::RP;
+    NRR_DYN_SMEM(s_dyn);
+    double2 *s_z = (double2 *)s_dyn;             // [HY][ZP]  z-window sums of the current plane
+    double2 *s_row = s_z + (size_t)HY * ZP;      // [TX][RP]  x-window sums, transposed
+
+    const int tid = threadIdx.x;
+    const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY, z0 = blockIdx.z * zchunk;
+    const int nzo = dims.z - B + 1;
+    const int zo_end = min(z0 + zchunk, nzo);
+    if (z0 >= zo_end) return;                    // uniform over the CTA
+    const int zi_end = zo_end + B - 1;
+    const size_t plane = (size_t)dims.x * dims.y;
+    const double nvox = (double)(B * B * B);
+
+    int gofs[NCOL], sidx[NCOL];                  // global offset inside a plane (-1: outside the volume), s_z slot (-1: none)
+#pragma unroll
+    for (int c = 0; c < NCOL; ++c) {
+        const int i = tid + c * C::NT;
+        const int ly = i / HX, lx = i - ly * HX;
+        const int gx = x0 + lx, gy = y0 + ly;
+        sidx[c] = i < HX * HY ? ly * ZP + lx : -1;
+        gofs[c] = (i < HX * HY && gx < dims.x && gy < dims.y) ? gy * dims.x + gx : -1;
+    }
+    double z1[NCOL], z2[NCOL];
+#pragma unroll
+    for (int c = 0; c < NCOL; ++c) { z1[c] = 0.0; z2[c] = 0.0; }
+
+    for (int zi = z0; zi < zi_end; ++zi) {
+        {
+            const bool emit = zi - z0 >= B - 1;  // uniform: the window is full, plane zo = zi - (B-1) is due
+            const bool drop = zi - z0 >= B;      // uniform: plane zi - B leaves the window (re-read: an L2 hit)
+            float vn[NCOL], vl[NCOL];
+#pragma unroll
+            for (int c = 0; c < NCOL; ++c) {
+                vn[c] = gofs[c] >= 0 ? __ldg(vol + (size_t)zi * plane + gofs[c]) : 0.f;
+                vl[c] = (drop && gofs[c] >= 0) ? __ldg(vol + (size_t)(zi - B) * plane + gofs[c]) : 0.f;
+            }
+#pragma unroll
+            for (int c = 0; c < NCOL; ++c) {
+                const double dn = (double)vn[c], dl = (double)vl[c];
+                z1[c] += dn - dl;
+                z2[c] = fma(dn, dn, z2[c]);
+                z2[c] = fma(-dl, dl, z2[c]);
+                if (emit && sidx[c] >= 0) s_z[sidx[c]] = make_double2(z1[c], z2[c]);
+            }
+            if (!emit) continue;
+            __syncthreads();
+            // x pass: thread = (row r, 8 consecutive origins), lanes walk r
+            if (tid < HY * (TX / C::XS)) {
+                const int r = tid % HY, xs = (tid / HY) * C::XS;
+                const double2 *zr = s_z + (size_t)r * ZP + xs;
+                double a = 0.0, b = 0.0;
+#pragma unroll
+                for (int j = 0; j < B; ++j) { a += zr[j].x; b += zr[j].y; }
+                s_row[(size_t)xs * RP + r] = make_double2(a, b);
+#pragma unroll
+                for (int j = 1; j < C::XS; ++j) {
+                    const double2 in = zr[j + B - 1], out = zr[j - 1];
+                    a += in.x - out.x;
+                    b += in.y - out.y;
+                    s_row[(size_t)(xs + j) * RP + r] = make_double2(a, b);
+                }
+            }
+            __syncthreads();
+            // y pass: thread = (column x, TY/2 consecutive origins), lanes walk x; writes are coalesced along x
+            if (tid < TX * 2) {
+                const int x = tid % TX, ys = (tid / TX) * C::YS;
+                const double2 *col = s_row + (size_t)x * RP + ys;
+                const int gx = x0 + x, zo = zi - (B - 1);
+                const bool x_ok = gx <= dims.x - B;
+                double a = 0.0, b = 0.0;
+#pragma unroll
+                for (int j = 0; j < B; ++j) { a += col[j].x; b += col[j].y; }
+#pragma unroll
+                for (int j = 0; j < C::YS; ++j) {
+                    if (j > 0) {
+                        const double2 in = col[j + B - 1], out = col[j - 1];
+                        a += in.x - out.x;
+                        b += in.y - out.y;
+                    }
+                    const int gy = y0 + ys + j;
+                    if (x_ok && gy <= dims.y - B) {
+                        const double ss = b - a * a / nvox;
+                        float rr = 0.f;
+                        if (ss > b * 9.094947017729282e-13 /* 2^-40 */) rr = rsqrtf((float)ss);
+                        inv_sd[(size_t)zo * plane + (size_t)gy * dims.x + gx] = rr;
+                    }
+                }
+            }
+            // the next plane's s_z stores follow this thread's y pass; every x-pass read of s_z precedes the
+            // barrier above, and the next x pass writes s_row only behind the next plane's first barrier
+        }
+    }
+}
+
+template <int B>
+int launch_slide(const float *moving, Int3 dims, float *inv_sd, cudaStream_t stream)
+{
+    using C = SlideCfg<B>;
+    const int nxo = dims.x - B + 1, nyo = dims.y - B + 1, nzo = dims.z - B + 1;
+    const int gx = (nxo + C::TX - 1) / C::TX, gy = (nyo + C::TY - 1) / C::TY;
+    // enough CTAs for two per SM; chunks of at least 2B planes keep the z halo below 50 %
+    int zsplit = (2 * 148 + gx * gy - 1) / (gx * gy);
+    const int max_split = (nzo + 2 * B - 1) / (2 * B);
+    if (zsplit > max_split) zsplit = max_split;
+    if (zsplit < 1) zsplit = 1;
+    const int zchunk = (nzo + zsplit - 1) / zsplit;
+    zsplit = (nzo + zchunk - 1) / zchunk;
+    if (gy > 65535 || zsplit > 65535) {
+        set_error("volume too large for the moving-volume statistics grid");
+        return NRR_E_DIMS;
+    }
+    auto kern = boxstat_slide_kernel<B>;
+    static bool configured = false;
+    if (!configured) {
+        NRR_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM));
+        configured = true;
+    }
+    NRR_LAUNCH(kern, dim3(gx, gy, zsplit), C::NT, C::SMEM, stream, moving, dims, zchunk, inv_sd);
+    NRR_LAUNCH_CHECK("boxstat_slide_kernel");
+    return NRR_OK;
+}
+
 }  // namespace
 
 int boxstat_enqueue(const float *moving, Int3 dims, Int3 block, float *inv_sd, cudaStream_t stream)
 {
     const int nxo = dims.x - block.x + 1, nyo = dims.y - block.y + 1, nzo = dims.z - block.z + 1;
     if (nxo < 1 || nyo < 1 || nzo < 1) return NRR_OK;
+    if (!g_boxstat_generic && block.x == block.y && block.y == block.z) {
+        switch (block.x) {
+        case 5: return launch_slide<5>(moving, dims, inv_sd, stream);
+        case 7: return launch_slide<7>(moving, dims, inv_sd, stream);
+        case 9: return launch_slide<9>(moving, dims, inv_sd, stream);
+        case 11: return launch_slide<11>(moving, dims, inv_sd, stream);
+        default: break;
+        }
+    }
     const int HX = TX + block.x - 1, HY = TY + block.y - 1;
     const size_t smem = sizeof(double2) * ((size_t)HY * TX + (size_t)block.z * kThreads) + sizeof(float) * (size_t)HX * HY;
     if (smem > 200 * 1024) {

@@ -17,6 +17,8 @@
 
 namespace nrr {
 
+int g_select_generic = 0;       // != 0: runtime-shaped statistics kernel and the multi-launch radix select
+
 namespace {
 
 constexpr int kRadixBins = 2048;
@@ -43,8 +45,9 @@ __device__ __forceinline__ unsigned int digit_of(unsigned long long key, int pas
 
 // Block-wide: the calling CTA (all threads) picks the radix digit of pass `pass` that contains the
 // k_remaining-th largest key of the current prefix bucket, from the global histogram `hist`.
-__device__ void pick_digit(const unsigned int *hist, SelectState *st, int pass)
+__device__ void pick_digit(const unsigned int *hist_, SelectState *st, int pass)
 {
+    const volatile unsigned int *hist = hist_;      // global (written by other CTAs before the ticket) or shared
     __shared__ unsigned int s_warp[32];
     __shared__ unsigned int s_found_bin, s_found_cum;
     const int nbins = 1 << c_width[pass];
@@ -56,7 +59,7 @@ __device__ void pick_digit(const unsigned int *hist, SelectState *st, int pass)
     unsigned int local = 0;
     for (int i = 0; i < per; ++i) {
         int bin = nbins - 1 - (tid * per + i);
-        if (bin >= 0) local += __ldcg(hist + bin);
+        if (bin >= 0) local += hist[bin];
     }
     // inclusive scan of `local` over the CTA
     unsigned int incl = local;
@@ -77,7 +80,7 @@ __device__ void pick_digit(const unsigned int *hist, SelectState *st, int pass)
         for (int i = 0; i < per; ++i) {
             int bin = nbins - 1 - (tid * per + i);
             if (bin < 0) break;
-            unsigned int c = __ldcg(hist + bin);
+            unsigned int c = hist[bin];
             if (cum + c >= k) { s_found_bin = (unsigned int)bin; s_found_cum = cum; break; }
             cum += c;
         }
@@ -107,7 +110,84 @@ __device__ bool flush_hist_and_ticket(unsigned int *s_hist, unsigned int *g_hist
     return s_last;
 }
 
-// S1 + S2 + radix pass 0.
+// Two-pass population variance of the block at origin (ox,oy,oz): every operation individually rounded
+// (no contraction), summation in x-fastest order -- the same sequence of IEEE operations as the oracle.
+__device__ double block_variance(const float *__restrict__ fixed, Int3 dims, Int3 block, int ox, int oy, int oz)
+{
+    const double nvox = (double)((long long)block.x * block.y * block.z);
+    double s = 0.0;
+    for (int z = 0; z < block.z; ++z)
+        for (int y = 0; y < block.y; ++y) {
+            const float *row = fixed + ((size_t)(oz + z) * dims.y + (oy + y)) * dims.x + ox;
+            for (int x = 0; x < block.x; ++x) s = __dadd_rn(s, (double)__ldg(row + x));
+        }
+    const double mean = __ddiv_rn(s, nvox);
+    double q = 0.0;
+    for (int z = 0; z < block.z; ++z)
+        for (int y = 0; y < block.y; ++y) {
+            const float *row = fixed + ((size_t)(oz + z) * dims.y + (oy + y)) * dims.x + ox;
+            for (int x = 0; x < block.x; ++x) {
+                const double d = __dsub_rn((double)__ldg(row + x), mean);
+                q = __dadd_rn(q, __dmul_rn(d, d));
+            }
+        }
+    return __ddiv_rn(q, nvox);
+}
+
+// Same arithmetic, same order, for a cubic block of compile-time edge B: the loads of a whole z-plane are
+// independent of the running sum, so they are issued ahead of the (inherently serial) chain of additions.
+template <int B>
+__device__ double block_variance_cubic(const float *__restrict__ fixed, Int3 dims, int ox, int oy, int oz)
+{
+    constexpr int RY = B <= 7 ? B : (B == 9 ? 5 : 4);      // rows loaded ahead of the additions (<= 49 values)
+    const double nvox = (double)(B * B * B);
+    const size_t plane = (size_t)dims.x * dims.y;
+    const float *org = fixed + ((size_t)oz * dims.y + oy) * dims.x + ox;
+    double s = 0.0;
+#pragma unroll 1
+    for (int z = 0; z < B; ++z) {
+#pragma unroll
+        for (int y0 = 0; y0 < B; y0 += RY) {
+            float v[RY * B];
+#pragma unroll
+            for (int y = 0; y < RY; ++y)
+#pragma unroll
+                for (int x = 0; x < B; ++x)
+                    if (y0 + y < B) v[y * B + x] = __ldg(org + z * plane + (size_t)(y0 + y) * dims.x + x);
+#pragma unroll
+            for (int y = 0; y < RY; ++y)
+#pragma unroll
+                for (int x = 0; x < B; ++x)
+                    if (y0 + y < B) s = __dadd_rn(s, (double)v[y * B + x]);
+        }
+    }
+    const double mean = __ddiv_rn(s, nvox);
+    double q = 0.0;
+#pragma unroll 1
+    for (int z = 0; z < B; ++z) {
+#pragma unroll
+        for (int y0 = 0; y0 < B; y0 += RY) {
+            float v[RY * B];
+#pragma unroll
+            for (int y = 0; y < RY; ++y)
+#pragma unroll
+                for (int x = 0; x < B; ++x)
+                    if (y0 + y < B) v[y * B + x] = __ldg(org + z * plane + (size_t)(y0 + y) * dims.x + x);
+#pragma unroll
+            for (int y = 0; y < RY; ++y)
+#pragma unroll
+                for (int x = 0; x < B; ++x)
+                    if (y0 + y < B) {
+                        const double d = __dsub_rn((double)v[y * B + x], mean);
+                        q = __dadd_rn(q, __dmul_rn(d, d));
+                    }
+        }
+    }
+    return __ddiv_rn(q, nvox);
+}
+
+// S1 + S2 + radix pass 0.  CB = compile-time cubic block edge, 0 = any block shape.
+template <int CB>
 __global__ void __launch_bounds__(kStatsThreads)
 stats_kernel(const float *__restrict__ fixed, Int3 dims, Int3 block, Int3 stride, Int3 grid, long long ngrid,
              double frac, const unsigned char *__restrict__ mask, double *__restrict__ var,
@@ -128,24 +208,8 @@ stats_kernel(const float *__restrict__ fixed, Int3 dims, Int3 block, Int3 stride
         in = (mask == nullptr) || mask[((size_t)cz * dims.y + cy) * dims.x + cx] != 0;
         double v = -1.0;
         if (in) {
-            const double nvox = (double)((long long)block.x * block.y * block.z);
-            double s = 0.0;
-            for (int z = 0; z < block.z; ++z)
-                for (int y = 0; y < block.y; ++y) {
-                    const float *row = fixed + ((size_t)(oz + z) * dims.y + (oy + y)) * dims.x + ox;
-                    for (int x = 0; x < block.x; ++x) s = __dadd_rn(s, (double)__ldg(row + x));
-                }
-            const double mean = __ddiv_rn(s, nvox);
-            double q = 0.0;
-            for (int z = 0; z < block.z; ++z)
-                for (int y = 0; y < block.y; ++y) {
-                    const float *row = fixed + ((size_t)(oz + z) * dims.y + (oy + y)) * dims.x + ox;
-                    for (int x = 0; x < block.x; ++x) {
-                        const double d = __dsub_rn((double)__ldg(row + x), mean);
-                        q = __dadd_rn(q, __dmul_rn(d, d));
-                    }
-                }
-            v = __ddiv_rn(q, nvox);
+            if constexpr (CB > 0) v = block_variance_cubic<CB>(fixed, dims, ox, oy, oz);
+            else v = block_variance(fixed, dims, block, ox, oy, oz);
             atomicAdd(&s_hist[digit_of(key_of(v), 0)], 1u);
         }
         var[g] = v;
@@ -306,6 +370,77 @@ compact_kernel(const double *__restrict__ var, long long ngrid, Int3 block, Int3
     }
 }
 
+// ---- small grids: passes 1..5, the threshold counts and the compaction in ONE single-CTA launch.
+// 60,000 keys (config 3) are 59 keys per thread and pass; seven tiny launches cost more than the work.
+constexpr int kSmallThreads = 1024;
+constexpr long long kSmallLimit = 1ll << 20;      // grid positions up to which the single-CTA tail is used
+
+__global__ void __launch_bounds__(kSmallThreads)
+select_small_kernel(const double *__restrict__ var, long long ngrid, Int3 block, Int3 stride, Int3 grid,
+                    SelectState *st, int *__restrict__ out_blocks, double *__restrict__ out_var, int capacity)
+{
+    __shared__ unsigned int s_hist[kRadixBins];
+    __shared__ unsigned long long s_carry;
+    const int tid = threadIdx.x;
+    for (int pass = 1; pass < kNumPasses; ++pass) {
+        for (int b = tid; b < kRadixBins; b += kSmallThreads) s_hist[b] = 0;
+        __syncthreads();
+        const unsigned long long prefix = st->prefix, mask = st->mask;
+        for (long long g = tid; g < ngrid; g += kSmallThreads) {
+            const unsigned long long key = key_of(var[g]);
+            if ((key & mask) == prefix) atomicAdd(&s_hist[digit_of(key, pass)], 1u);
+        }
+        __syncthreads();
+        pick_digit(s_hist, st, pass);      // thread 0 updates *st; the barrier below publishes it to the CTA
+        __syncthreads();
+    }
+    const unsigned int K = st->k;
+    if (K == 0) return;
+    const unsigned long long T = st->prefix;
+    const unsigned int ties = st->k_remaining;
+    if (tid == 0) s_carry = 0ull;
+    __syncthreads();
+    constexpr int IPT = 4;
+    for (long long start = 0; start < ngrid; start += (long long)kSmallThreads * IPT) {
+        const long long base = start + (long long)tid * IPT;
+        unsigned long long keys[IPT];
+        unsigned int gt = 0, eq = 0;
+#pragma unroll
+        for (int i = 0; i < IPT; ++i) {
+            const long long g = base + i;
+            keys[i] = g < ngrid ? key_of(var[g]) : 0ull;
+            gt += keys[i] > T;
+            eq += (keys[i] == T) && (g < ngrid);
+        }
+        unsigned long long tot;
+        const unsigned long long ex = block_exclusive_scan_u64(pack_counts(gt, eq), &tot) + s_carry;
+        unsigned int gt_before = (unsigned int)(ex >> 32), eq_before = (unsigned int)(ex & 0xffffffffu);
+#pragma unroll
+        for (int i = 0; i < IPT; ++i) {
+            const long long g = base + i;
+            if (g >= ngrid) break;
+            const bool is_gt = keys[i] > T, is_eq = keys[i] == T;
+            if (is_gt || (is_eq && eq_before < ties)) {
+                const unsigned int pos = gt_before + (eq_before < ties ? eq_before : ties);
+                if (pos < (unsigned int)capacity) {
+                    const int gi = (int)(g % grid.x);
+                    const int gj = (int)((g / grid.x) % grid.y);
+                    const int gk = (int)(g / ((long long)grid.x * grid.y));
+                    out_blocks[3 * (size_t)pos + 0] = gi * stride.x + (block.x - 1) / 2;
+                    out_blocks[3 * (size_t)pos + 1] = gj * stride.y + (block.y - 1) / 2;
+                    out_blocks[3 * (size_t)pos + 2] = gk * stride.z + (block.z - 1) / 2;
+                    if (out_var) out_var[pos] = var[g];
+                }
+            }
+            gt_before += is_gt;
+            eq_before += is_eq;
+        }
+        __syncthreads();                   // every thread has read s_carry
+        if (tid == 0) s_carry += tot;
+        __syncthreads();
+    }
+}
+
 struct ScratchLayout {
     size_t state, hist, var, counts, offsets, total;
 };
@@ -347,9 +482,23 @@ int select_enqueue(const float *fixed, Int3 dims, Int3 block, Int3 stride, Int3 
     if (ngrid == 0) return NRR_OK;
 
     const unsigned int stats_ctas = (unsigned int)((ngrid + kStatsThreads - 1) / kStatsThreads);
-    NRR_LAUNCH(stats_kernel, stats_ctas, kStatsThreads, 0, stream, fixed, dims, block, stride, grid, ngrid, frac, mask,
-               var, hist, st);
+    void (*stats)(const float *, Int3, Int3, Int3, Int3, long long, double, const unsigned char *, double *,
+                  unsigned int *, SelectState *) = stats_kernel<0>;
+    if (!g_select_generic && block.x == block.y && block.y == block.z) {
+        if (block.x == 5) stats = stats_kernel<5>;
+        else if (block.x == 7) stats = stats_kernel<7>;
+        else if (block.x == 9) stats = stats_kernel<9>;
+        else if (block.x == 11) stats = stats_kernel<11>;
+    }
+    NRR_LAUNCH(stats, stats_ctas, kStatsThreads, 0, stream, fixed, dims, block, stride, grid, ngrid, frac, mask, var,
+               hist, st);
     NRR_LAUNCH_CHECK("stats_kernel");
+    if (!g_select_generic && ngrid <= kSmallLimit) {
+        NRR_LAUNCH(select_small_kernel, 1, kSmallThreads, 0, stream, var, ngrid, block, stride, grid, st, out_blocks,
+                   out_var, capacity);
+        NRR_LAUNCH_CHECK("select_small_kernel");
+        return NRR_OK;
+    }
     const unsigned int chunks = (unsigned int)((ngrid + kChunk - 1) / kChunk);
     for (int pass = 1; pass < kNumPasses; ++pass) {
         NRR_LAUNCH(radix_pass_kernel, chunks, kScanThreads, 0, stream, var, ngrid, hist + (size_t)pass * kRadixBins, st, pass);

@@ -26,6 +26,7 @@ def lib():
         L.nrr_bm_select_blocks_host.argtypes = [vp, i3, i3, i3, cd, vp, vp, ci, ctypes.POINTER(ci), vp, ctypes.POINTER(ci)]
         L.nrr_bm_match_host.argtypes = [vp, vp, i3, vp, ci, i3, i3, vp, vp]
         L.nrr_bm_match_info.argtypes = [i3, i3, i3, i3]
+        L.nrr_bm_moving_stats_host.argtypes = [vp, i3, i3, vp]
         _lib = L
     return _lib
 
@@ -70,3 +71,10 @@ def match(fixed, moving, blocks, block, window):
     _check(lib().nrr_bm_match_host(fixed.ctypes.data, moving.ctypes.data, _i3((nx, ny, nz)), blocks.ctypes.data, n,
                                    _i3(block), _i3(window), disp.ctypes.data, ncc.ctypes.data))
     return disp, ncc
+
+
+def moving_stats(moving, block, fill=-7.0):
+    nz, ny, nx = moving.shape
+    out = np.full(moving.shape, fill, np.float32)
+    _check(lib().nrr_bm_moving_stats_host(moving.ctypes.data, _i3((nx, ny, nz)), _i3(block), out.ctypes.data))
+    return out

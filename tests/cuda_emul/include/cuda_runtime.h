@@ -226,3 +226,4 @@ static inline double __ddiv_rn(double a, double b) { return a / b; }
 static inline size_t __cvta_generic_to_shared(const void *p) { return (size_t)p; }
 using std::max;
 using std::min;
+static inline float rsqrtf(float x) { return 1.0f / sqrtf(x); }

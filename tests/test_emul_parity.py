@@ -30,7 +30,8 @@ def _shift_noise(vol, s, noise, seed):
 
 @pytest.fixture(autouse=True)
 def _default_options():
-    for name, v in (("force_rows", 0), ("force_generic", 0), ("disable_tma", 0), ("pair_blocks_per_cta", 0), ("tie_band", 1e-4)):
+    for name, v in (("force_rows", 0), ("force_generic", 0), ("disable_tma", 0), ("pair_blocks_per_cta", 0), ("tie_band", 1e-4),
+                    ("select_generic", 0), ("boxstat_generic", 0)):
         _emul.set_option(name, v)
     yield
 
@@ -46,8 +47,29 @@ def test_emulated_selection_matches_the_oracle(dims, block, stride, frac, mask_r
     vol = _smooth(dims, 100 + dims[0])
     mask = None if mask_r is None else spherical_mask(dims, mask_r)
     ora = oracle.select(vol, block, stride, frac, mask)
-    blocks, n, ncand, var = _emul.select(vol, block, stride, frac, mask)
+    for generic in (0, 1):       # single-CTA tail + unrolled statistics / multi-launch radix select + runtime shapes
+        _emul.set_option("select_generic", generic)
+        blocks, n, ncand, var = _emul.select(vol, block, stride, frac, mask)
+        assert_select_parity(blocks, n, ncand, ora, var)
+    _emul.set_option("select_generic", 0)
+
+
+def test_emulated_selection_ties_go_to_the_lower_index():
+    vol = np.full((12, 15, 20), 42.0, dtype=np.float32)            # uniform image: first K grid positions
+    ora = oracle.select(vol, (3, 3, 3), (3, 3, 3), 0.25)
+    blocks, n, ncand, var = _emul.select(vol, (3, 3, 3), (3, 3, 3), 0.25)
     assert_select_parity(blocks, n, ncand, ora, var)
+    vol2 = np.zeros((10, 10, 30), dtype=np.float32)                # the same pattern three times: exact variance ties
+    pat = np.arange(125, dtype=np.float32).reshape(5, 5, 5)
+    for x in (0, 10, 25):
+        vol2[0:5, 5:10, x:x + 5] = pat
+    for frac in (0.1, 0.17, 0.34):                                  # K cuts through the tied group
+        ora = oracle.select(vol2, (5, 5, 5), (5, 5, 5), frac)
+        for generic in (0, 1):
+            _emul.set_option("select_generic", generic)
+            blocks, n, ncand, var = _emul.select(vol2, (5, 5, 5), (5, 5, 5), frac)
+            assert_select_parity(blocks, n, ncand, ora, var)
+    _emul.set_option("select_generic", 0)
 
 
 def test_emulated_tiny_config_all_three_matching_kernels():
@@ -120,3 +142,33 @@ def test_emulated_degenerate_inputs():
     bad[1] = (1, 2, 2)                                     # origin (-1, 0, 0): leaves the volume
     with pytest.raises(RuntimeError, match="leaves the volume"):
         _emul.match(fixed, moving, bad, block, window)
+
+
+@pytest.mark.parametrize("dims,block,generic", [
+    ((70, 45, 33), (7, 7, 7), 0),        # sliding kernel: two x tiles, ragged y and z, several z chunks
+    ((70, 45, 33), (7, 7, 7), 1),        # generic kernel on the same input
+    ((33, 29, 40), (5, 5, 5), 0),
+    ((40, 38, 30), (9, 9, 9), 0),
+    ((36, 30, 28), (11, 11, 11), 0),
+    ((30, 22, 21), (3, 5, 7), 0),        # non-cubic: generic kernel
+])
+def test_emulated_moving_stats(dims, block, generic):
+    """inv_sd[p] = 1/sqrt(SS of the moving block with origin p) against a plain numpy fp64 evaluation."""
+    vol = _smooth(dims, 21)
+    vol[:6, :8, :9] = 321.0                                 # a constant corner: SS = 0 -> inv_sd = 0
+    _emul.set_option("boxstat_generic", generic)
+    got = _emul.moving_stats(vol, block)
+    _emul.set_option("boxstat_generic", 0)
+    nz, ny, nx = vol.shape
+    bx, by, bz = block
+    v = vol.astype(np.float64)
+    win = np.lib.stride_tricks.sliding_window_view(v, (bz, by, bx))
+    ss = ((win - win.mean(axis=(3, 4, 5), keepdims=True)) ** 2).sum(axis=(3, 4, 5))
+    want = np.where(ss > 1e-9, 1.0 / np.sqrt(np.maximum(ss, 1e-300)), 0.0)
+    valid = got[: nz - bz + 1, : ny - by + 1, : nx - bx + 1]
+    assert np.all(valid[ss <= 1e-9] == 0.0)
+    rel = np.abs(valid - want)[ss > 1e-9] * np.sqrt(ss[ss > 1e-9])
+    assert rel.max() < 1e-6, rel.max()
+    untouched = np.ones(vol.shape, bool)
+    untouched[: nz - bz + 1, : ny - by + 1, : nx - bx + 1] = False
+    assert np.all(got[untouched] == -7.0)                   # origins whose block leaves the volume are not written
