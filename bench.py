@@ -2,7 +2,8 @@
 """bench.py -- one JSON line for the block-matching hot path on B200.
 
 A "step" is one pass of the whole hot path over one synthetic volume pair: variance-based block selection
-(S1-S3) followed by exhaustive NCC matching (M1-M5), through the C ABI of libnrr_bm.so.
+(S1-S3) followed by exhaustive NCC matching (M1-M5), through the C ABI of libnrr_bm.so (nrr_bm_register: the
+selection, the moving-volume statistics and the matching kernels enqueued back to back, no host synchronisation).
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload fullres]
 
@@ -194,10 +195,18 @@ def main():
     flush = torch.empty(256 * 1024 * 1024 // 4, dtype=torch.float32, device=dev)   # 256 MB > 126 MB L2
     stream = torch.cuda.current_stream()
 
+    ngrid = 1
+    for a in range(3):
+        ngrid *= (cfg.dims[a] - cfg.block[a]) // cfg.stride[a] + 1
+    cap = max(1, min(ngrid, int(np.floor(0.5 + ngrid * cfg.frac))))      # host-side upper bound on K
+    o_blocks = torch.empty((cap, 3), dtype=torch.int32, device=dev)
+    o_disp = torch.empty((cap, 3), dtype=torch.int32, device=dev)
+    o_ncc = torch.empty((cap,), dtype=torch.float32, device=dev)
+    o_n = torch.zeros((), dtype=torch.int32, device=dev)
+
     def step():
-        blocks, n, ncand = nrr.nrr_bm_select_blocks(fixed, cfg.block, cfg.stride, cfg.frac, mask)
-        disp, ncc = nrr.nrr_bm_match(fixed, moving, blocks, cfg.block, cfg.window)
-        return blocks, n, disp, ncc
+        nrr.nrr_bm_register(fixed, moving, cfg.block, cfg.stride, cfg.window, cfg.frac, mask, capacity=cap,
+                            out_blocks=o_blocks, out_n=o_n, out_disp=o_disp, out_ncc=o_ncc)
 
     def barrier():
         torch.cuda.synchronize()
@@ -207,8 +216,10 @@ def main():
 
     for _ in range(args.warmup):
         flush.zero_()
-        blocks, n, disp, ncc = step()
+        step()
     nrr.nrr_bm_check_async_error()
+    n = int(o_n.item())
+    blocks, disp, ncc = o_blocks[:n], o_disp[:n], o_ncc[:n]
     valid = valid_candidates(blocks.cpu().numpy(), cfg)
     nvox_block = cfg.block[0] * cfg.block[1] * cfg.block[2]
     useful_fma = int(valid.sum()) * nvox_block
@@ -246,7 +257,6 @@ def main():
     fixed_p = torch.from_numpy(fixed_h).pin_memory()
     moving_p = torch.from_numpy(moving_h).pin_memory()
     mask_p = torch.from_numpy(mask_h).pin_memory() if mask_h is not None else None
-    cap = int(n)
     ob = torch.empty((cap, 3), dtype=torch.int32).pin_memory()
     od = torch.empty((cap, 3), dtype=torch.int32).pin_memory()
     on = torch.empty((cap,), dtype=torch.float32).pin_memory()
@@ -282,8 +292,12 @@ def main():
         peak_measured = nrr.nrr_bm_fp32_peak()
     except Exception as e:  # pragma: no cover
         print("fp32 peak microbenchmark failed: %s" % e, file=sys.stderr)
+    info = nrr.nrr_bm_match_info(cfg.dims, cfg.block, cfg.window)
+    kernel_name = {2: "match_pair_kernel", 1: "match_rows_kernel", 0: "match_generic_kernel"}[info["kernel"]]
     roofline = {
-        "bound": "alu", "kernel": "match_rows_kernel", "achieved": achieved_tflops, "peak": FP32_PEAK_TFLOPS,
+        "bound": "alu", "kernel": kernel_name, "launch": {"threads": info["threads"], "smem_bytes": info["smem_bytes"],
+                                                          "blocks_per_cta": info["blocks_per_cta"], "tma": info["tma"]},
+        "achieved": achieved_tflops, "peak": FP32_PEAK_TFLOPS,
         "unit": "TFLOP/s", "frac": achieved_tflops / FP32_PEAK_TFLOPS,
         "peak_source": "derived: 148 SMs x 128 FP32 lanes x 2 x 1.965 GHz (MEASURED_PEAKS.json has no FP32 figure)",
         "peak_measured_ffma": peak_measured,
@@ -320,6 +334,7 @@ def main():
         "ms_per_volume_pair": ms_per_step,
         "phase_ms": {"select": prof["select_ms"] / max(1, prof["select_calls"]),
                      "moving_stats": prof["moving_stats_ms"] / max(1, prof["moving_stats_calls"]),
+                     "fixed_records": prof["prep_ms"] / max(1, prof["prep_calls"]),
                      "match": match_ms},
         "match_only": {"blocks_per_sec": n / (match_ms * 1e-3), "cand_evals_per_sec": float(valid.sum()) / (match_ms * 1e-3)},
         "fp32_peak_frac": achieved_tflops / FP32_PEAK_TFLOPS,

@@ -113,6 +113,21 @@ NRR_BM_API int nrr_bm_match(const float *fixed, const float *moving, const int d
                  const int block[3], const int window[3], int *out_disp, float *out_ncc, void *stream);
 
 /*
+ * Selection + matching of one volume pair in ONE asynchronous call (no host synchronisation at all): the
+ * selection kernels, the moving-volume statistics and the matching kernels are enqueued back to back; the
+ * matching kernels are launched for the host-side upper bound floor(0.5 + grid positions * frac) on K and read
+ * K itself from device memory.  This is the call for pipelines and parameter sweeps that must not stall the
+ * stream (BASELINE.json config 5: 32 settings "in one launch sequence").  Arguments as in nrr_bm_select_blocks
+ * and nrr_bm_match, except
+ *   out_n  [out] DEVICE int (nullable): K.  If K > capacity only the first `capacity` blocks (ascending
+ *                candidate index) are written and matched; the caller sees K > capacity after its own sync.
+ * Rows [K, capacity) of out_blocks / out_disp / out_ncc are left untouched.
+ */
+NRR_BM_API int nrr_bm_register(const float *fixed, const float *moving, const int dims[3], const int block[3],
+                    const int stride[3], const int window[3], double frac, const unsigned char *mask, int *out_blocks,
+                    int capacity, int *out_n, int *out_disp, float *out_ncc, void *stream);
+
+/*
  * Per-candidate normalisers of the moving volume (row M2 of the hot path; nrr_bm_match runs this itself,
  * the entry point exposes it for tests and for callers that match one moving volume against many block lists).
  * For every block ORIGIN p whose block fits in the volume,
@@ -151,25 +166,30 @@ NRR_BM_API int nrr_bm_register_host(const float *fixed, const float *moving, con
  *    events on the caller's stream.  nrr_bm_profile_read synchronises those events and returns the
  *    accumulated milliseconds and call counts since the last read, then resets them:
  *      ms[0] = selection kernels (statistics + radix select + compaction), ms[1] = moving-volume statistics
- *      (per-candidate normalisers), ms[2] = matching kernel;  calls[i] = number of timed launches groups.
+ *      (per-candidate normalisers), ms[2] = matching kernel alone, ms[3] = fixed-block records (the matching
+ *      kernel's prep kernel);  calls[i] = number of timed launch groups.
  *  nrr_bm_launch_count(): kernels launched by this library on this thread since the last reset.
  *  nrr_bm_match_info: which matching kernel a (block, window, dims) triple dispatches to.
- *      info[0] = 1 fast register-tiled kernel / 0 generic kernel, info[1] = threads per CTA,
- *      info[2] = dynamic shared memory bytes, info[3] = 1 if TMA staging is used, info[4] = candidates.
+ *      info[0] = 2 pair kernel (two candidate rows per thread) / 1 one-row-per-thread kernel / 0 generic kernel,
+ *      info[1] = threads per CTA, info[2] = dynamic shared memory bytes, info[3] = 1 if TMA staging is used,
+ *      info[4] = candidates per block, info[5] = blocks per CTA.
  *  nrr_bm_fp32_peak: runs an FFMA-only microbenchmark on `stream`'s device and returns the measured
  *      dense FP32 rate in TFLOP/s (the denominator context for the matching kernel's roofline).
  */
 NRR_BM_API int nrr_bm_profile_enable(int on);
-NRR_BM_API int nrr_bm_profile_read(double ms[3], int calls[3]);
+NRR_BM_API int nrr_bm_profile_read(double ms[4], int calls[4]);
 NRR_BM_API long long nrr_bm_launch_count(int reset);
-NRR_BM_API int nrr_bm_match_info(const int dims[3], const int block[3], const int window[3], int info[5]);
+NRR_BM_API int nrr_bm_match_info(const int dims[3], const int block[3], const int window[3], int info[6]);
 NRR_BM_API int nrr_bm_fp32_peak(double *out_tflops, void *stream);
 
 /* Tuning / experiment knobs (process-wide; results stay within the documented tolerances):
  *   "tie_band"      FP32 candidates within this NCC distance of the FP32 maximum are re-scored in FP64
  *                   (default 1e-4; 0 disables the re-score except for exact FP32 ties)
  *   "force_generic" != 0: always use the generic matching kernel
- *   "disable_tma"   != 0: stage shared memory with plain loads instead of TMA */
+ *   "force_rows"    != 0: skip the pair kernel (one candidate row per thread instead)
+ *   "disable_tma"   != 0: stage shared memory with plain loads instead of TMA (implies no pair kernel)
+ *   "pair_blocks_per_cta"  > 0: blocks per CTA of the pair kernel (0 = the planner's choice)
+ *   "boxstat_generic" / "select_generic" != 0: the runtime-shaped moving-statistics / selection kernels */
 NRR_BM_API int nrr_bm_set_option(const char *name, double value);
 
 NRR_BM_API const char *nrr_bm_last_error(void);

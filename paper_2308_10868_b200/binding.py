@@ -20,7 +20,7 @@ NRR_E_NULL, NRR_E_DIMS, NRR_E_BLOCK, NRR_E_STRIDE, NRR_E_WINDOW, NRR_E_FRAC = -1
 NRR_E_CAPACITY, NRR_E_BOUNDS, NRR_E_SMEM, NRR_E_CUDA, NRR_E_ARG = -7, -8, -9, -10, -11
 
 EXPORTS = [
-    "nrr_bm_select_blocks", "nrr_bm_match", "nrr_bm_check_async_error", "nrr_bm_moving_stats", "nrr_bm_moving_stats_host",
+    "nrr_bm_select_blocks", "nrr_bm_match", "nrr_bm_register", "nrr_bm_check_async_error", "nrr_bm_moving_stats", "nrr_bm_moving_stats_host",
     "nrr_bm_select_blocks_host", "nrr_bm_match_host", "nrr_bm_register_host",
     "nrr_bm_profile_enable", "nrr_bm_profile_read", "nrr_bm_launch_count", "nrr_bm_match_info",
     "nrr_bm_fp32_peak", "nrr_bm_set_option", "nrr_bm_last_error", "nrr_bm_status_string", "nrr_bm_version",
@@ -51,6 +51,8 @@ def lib() -> ctypes.CDLL:
     L.nrr_bm_select_blocks.argtypes = [vp, i3, i3, i3, cd, vp, vp, ci, i3, vp, i3, vp]
     L.nrr_bm_match.restype = ci
     L.nrr_bm_match.argtypes = [vp, vp, i3, vp, ci, i3, i3, vp, vp, vp]
+    L.nrr_bm_register.restype = ci
+    L.nrr_bm_register.argtypes = [vp, vp, i3, i3, i3, i3, cd, vp, vp, ci, vp, vp, vp, vp]
     L.nrr_bm_moving_stats.restype = ci
     L.nrr_bm_moving_stats.argtypes = [vp, i3, i3, vp, vp]
     L.nrr_bm_moving_stats_host.restype = ci
@@ -173,6 +175,41 @@ def nrr_bm_match(fixed, moving, blocks, block, window, out_disp=None, out_ncc=No
     return out_disp, out_ncc
 
 
+def nrr_bm_register(fixed, moving, block, stride, window, frac: float, mask=None, capacity: Optional[int] = None,
+                    out_blocks=None, out_n=None, out_disp=None, out_ncc=None, stream=None):
+    """Device form, fully asynchronous: select + match of one pair with no host synchronisation.
+    Returns (blocks [capacity][3], n (CUDA int32 scalar tensor: K), disp [capacity][3], ncc [capacity]); rows
+    beyond K are untouched.  Read n (e.g. int(n)) only after the work on `stream` may be waited for."""
+    import torch
+    fixed = _dev(fixed, torch.float32, "fixed")
+    moving = _dev(moving, torch.float32, "moving")
+    if tuple(fixed.shape) != tuple(moving.shape):
+        raise ValueError("volume shape mismatch")
+    dims = _dims_of(fixed)
+    if mask is not None:
+        mask = _dev(mask, torch.uint8, "mask")
+    if capacity is None:
+        ngrid = 1
+        for a in range(3):
+            ngrid *= max(0, (dims[a] - int(block[a])) // max(1, int(stride[a])) + 1)
+        capacity = max(1, min(ngrid, int(np.floor(0.5 + ngrid * float(frac)))))
+    dev = fixed.device
+    if out_blocks is None:
+        out_blocks = torch.empty((capacity, 3), dtype=torch.int32, device=dev)
+    if out_disp is None:
+        out_disp = torch.empty((capacity, 3), dtype=torch.int32, device=dev)
+    if out_ncc is None:
+        out_ncc = torch.empty((capacity,), dtype=torch.float32, device=dev)
+    if out_n is None:
+        out_n = torch.empty((), dtype=torch.int32, device=dev)
+    with torch.cuda.device(dev):
+        _check(lib().nrr_bm_register(fixed.data_ptr(), moving.data_ptr(), _i3(dims), _i3(block), _i3(stride), _i3(window),
+                                     float(frac), mask.data_ptr() if mask is not None else None, out_blocks.data_ptr(),
+                                     int(capacity), out_n.data_ptr(), out_disp.data_ptr(), out_ncc.data_ptr(),
+                                     _stream_ptr(stream)))
+    return out_blocks, out_n, out_disp, out_ncc
+
+
 def nrr_bm_moving_stats(moving, block, out_inv_sd=None, stream=None):
     """Device form, asynchronous. Returns inv_sd fp32 CUDA [nz][ny][nx] (entries whose block leaves the volume untouched)."""
     import torch
@@ -253,11 +290,11 @@ def nrr_bm_profile_enable(on: bool) -> None:
 
 
 def nrr_bm_profile_read():
-    ms = (ctypes.c_double * 3)()
-    calls = (ctypes.c_int * 3)()
+    ms = (ctypes.c_double * 4)()
+    calls = (ctypes.c_int * 4)()
     _check(lib().nrr_bm_profile_read(ms, calls))
-    return {"select_ms": ms[0], "moving_stats_ms": ms[1], "match_ms": ms[2],
-            "select_calls": calls[0], "moving_stats_calls": calls[1], "match_calls": calls[2]}
+    return {"select_ms": ms[0], "moving_stats_ms": ms[1], "match_ms": ms[2], "prep_ms": ms[3],
+            "select_calls": calls[0], "moving_stats_calls": calls[1], "match_calls": calls[2], "prep_calls": calls[3]}
 
 
 def nrr_bm_launch_count(reset: bool = False) -> int:
@@ -265,9 +302,10 @@ def nrr_bm_launch_count(reset: bool = False) -> int:
 
 
 def nrr_bm_match_info(dims, block, window):
-    info = (ctypes.c_int * 5)()
+    info = (ctypes.c_int * 6)()
     _check(lib().nrr_bm_match_info(_i3(dims), _i3(block), _i3(window), info))
-    return {"fast": bool(info[0]), "threads": info[1], "smem_bytes": info[2], "tma": bool(info[3]), "candidates": info[4]}
+    return {"fast": bool(info[0]), "kernel": info[0], "threads": info[1], "smem_bytes": info[2], "tma": bool(info[3]),
+            "candidates": info[4], "blocks_per_cta": info[5]}
 
 
 def nrr_bm_fp32_peak(stream=None) -> float:

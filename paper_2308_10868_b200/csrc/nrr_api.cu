@@ -1,6 +1,7 @@
 // nrr_api.cu -- the extern "C" boundary of libnrr_bm.so (include/nrr_bm.h): argument validation, scratch
 // management, the host-buffer forms, instrumentation.  Every step of the path itself runs in the kernels of
 // nrr_select.cu / nrr_boxstat.cu / nrr_match.cu; nothing here computes on the CPU.
+#include <math.h>
 #include <stdarg.h>
 #include <stdio.h>
 #include <string.h>
@@ -54,24 +55,14 @@ int ensure_thread_state()
     return NRR_OK;
 }
 
+constexpr int kPhases = 4;
+thread_local cudaEvent_t t_open[kPhases] = {nullptr, nullptr, nullptr, nullptr};
+
 struct Span {      // brackets a phase with events when profiling is on
     int phase;
     cudaStream_t stream;
-    cudaEvent_t e0 = nullptr, e1 = nullptr;
-    Span(int p, cudaStream_t s) : phase(p), stream(s)
-    {
-        if (!t_profile) return;
-        if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) { e0 = e1 = nullptr; return; }
-        cudaEventRecord(e0, stream);
-    }
-    void stop()
-    {
-        if (!e0) return;
-        cudaEventRecord(e1, stream);
-        if (!t_spans) t_spans = new std::vector<TimedSpan>();
-        t_spans->push_back({phase, e0, e1});
-        e0 = e1 = nullptr;
-    }
+    Span(int p, cudaStream_t s) : phase(p), stream(s) { profile_begin(phase, stream); }
+    void stop() { profile_end(phase, stream); }
 };
 
 int fail(int code, const char *fmt, ...)
@@ -177,13 +168,57 @@ int match_device(const float *fixed, const float *moving, const int dims[3], con
     Span s1(1, stream);
     rc = boxstat_enqueue(moving, i3(dims), i3(block), inv_sd, stream);
     s1.stop();
-    if (rc == NRR_OK) {
-        Span s2(2, stream);
-        rc = match_enqueue(fixed, moving, inv_sd, i3(dims), blocks, n, i3(block), i3(window), out_disp, out_ncc,
+    if (rc == NRR_OK)
+        rc = match_enqueue(fixed, moving, inv_sd, i3(dims), blocks, n, nullptr, i3(block), i3(window), out_disp, out_ncc,
                            t_err_flag, stream);
-        s2.stop();
-    }
     cudaError_t e = cudaFreeAsync(inv_sd, stream);
+    if (rc == NRR_OK && e != cudaSuccess) return cuda_fail(e, "cudaFreeAsync");
+    return rc;
+}
+
+// select + match of one pair with no host synchronisation: the matching kernels are launched for an upper bound
+// on K known on the host and read K itself from the selection state on the device.
+int register_device(const float *fixed, const float *moving, const int dims[3], const int block[3],
+                    const int stride[3], const int window[3], double frac, const unsigned char *mask, int *out_blocks,
+                    int capacity, int *out_n_dev, int *out_disp, float *out_ncc, cudaStream_t stream)
+{
+    int rc = ensure_thread_state();
+    if (rc) return rc;
+    MatchPlan plan;
+    if ((rc = match_plan(i3(dims), i3(block), i3(window), moving, fixed, &plan))) return rc;
+    const Int3 g = grid_of(dims, block, stride);
+    const long long ngrid = (long long)g.x * g.y * g.z;
+    if (ngrid > 0x7fffffffll) return fail(NRR_E_DIMS, "stride grid has %lld positions (limit 2^31-1)", ngrid);
+    void *scratch = nullptr;
+    NRR_CUDA(cudaMallocAsync(&scratch, select_scratch_bytes(ngrid), stream));
+    SelectState *st = nullptr;
+    Span span(0, stream);
+    rc = select_enqueue(fixed, i3(dims), i3(block), i3(stride), g, frac, mask, out_blocks, capacity, nullptr, scratch,
+                        &st, stream);
+    span.stop();
+    if (rc == NRR_OK && out_n_dev)
+        rc = cudaMemcpyAsync(out_n_dev, &st->k, sizeof(int), cudaMemcpyDeviceToDevice, stream) == cudaSuccess
+                 ? NRR_OK : fail(NRR_E_CUDA, "copy of K failed");
+    // K = floor(0.5 + N*frac) with N <= ngrid candidates, so K <= floor(0.5 + ngrid*frac)
+    double kmax = floor(0.5 + (double)ngrid * frac);
+    if (kmax > (double)ngrid) kmax = (double)ngrid;
+    const int n_cap = (int)(kmax < (double)capacity ? kmax : (double)capacity);
+    if (rc == NRR_OK && n_cap > 0) {
+        const size_t nvox = (size_t)dims[0] * dims[1] * dims[2];
+        float *inv_sd = nullptr;
+        cudaError_t e = cudaMallocAsync((void **)&inv_sd, nvox * sizeof(float), stream);
+        if (e != cudaSuccess) rc = cuda_fail(e, "cudaMallocAsync");
+        if (rc == NRR_OK) {
+            Span s1(1, stream);
+            rc = boxstat_enqueue(moving, i3(dims), i3(block), inv_sd, stream);
+            s1.stop();
+        }
+        if (rc == NRR_OK)
+            rc = match_enqueue(fixed, moving, inv_sd, i3(dims), out_blocks, n_cap, &st->k, i3(block), i3(window),
+                               out_disp, out_ncc, t_err_flag, stream);
+        if (inv_sd) cudaFreeAsync(inv_sd, stream);
+    }
+    cudaError_t e = cudaFreeAsync(scratch, stream);
     if (rc == NRR_OK && e != cudaSuccess) return cuda_fail(e, "cudaFreeAsync");
     return rc;
 }
@@ -239,6 +274,26 @@ int cuda_fail(cudaError_t e, const char *what)
 
 void count_launch(int n) { t_launches += n; }
 
+void profile_begin(int phase, cudaStream_t stream)
+{
+    if (!t_profile || phase < 0 || phase >= kPhases || t_open[phase]) return;
+    cudaEvent_t e = nullptr;
+    if (cudaEventCreate(&e) != cudaSuccess) return;
+    cudaEventRecord(e, stream);
+    t_open[phase] = e;
+}
+
+void profile_end(int phase, cudaStream_t stream)
+{
+    if (phase < 0 || phase >= kPhases || !t_open[phase]) return;
+    cudaEvent_t e1 = nullptr;
+    if (cudaEventCreate(&e1) != cudaSuccess) { cudaEventDestroy(t_open[phase]); t_open[phase] = nullptr; return; }
+    cudaEventRecord(e1, stream);
+    if (!t_spans) t_spans = new std::vector<TimedSpan>();
+    t_spans->push_back({phase, t_open[phase], e1});
+    t_open[phase] = nullptr;
+}
+
 }  // namespace nrr
 
 using namespace nrr;
@@ -289,6 +344,21 @@ int nrr_bm_moving_stats_host(const float *moving, const int dims[3], const int b
     NRR_CUDA(cudaMemcpyAsync(out_inv_sd, d_out.p, nvox * sizeof(float), cudaMemcpyDeviceToHost, s));
     NRR_CUDA(cudaStreamSynchronize(s));
     return NRR_OK;
+}
+
+int nrr_bm_register(const float *fixed, const float *moving, const int dims[3], const int block[3], const int stride[3],
+                    const int window[3], double frac, const unsigned char *mask, int *out_blocks, int capacity,
+                    int *out_n, int *out_disp, float *out_ncc, void *stream)
+{
+    int dummy = 0;
+    int rc = check_select_args(fixed, dims, block, stride, frac, out_blocks, capacity, &dummy);
+    if (rc) return rc;
+    if (!moving || !window) return fail(NRR_E_NULL, "moving/window is NULL");
+    for (int a = 0; a < 3; ++a)
+        if (window[a] < 0) return fail(NRR_E_WINDOW, "window[%d] = %d < 0", a, window[a]);
+    if (capacity > 0 && (!out_disp || !out_ncc)) return fail(NRR_E_NULL, "out_disp/out_ncc is NULL with capacity > 0");
+    return register_device(fixed, moving, dims, block, stride, window, frac, mask, out_blocks, capacity, out_n, out_disp,
+                           out_ncc, (cudaStream_t)stream);
 }
 
 int nrr_bm_check_async_error(void *stream) { return check_async((cudaStream_t)stream); }
@@ -358,16 +428,21 @@ int nrr_bm_register_host(const float *fixed, const float *moving, const int dims
     if (mask) NRR_CUDA(d_mask.upload(mask, nvox));
     NRR_CUDA(d_moving.upload(moving, nvox * sizeof(float)));      // overlaps the selection kernels' queueing
     NRR_CUDA(d_blocks.alloc((size_t)capacity * 3 * sizeof(int)));
-    rc = select_device((const float *)d_fixed.p, dims, block, stride, frac, (const unsigned char *)d_mask.p,
-                       (int *)d_blocks.p, capacity, out_n, nullptr, nullptr, s);
+    DevBuf d_n(s);
+    NRR_CUDA(d_n.alloc(sizeof(int)));
+    NRR_CUDA(d_disp.alloc((size_t)capacity * 3 * sizeof(int)));
+    NRR_CUDA(d_ncc.alloc((size_t)capacity * sizeof(float)));
+    rc = register_device((const float *)d_fixed.p, (const float *)d_moving.p, dims, block, stride, window, frac,
+                         (const unsigned char *)d_mask.p, (int *)d_blocks.p, capacity, (int *)d_n.p, (int *)d_disp.p,
+                         (float *)d_ncc.p, s);
     if (rc) return rc;
+    int *h_n = (int *)((char *)t_pinned + 2048);
+    NRR_CUDA(cudaMemcpyAsync(h_n, d_n.p, sizeof(int), cudaMemcpyDeviceToHost, s));
+    NRR_CUDA(cudaStreamSynchronize(s));
+    *out_n = *h_n;
+    if (*out_n > capacity) return fail(NRR_E_CAPACITY, "K = %d selected blocks exceed capacity = %d", *out_n, capacity);
     const int n = *out_n;
     if (n == 0) return NRR_OK;
-    NRR_CUDA(d_disp.alloc((size_t)n * 3 * sizeof(int)));
-    NRR_CUDA(d_ncc.alloc((size_t)n * sizeof(float)));
-    rc = match_device((const float *)d_fixed.p, (const float *)d_moving.p, dims, (const int *)d_blocks.p, n, block,
-                      window, (int *)d_disp.p, (float *)d_ncc.p, s);
-    if (rc) return rc;
     NRR_CUDA(cudaMemcpyAsync(out_blocks, d_blocks.p, (size_t)n * 3 * sizeof(int), cudaMemcpyDeviceToHost, s));
     NRR_CUDA(cudaMemcpyAsync(out_disp, d_disp.p, (size_t)n * 3 * sizeof(int), cudaMemcpyDeviceToHost, s));
     NRR_CUDA(cudaMemcpyAsync(out_ncc, d_ncc.p, (size_t)n * sizeof(float), cudaMemcpyDeviceToHost, s));
@@ -380,10 +455,10 @@ int nrr_bm_profile_enable(int on)
     return NRR_OK;
 }
 
-int nrr_bm_profile_read(double ms[3], int calls[3])
+int nrr_bm_profile_read(double ms[4], int calls[4])
 {
     if (!ms || !calls) return fail(NRR_E_NULL, "ms/calls is NULL");
-    for (int i = 0; i < 3; ++i) { ms[i] = 0.0; calls[i] = 0; }
+    for (int i = 0; i < kPhases; ++i) { ms[i] = 0.0; calls[i] = 0; }
     if (!t_spans) return NRR_OK;
     int rc = NRR_OK;
     for (TimedSpan &sp : *t_spans) {
@@ -391,7 +466,7 @@ int nrr_bm_profile_read(double ms[3], int calls[3])
         cudaError_t e = cudaEventSynchronize(sp.e1);
         if (e == cudaSuccess) e = cudaEventElapsedTime(&t, sp.e0, sp.e1);
         if (e != cudaSuccess) rc = cuda_fail(e, "profile events");
-        else if (sp.phase >= 0 && sp.phase < 3) { ms[sp.phase] += (double)t; calls[sp.phase] += 1; }
+        else if (sp.phase >= 0 && sp.phase < kPhases) { ms[sp.phase] += (double)t; calls[sp.phase] += 1; }
         cudaEventDestroy(sp.e0);
         cudaEventDestroy(sp.e1);
     }
@@ -406,7 +481,7 @@ long long nrr_bm_launch_count(int reset)
     return v;
 }
 
-int nrr_bm_match_info(const int dims[3], const int block[3], const int window[3], int info[5])
+int nrr_bm_match_info(const int dims[3], const int block[3], const int window[3], int info[6])
 {
     if (!info || !window) return fail(NRR_E_NULL, "info/window is NULL");
     int rc = check_dims_block(dims, block);
@@ -417,7 +492,7 @@ int nrr_bm_match_info(const int dims[3], const int block[3], const int window[3]
     memset(&plan, 0, sizeof(plan));
     rc = match_plan(i3(dims), i3(block), i3(window), nullptr, nullptr, &plan);
     if (rc) return rc;
-    info[0] = plan.fast; info[1] = plan.threads; info[2] = plan.smem_bytes; info[3] = plan.tma; info[4] = plan.candidates;
+    info[0] = plan.fast; info[1] = plan.threads; info[2] = plan.smem_bytes; info[3] = plan.tma; info[4] = plan.candidates; info[5] = plan.blocks_per_cta;
     return NRR_OK;
 }
 

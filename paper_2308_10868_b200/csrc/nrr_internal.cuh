@@ -23,6 +23,10 @@ struct Int3 { int x, y, z; };
 void set_error(const char *fmt, ...);
 int cuda_fail(cudaError_t e, const char *what);   // records the message, returns NRR_E_CUDA
 void count_launch(int n = 1);
+// CUDA-event brackets around a phase on the caller's stream (no-ops unless nrr_bm_profile_enable(1)):
+// 0 selection, 1 moving-volume statistics, 2 matching kernel, 3 fixed-block records (prep kernel)
+void profile_begin(int phase, cudaStream_t stream);
+void profile_end(int phase, cudaStream_t stream);
 
 #define NRR_CUDA(call)                                              \
     do {                                                            \
@@ -71,9 +75,12 @@ struct MatchPlan {
 };
 int match_plan(Int3 dims, Int3 block, Int3 window, const void *moving_ptr, const void *fixed_ptr,
                MatchPlan *plan);
+// n_dev (nullable, DEVICE): the number of blocks is min(n, *n_dev), read by the kernels themselves, so a caller
+// that only knows an upper bound n on the host (selection still in flight) needs no synchronisation.
 int match_enqueue(const float *fixed, const float *moving, const float *inv_sd, Int3 dims, const int *blocks,
-                  int n, Int3 block, Int3 window, int *out_disp, float *out_ncc, unsigned int *err_flag,
-                  cudaStream_t stream);
+                  int n, const unsigned int *n_dev, Int3 block, Int3 window, int *out_disp, float *out_ncc,
+                  unsigned int *err_flag, cudaStream_t stream);
+extern thread_local const unsigned int *t_match_n_dev;      // set by match_enqueue for the launchers
 
 // nrr_match_pair.cu: tries the pair kernel; *handled tells whether it took the call.
 int match_pair_dispatch(const float *fixed, const float *moving, const float *inv_sd, Int3 dims, const int *blocks,

@@ -32,6 +32,7 @@ namespace nrr {
 float g_tie_band = 1e-4f;     // FP32 candidates this close to the FP32 maximum are re-scored in FP64
 int g_force_generic = 0;
 int g_disable_tma = 0;
+thread_local const unsigned int *t_match_n_dev = nullptr;
 int g_force_rows = 0;          // != 0: skip the pair kernel (one candidate row per thread instead)
 
 namespace {
@@ -88,9 +89,10 @@ __global__ void __launch_bounds__(kFastMaxThreads) match_rows_kernel(const __gri
                                   const float *__restrict__ fixed, const float *__restrict__ moving,
                                   const float *__restrict__ inv_sd, Int3 dims, const int *__restrict__ blocks,
                                   int rz, float tie_band, int *__restrict__ out_disp, float *__restrict__ out_ncc,
-                                  unsigned int *err_flag)
+                                  unsigned int *err_flag, const unsigned int *__restrict__ n_dev)
 {
     using C = FastCfg<B, R>;
+    if (n_dev && blockIdx.x >= *n_dev) return;      // uniform: the launch was sized for an upper bound
     constexpr int W = C::W, PITCH = C::PITCH, PROWS = C::PROWS, FP = C::FP;
     NRR_DYN_SMEM(s_raw);
     unsigned char *s_base = s_raw + ((128u - (smem_u32(s_raw) & 127u)) & 127u);   // keeps the shared address space
@@ -260,8 +262,9 @@ __global__ void __launch_bounds__(128)
 match_generic_kernel(const float *__restrict__ fixed, const float *__restrict__ moving,
                      const float *__restrict__ inv_sd, Int3 dims, const int *__restrict__ blocks, Int3 block,
                      Int3 window, float tie_band, int *__restrict__ out_disp, float *__restrict__ out_ncc,
-                     unsigned int *err_flag)
+                     unsigned int *err_flag, const unsigned int *__restrict__ n_dev)
 {
+    if (n_dev && blockIdx.x >= *n_dev) return;      // uniform: the launch was sized for an upper bound
     NRR_DYN_SMEM(s_raw);
     const int nvox = block.x * block.y * block.z;
     const int wx = 2 * window.x + 1, wy = 2 * window.y + 1, wz = 2 * window.z + 1;
@@ -405,8 +408,10 @@ int launch_fast(const float *fixed, const float *moving, const float *inv_sd, In
         NRR_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         configured_smem = (int)smem;
     }
+    profile_begin(2, stream);
     NRR_LAUNCH(kern, n, threads, smem, stream, tm_m, use_tma, fixed, moving, inv_sd, dims, blocks, rz, g_tie_band,
-               out_disp, out_ncc, err_flag);
+               out_disp, out_ncc, err_flag, t_match_n_dev);
+    profile_end(2, stream);
     NRR_LAUNCH_CHECK("match_rows_kernel");
     return NRR_OK;
 }
@@ -482,8 +487,10 @@ int dispatch(const float *fixed, const float *moving, const float *inv_sd, Int3 
         NRR_CUDA(cudaFuncSetAttribute(match_generic_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         configured_smem = (int)smem;
     }
+    profile_begin(2, stream);
     NRR_LAUNCH(match_generic_kernel, n, 128, smem, stream, fixed, moving, inv_sd, dims, blocks, block, window,
-               g_tie_band, out_disp, out_ncc, err_flag);
+               g_tie_band, out_disp, out_ncc, err_flag, t_match_n_dev);
+    profile_end(2, stream);
     NRR_LAUNCH_CHECK("match_generic_kernel");
     return NRR_OK;
 }
@@ -497,10 +504,14 @@ int match_plan(Int3 dims, Int3 block, Int3 window, const void *moving_ptr, const
 }
 
 int match_enqueue(const float *fixed, const float *moving, const float *inv_sd, Int3 dims, const int *blocks, int n,
-                  Int3 block, Int3 window, int *out_disp, float *out_ncc, unsigned int *err_flag, cudaStream_t stream)
+                  const unsigned int *n_dev, Int3 block, Int3 window, int *out_disp, float *out_ncc,
+                  unsigned int *err_flag, cudaStream_t stream)
 {
     if (n == 0) return NRR_OK;
-    return dispatch(fixed, moving, inv_sd, dims, blocks, n, block, window, out_disp, out_ncc, err_flag, stream, nullptr);
+    t_match_n_dev = n_dev;
+    const int rc = dispatch(fixed, moving, inv_sd, dims, blocks, n, block, window, out_disp, out_ncc, err_flag, stream, nullptr);
+    t_match_n_dev = nullptr;
+    return rc;
 }
 
 }  // namespace nrr

@@ -150,9 +150,10 @@ constexpr int kPrepWarps = 4;
 template <int B, int R>
 __global__ void __launch_bounds__(kPrepWarps * 32)
 prep_kernel(const float *__restrict__ fixed, Int3 dims, const int *__restrict__ blocks, int n,
-            float *__restrict__ records, int *__restrict__ out_disp, float *__restrict__ out_ncc,
-            unsigned int *err_flag)
+            const unsigned int *__restrict__ n_dev, float *__restrict__ records, int *__restrict__ out_disp,
+            float *__restrict__ out_ncc, unsigned int *err_flag)
 {
+    if (n_dev) n = min(n, (int)*n_dev);               // the launch was sized for an upper bound
     using C = PairCfg<B, R>;
     constexpr int NVOX = B * B * B;
     __shared__ float s_f[kPrepWarps][NVOX];
@@ -318,6 +319,7 @@ struct PairArgs {
     const float *fixed, *moving, *inv_sd, *records;
     const int *blocks;
     const uint32_t *task_tab;      // [threads]: valid << 31 | g << 16 | dy << 8 | p
+    const unsigned int *n_dev;     // nullable: the number of blocks is min(n, *n_dev)
     int *out_disp;
     float *out_ncc;
     Int3 dims;
@@ -339,8 +341,10 @@ match_pair_kernel(const __grid_constant__ CUtensorMap tm_moving, const PairArgs 
     PairCtrl *ctrl = (PairCtrl *)((unsigned char *)s_recs + (size_t)a.G * C::REC_BYTES);
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int n = a.n_dev ? min(a.n, (int)*a.n_dev) : a.n;
     const int b0 = blockIdx.x * a.G;
-    const int gact = min(a.G, a.n - b0);
+    if (b0 >= n) return;                               // uniform: the launch was sized for an upper bound
+    const int gact = min(a.G, n - b0);
     const int rz = a.rz, WZ = 2 * rz + 1, UZ = B + 2 * rz;
     const Int3 dims = a.dims;
     const uint32_t union_bytes = (uint32_t)(sizeof(float) * UZ * UX * PITCH);
@@ -655,8 +659,10 @@ int launch_pair(const float *fixed, const float *moving, const float *inv_sd, In
     float *records = nullptr;
     NRR_CUDA(cudaMallocAsync((void **)&records, (size_t)n * C::REC_BYTES, stream));
     auto prep = prep_kernel<B, R>;
-    NRR_LAUNCH(prep, (n + kPrepWarps - 1) / kPrepWarps, kPrepWarps * 32, 0, stream, fixed, dims, blocks, n, records,
-               out_disp, out_ncc, err_flag);
+    profile_begin(3, stream);
+    NRR_LAUNCH(prep, (n + kPrepWarps - 1) / kPrepWarps, kPrepWarps * 32, 0, stream, fixed, dims, blocks, n,
+               t_match_n_dev, records, out_disp, out_ncc, err_flag);
+    profile_end(3, stream);
     NRR_LAUNCH_CHECK("prep_kernel");
     auto kern = match_pair_kernel<B, R>;
     static size_t configured_smem = 0;     // per instantiation
@@ -666,9 +672,11 @@ int launch_pair(const float *fixed, const float *moving, const float *inv_sd, In
     }
     PairArgs a;
     a.fixed = fixed; a.moving = moving; a.inv_sd = inv_sd; a.records = records; a.blocks = blocks; a.task_tab = tab;
-    a.out_disp = out_disp; a.out_ncc = out_ncc; a.dims = dims; a.n = n; a.rz = rz; a.G = g.G;
+    a.out_disp = out_disp; a.out_ncc = out_ncc; a.dims = dims; a.n = n; a.rz = rz; a.G = g.G; a.n_dev = t_match_n_dev;
     a.n_pair_warps = g.n_pair_warps; a.union_stride = g.union_stride; a.tie_band = g_tie_band;
+    profile_begin(2, stream);
     NRR_LAUNCH(kern, (n + g.G - 1) / g.G, g.threads, g.smem, stream, tm_m, a);
+    profile_end(2, stream);
     NRR_LAUNCH_CHECK("match_pair_kernel");
     NRR_CUDA(cudaFreeAsync(records, stream));
     return NRR_OK;

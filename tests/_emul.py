@@ -27,6 +27,7 @@ def lib():
         L.nrr_bm_match_host.argtypes = [vp, vp, i3, vp, ci, i3, i3, vp, vp]
         L.nrr_bm_match_info.argtypes = [i3, i3, i3, i3]
         L.nrr_bm_moving_stats_host.argtypes = [vp, i3, i3, vp]
+        L.nrr_bm_register_host.argtypes = [vp, vp, i3, i3, i3, i3, cd, vp, vp, ci, ctypes.POINTER(ci), vp, vp]
         _lib = L
     return _lib
 
@@ -78,3 +79,16 @@ def moving_stats(moving, block, fill=-7.0):
     out = np.full(moving.shape, fill, np.float32)
     _check(lib().nrr_bm_moving_stats_host(moving.ctypes.data, _i3((nx, ny, nz)), _i3(block), out.ctypes.data))
     return out
+
+
+def register(fixed, moving, block, stride, window, frac, mask=None):
+    nz, ny, nx = fixed.shape
+    cap = max(1, int(np.prod([max(0, ((nx, ny, nz)[a] - block[a]) // stride[a] + 1) for a in range(3)])))
+    blocks = np.full((cap, 3), -99, np.int32)
+    disp = np.full((cap, 3), -99, np.int32)
+    ncc = np.full((cap,), -99.0, np.float32)
+    n = ctypes.c_int(0)
+    _check(lib().nrr_bm_register_host(fixed.ctypes.data, moving.ctypes.data, _i3((nx, ny, nz)), _i3(block), _i3(stride),
+                                      _i3(window), float(frac), None if mask is None else mask.ctypes.data,
+                                      blocks.ctypes.data, cap, ctypes.byref(n), disp.ctypes.data, ncc.ctypes.data))
+    return blocks[:n.value], disp[:n.value], ncc[:n.value]

@@ -172,3 +172,23 @@ def test_emulated_moving_stats(dims, block, generic):
     untouched = np.ones(vol.shape, bool)
     untouched[: nz - bz + 1, : ny - by + 1, : nx - bx + 1] = False
     assert np.all(got[untouched] == -7.0)                   # origins whose block leaves the volume are not written
+
+
+def test_emulated_register_needs_no_host_side_count():
+    """nrr_bm_register: the matching kernels are launched for an upper bound on K and read K on the device
+    (masked case: N < grid positions, so whole CTAs find nothing to do)."""
+    dims, block, stride, window = (36, 32, 28), (5, 5, 5), (4, 4, 4), (3, 3, 3)
+    fixed = _smooth(dims, 77)
+    moving = _shift_noise(fixed, (-1, 2, 1), 6.0, 78)
+    mask = spherical_mask(dims, 11.0)
+    ora_sel = oracle.select(fixed, block, stride, 0.5, mask)
+    ora = oracle.match(fixed, moving, ora_sel["centres"], block, window)
+    assert 0 < len(ora_sel["centres"]) < 0.2 * 8 * 7 * 6             # far fewer than the host-side bound
+    for opts in (dict(), dict(force_rows=1), dict(force_generic=1)):
+        for k, v in opts.items():
+            _emul.set_option(k, v)
+        blocks, disp, ncc = _emul.register(fixed, moving, block, stride, window, 0.5, mask)
+        assert np.array_equal(blocks, ora_sel["centres"])
+        assert_match_parity(disp, ncc, ora, "register %s" % (opts,))
+        for k in opts:
+            _emul.set_option(k, 0)

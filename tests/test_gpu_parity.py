@@ -135,27 +135,66 @@ def test_match_parity_small(dims, block, window, fast):
     print("%s %s %s: %d blocks, %d exempt" % (dims, block, window, n, exempt))
 
 
-def test_match_generic_equals_fast_kernel():
+def _with_options(opts, fn):
+    for k, v in opts.items():
+        nrr.nrr_bm_set_option(k, v)
+    try:
+        return fn()
+    finally:
+        for k in opts:
+            nrr.nrr_bm_set_option(k, 0)
+
+
+def test_match_every_kernel_on_the_same_input():
+    """Pair kernel (default), one-row-per-thread kernel with TMA and with plain staging, generic kernel."""
     dims, block, window = (48, 44, 40), (7, 7, 7), (5, 5, 5)
     vol = _smooth(dims, 31)
     mov = _shift_noise(vol, (2, 1, -2), 25.0, 32)
     sel = oracle.select(vol, block, (5, 5, 5), 0.5)
     c = _cuda(sel["centres"])
-    d1, n1 = nrr.nrr_bm_match(_cuda(vol), _cuda(mov), c, block, window)
-    nrr.nrr_bm_set_option("force_generic", 1)
-    try:
-        d2, n2 = nrr.nrr_bm_match(_cuda(vol), _cuda(mov), c, block, window)
-    finally:
-        nrr.nrr_bm_set_option("force_generic", 0)
-    nrr.nrr_bm_set_option("disable_tma", 1)
-    try:
-        d3, n3 = nrr.nrr_bm_match(_cuda(vol), _cuda(mov), c, block, window)
-    finally:
-        nrr.nrr_bm_set_option("disable_tma", 0)
+    run = lambda: nrr.nrr_bm_match(_cuda(vol), _cuda(mov), c, block, window)
+    assert nrr.nrr_bm_match_info(dims, block, window)["kernel"] == 2
+    d0, n0 = run()
+    d1, n1 = _with_options({"force_rows": 1}, run)
+    d2, n2 = _with_options({"force_generic": 1}, run)
+    d3, n3 = _with_options({"force_rows": 1, "disable_tma": 1}, run)
+    d4, n4 = _with_options({"pair_blocks_per_cta": 3}, run)           # another grouping, partial last CTA
     ora = oracle.match(vol, mov, sel["centres"], block, window)
-    for d, n_, lab in ((d1, n1, "fast+tma"), (d2, n2, "generic"), (d3, n3, "fast, plain staging")):
+    for d, n_, lab in ((d0, n0, "pair"), (d1, n1, "rows+tma"), (d2, n2, "generic"), (d3, n3, "rows, plain staging"),
+                       (d4, n4, "pair, G=3")):
         assert_match_parity(d.cpu().numpy(), n_.cpu().numpy(), ora, label=lab)
-    assert torch.equal(d1, d3) and torch.equal(n1, n3)      # staging path must not change a bit
+    assert torch.equal(d1, d3) and torch.equal(n1, n3)      # the staging path must not change a bit
+    assert torch.equal(d0, d4) and torch.equal(n0, n4)      # nor may the grouping of blocks into CTAs
+
+
+def test_moving_stats_against_numpy():
+    dims, block = (70, 45, 33), (7, 7, 7)
+    vol = _smooth(dims, 21)
+    vol[:6, :8, :9] = 321.0                                  # a constant corner: SS = 0 -> inv_sd = 0
+    v = vol.astype(np.float64)
+    win = np.lib.stride_tricks.sliding_window_view(v, block[::-1])
+    ss = ((win - win.mean(axis=(3, 4, 5), keepdims=True)) ** 2).sum(axis=(3, 4, 5))
+    want = np.where(ss > 1e-9, 1.0 / np.sqrt(np.maximum(ss, 1e-300)), 0.0)
+    for generic in (0, 1):
+        out = torch.full(vol.shape, -7.0, dtype=torch.float32, device="cuda")
+        got = _with_options({"boxstat_generic": generic}, lambda: nrr.nrr_bm_moving_stats(_cuda(vol), block, out)).cpu().numpy()
+        valid = got[: ss.shape[0], : ss.shape[1], : ss.shape[2]]
+        assert np.all(valid[ss <= 1e-9] == 0.0)
+        rel = np.abs(valid - want)[ss > 1e-9] * np.sqrt(ss[ss > 1e-9])
+        assert rel.max() < 2e-6, rel.max()
+        untouched = np.ones(vol.shape, bool)
+        untouched[: ss.shape[0], : ss.shape[1], : ss.shape[2]] = False
+        assert np.all(got[untouched] == -7.0)
+
+
+def test_select_generic_path_equals_default():
+    cfg = CONFIGS["intraop"]
+    fixed, _, mask = pair("intraop")
+    ora = oracle.select(fixed, cfg.block, cfg.stride, cfg.frac, mask)
+    for generic in (0, 1):
+        blocks, n, ncand, var = _with_options({"select_generic": generic}, lambda: nrr.nrr_bm_select_blocks(
+            _cuda(fixed), cfg.block, cfg.stride, cfg.frac, _cuda(mask), want_var=True))
+        assert_select_parity(blocks.cpu().numpy(), n, ncand, ora, var.cpu().numpy())
 
 
 def test_match_largest_fast_instantiation():
@@ -216,6 +255,25 @@ def test_host_forms_equal_device_forms():
     assert np.array_equal(hd, disp.cpu().numpy()) and np.array_equal(hs, ncc.cpu().numpy())
     rb, rd, rs = nrr.nrr_bm_register_host(fixed, moving, cfg.block, cfg.stride, cfg.window, cfg.frac)
     assert np.array_equal(rb, hb) and np.array_equal(rd, hd) and np.array_equal(rs, hs)
+
+
+@pytest.mark.parametrize("name", ["tiny", "intraop"])
+def test_register_device_form_equals_select_then_match(name):
+    """nrr_bm_register: no host synchronisation, K read on the device by kernels launched for an upper bound."""
+    cfg = CONFIGS[name]
+    fixed, moving, mask = pair(name)
+    f, m, k = _cuda(fixed), _cuda(moving), _cuda(mask)
+    blocks, n, ncand = nrr.nrr_bm_select_blocks(f, cfg.block, cfg.stride, cfg.frac, k)
+    disp, ncc = nrr.nrr_bm_match(f, m, blocks, cfg.block, cfg.window)
+    rb, rn, rd, rs = nrr.nrr_bm_register(f, m, cfg.block, cfg.stride, cfg.window, cfg.frac, k)
+    nrr.nrr_bm_check_async_error()
+    assert int(rn.item()) == n and rb.shape[0] >= n
+    assert torch.equal(rb[:n], blocks) and torch.equal(rd[:n], disp) and torch.equal(rs[:n], ncc)
+    # a capacity below K: the first `capacity` blocks are matched, K is still reported
+    rb2, rn2, rd2, rs2 = nrr.nrr_bm_register(f, m, cfg.block, cfg.stride, cfg.window, cfg.frac, k, capacity=n // 2)
+    torch.cuda.synchronize()
+    assert int(rn2.item()) == n
+    assert torch.equal(rb2, blocks[: n // 2]) and torch.equal(rd2, disp[: n // 2]) and torch.equal(rs2, ncc[: n // 2])
 
 
 @pytest.mark.parametrize("name", ["tiny", "intraop", "fullres"])
