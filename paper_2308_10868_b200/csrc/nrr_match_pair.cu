@@ -38,6 +38,7 @@
 #include <math.h>
 #include <string.h>
 
+#include <functional>
 #include <map>
 #include <mutex>
 #include <vector>
@@ -318,7 +319,7 @@ __device__ __forceinline__ void single_row(const float *urow, const float *rec, 
 struct PairArgs {
     const float *fixed, *moving, *inv_sd, *records;
     const int *blocks;
-    const uint32_t *task_tab;      // [threads]: valid << 31 | g << 16 | dy << 8 | p
+    const uint32_t *task_tab;      // [threads]: valid << 31 | single-row warp << 30 | g << 16 | dy << 8 | p
     const unsigned int *n_dev;     // nullable: the number of blocks is min(n, *n_dev)
     int *out_disp;
     float *out_ncc;
@@ -378,7 +379,7 @@ match_pair_kernel(const __grid_constant__ CUtensorMap tm_moving, const PairArgs 
     // this lane's task
     const uint32_t task = a.task_tab[tid];
     const int g = (task >> 16) & 0xff, dyi = (task >> 8) & 0xff, p = task & 0xff;
-    const bool is_pair = warp < a.n_pair_warps;
+    const bool is_pair = !((task >> 30) & 1);          // uniform over the warp
     const int dzA = is_pair ? 2 * p : WZ - 1;
     __syncthreads();                                   // org[] and the barrier are visible
     const int4 org = ctrl->org[g < gact ? g : 0];
@@ -603,7 +604,32 @@ std::vector<uint32_t> build_task_table(int rz, const PairGeom &g)
         for (int d = 0; d < C::W; ++d) { dy.push_back(d); p.push_back(0); res.push_back((P4 * d + PLANE4 * (WZ - 1)) & 7); }
         place_tasks(tab, g.n_pair_warps * 32 + blk * g.single_lanes_per_block, g.single_lanes_per_block, blk, dy, p, res);
     }
-    return tab;
+    // Warp w issues from scheduler w % 4.  A pair warp carries two rows of work per lane, a single-row warp one:
+    // choose which warp slots the single-row warps take so that the four schedulers get equal work.
+    const int nw = g.n_pair_warps + g.n_single_warps;
+    std::vector<int> best_slots, slots(g.n_single_warps);
+    int best_max = 1 << 30;
+    std::function<void(int, int)> rec = [&](int k, int from) {
+        if (k == g.n_single_warps) {
+            int load[4] = {0, 0, 0, 0};
+            for (int w = 0; w < nw; ++w) load[w & 3] += 2;
+            for (int s : slots) load[s & 3] -= 1;
+            const int mx = std::max(std::max(load[0], load[1]), std::max(load[2], load[3]));
+            if (mx < best_max) { best_max = mx; best_slots = slots; }
+            return;
+        }
+        for (int s = from; s < nw; ++s) { slots[k] = s; rec(k + 1, s + 1); }
+    };
+    rec(0, 0);
+    std::vector<char> is_single(nw, 0);
+    for (int s : best_slots) is_single[s] = 1;
+    std::vector<uint32_t> out((size_t)g.threads, 0u);
+    int vp = 0, vs = g.n_pair_warps;                 // next virtual pair / single warp
+    for (int w = 0; w < nw; ++w) {
+        const int v = is_single[w] ? vs++ : vp++;
+        for (int l = 0; l < 32; ++l) out[(size_t)w * 32 + l] = tab[(size_t)v * 32 + l] | (is_single[w] ? 0x40000000u : 0u);
+    }
+    return out;
 }
 
 std::mutex g_tab_mutex;

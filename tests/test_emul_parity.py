@@ -192,3 +192,19 @@ def test_emulated_register_needs_no_host_side_count():
         assert_match_parity(disp, ncc, ora, "register %s" % (opts,))
         for k in opts:
             _emul.set_option(k, 0)
+
+
+@pytest.mark.parametrize("b,r,rz", [(7, 5, 5), (5, 3, 3), (7, 5, 3)])
+def test_emulated_pair_kernel_every_candidate_row_can_win(b, r, rz):
+    """Plants, for block i, an exact copy of the fixed block at displacement d_i in a noise volume, with the d_i
+    running over EVERY (dy, dz) candidate row and every dx: a candidate row missing from the lane -> task table,
+    or a wrong index in the epilogue, loses its block."""
+    from nrr_inputs.planted import planted_pair
+    fixed, moving, centres, want = planted_pair(b, r, rz)
+    block, window = (b, b, b), (r, r, rz)
+    assert _emul.match_info(fixed.shape[::-1], block, window)["kernel"] == 2
+    disp, ncc = _emul.match(fixed, moving, centres, block, window)
+    assert np.array_equal(disp, want)
+    assert np.all(np.abs(ncc - 1.0) < 1e-5)
+    om = oracle.match(fixed, moving, centres, block, window)
+    assert_match_parity(disp, ncc, om, "planted displacements")

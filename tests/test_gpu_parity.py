@@ -167,6 +167,20 @@ def test_match_every_kernel_on_the_same_input():
     assert torch.equal(d0, d4) and torch.equal(n0, n4)      # nor may the grouping of blocks into CTAs
 
 
+@pytest.mark.parametrize("b,r,rz", [(7, 5, 5), (5, 3, 3), (7, 5, 3), (9, 7, 7), (11, 9, 9), (5, 9, 9), (11, 3, 3)])
+def test_match_every_candidate_row_can_win(b, r, rz):
+    """Planted displacements covering every (dy, dz) candidate row and every dx of the window (nrr_inputs.planted)."""
+    from nrr_inputs.planted import planted_pair
+    fixed, moving, centres, want = planted_pair(b, r, rz)
+    block, window = (b, b, b), (r, r, rz)
+    assert nrr.nrr_bm_match_info(fixed.shape[::-1], block, window)["kernel"] == 2
+    for opts in ({}, {"force_rows": 1}):
+        disp, ncc = _with_options(opts, lambda: nrr.nrr_bm_match(_cuda(fixed), _cuda(moving), _cuda(centres), block, window))
+        nrr.nrr_bm_check_async_error()
+        assert np.array_equal(disp.cpu().numpy(), want), opts
+        assert np.all(np.abs(ncc.cpu().numpy() - 1.0) < 1e-5)
+
+
 def test_moving_stats_against_numpy():
     dims, block = (70, 45, 33), (7, 7, 7)
     vol = _smooth(dims, 21)
@@ -316,19 +330,22 @@ def test_match_parity_highres_sampled():
 
 
 def test_match_parity_batch_sampled():
-    """Config 5: 32 settings on the fullres pair; per setting the selection is checked in full and 48 sampled
-    blocks are checked against the oracle."""
-    cfg = CONFIGS["fullres"]
+    """Config 5: 32 settings on the fullres pair, enqueued as ONE launch sequence (nrr_bm_register: no host
+    synchronisation between settings); per setting the selection is checked in full and 48 sampled blocks are
+    checked against the oracle."""
     fixed, moving, mask = pair("fullres")
     f, m, k = _cuda(fixed), _cuda(moving), _cuda(mask)
-    total_exempt = 0
-    for si, st in enumerate(batch_settings()):
+    settings = list(batch_settings())
+    assert len(settings) == 32
+    launched = [nrr.nrr_bm_register(f, m, st.block, st.stride, st.window, st.frac, k) for st in settings]
+    nrr.nrr_bm_check_async_error()                                   # the only synchronisation
+    total_exempt = total_blocks = 0
+    for si, (st, (rb, rn, rd, rs)) in enumerate(zip(settings, launched)):
+        n = int(rn.item())
         ora_sel = oracle.select(fixed, st.block, st.stride, st.frac, mask)
-        blocks, n, ncand = nrr.nrr_bm_select_blocks(f, st.block, st.stride, st.frac, k)
-        assert_select_parity(blocks.cpu().numpy(), n, ncand, ora_sel)
-        disp, ncc = nrr.nrr_bm_match(f, m, blocks, st.block, st.window)
+        assert_select_parity(rb[:n].cpu().numpy(), n, ora_sel["n_candidates"], ora_sel)
         idx = np.sort(np.random.default_rng(1000 + si).choice(n, 48, replace=False))
         ora = oracle.match(fixed, moving, ora_sel["centres"][idx], st.block, st.window)
-        total_exempt += assert_match_parity(disp.cpu().numpy()[idx], ncc.cpu().numpy()[idx], ora, label=str(st))
-    nrr.nrr_bm_check_async_error()
-    print("batch: 32 settings, %d exempt blocks among the samples" % total_exempt)
+        total_exempt += assert_match_parity(rd[:n].cpu().numpy()[idx], rs[:n].cpu().numpy()[idx], ora, label=str(st))
+        total_blocks += n
+    print("batch: 32 settings, %d blocks, %d exempt blocks among the samples" % (total_blocks, total_exempt))
