@@ -694,6 +694,8 @@ int launch_pair(const float *fixed, const float *moving, const float *inv_sd, In
     static size_t configured_smem = 0;     // per instantiation
     if (g.smem > configured_smem) {
         NRR_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem));
+        // two CTAs per SM only fit if the L1/shared split is at its shared-memory maximum
+        NRR_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared));
         configured_smem = g.smem;
     }
     PairArgs a;

@@ -11,9 +11,12 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(os.path.dirname(HERE))
 CSRC = os.path.join(ROOT, "paper_2308_10868_b200", "csrc")
 SOURCES = ["nrr_api.cu", "nrr_select.cu", "nrr_boxstat.cu", "nrr_match.cu", "nrr_match_pair.cu"]   # not the FFMA microbenchmark
-LIB = os.path.join(HERE, "libnrr_bm_emul.so")
+ASAN = os.environ.get("NRR_EMUL_ASAN", "0") == "1"      # AddressSanitizer build: LD_PRELOAD libasan when loading it
+LIB = os.path.join(HERE, "libnrr_bm_emul_asan.so" if ASAN else "libnrr_bm_emul.so")
 FLAGS = ["-std=c++17", "-O1", "-g", "-ffp-contract=off", "-fPIC", "-fvisibility=hidden", "-fno-strict-aliasing",
          "-Wno-attributes", "-Wno-unknown-pragmas", "-I", os.path.join(HERE, "include")]
+if ASAN:
+    FLAGS += ["-fsanitize=address", "-fno-omit-frame-pointer"]
 
 
 def needs_build() -> bool:
@@ -29,7 +32,7 @@ def needs_build() -> bool:
 def build(force: bool = False) -> str:
     if not force and not needs_build():
         return LIB
-    objdir = os.path.join(HERE, "build")
+    objdir = os.path.join(HERE, "build", "asan" if ASAN else "plain")
     os.makedirs(objdir, exist_ok=True)
     procs, objs = [], []
     for src in SOURCES:
@@ -51,7 +54,7 @@ def build(force: bool = False) -> str:
     if failed:
         raise RuntimeError("g++ failed building the CUDA emulation")
     tmp = LIB + ".tmp.%d" % os.getpid()
-    subprocess.run(["g++", "-shared", "-o", tmp] + objs, check=True)
+    subprocess.run(["g++", "-shared"] + (["-fsanitize=address"] if ASAN else []) + ["-o", tmp] + objs, check=True)
     os.replace(tmp, LIB)
     return LIB
 

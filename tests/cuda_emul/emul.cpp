@@ -15,6 +15,13 @@
 
 #include "include/cuda.h"
 
+#if defined(__SANITIZE_ADDRESS__)      // AddressSanitizer build: tell it about the fiber stacks
+#include <sanitizer/common_interface_defs.h>
+#define EMUL_ASAN 1
+#else
+#define EMUL_ASAN 0
+#endif
+
 namespace emul {
 
 uint3 g_threadIdx, g_blockIdx;
@@ -48,33 +55,64 @@ struct Cta {
     int bar_arrived = 0, bar_count_pred = 0, bar_result = 0;
     unsigned bar_gen = 0;
     unsigned long long progress = 0;
-    std::vector<unsigned char> smem;
+    unsigned char *smem_raw = nullptr;
+    size_t smem_bytes = 0;
     unsigned char *smem_aligned = nullptr;
     std::map<void *, MBar> mbars;
     const std::function<void()> *body = nullptr;
     ucontext_t sched;
     Fiber *cur = nullptr;
+    const void *sched_stack_bottom = nullptr;
+    size_t sched_stack_size = 0;
 };
 
 Cta *g_cta = nullptr;
 
+// All context switches go through these two, so that the sanitizer (when built with it) follows the stacks.
+void switch_to_fiber(Cta *c, Fiber *f)
+{
+#if EMUL_ASAN
+    void *fake = nullptr;
+    __sanitizer_start_switch_fiber(&fake, f->stack.data(), f->stack.size());
+    swapcontext(&c->sched, &f->ctx);
+    __sanitizer_finish_switch_fiber(fake, nullptr, nullptr);
+#else
+    swapcontext(&c->sched, &f->ctx);
+#endif
+}
+void switch_to_scheduler(Cta *c, Fiber *f, bool final)
+{
+#if EMUL_ASAN
+    void *fake = nullptr;
+    __sanitizer_start_switch_fiber(final ? nullptr : &fake, c->sched_stack_bottom, c->sched_stack_size);
+    swapcontext(&f->ctx, &c->sched);
+    __sanitizer_finish_switch_fiber(fake, nullptr, nullptr);
+#else
+    (void)final;
+    swapcontext(&f->ctx, &c->sched);
+#endif
+}
+
 void fiber_entry()
 {
     Cta *c = g_cta;
+#if EMUL_ASAN
+    __sanitizer_finish_switch_fiber(nullptr, &c->sched_stack_bottom, &c->sched_stack_size);
+#endif
     (*c->body)();
     Fiber *f = c->cur;
     f->done = true;
     c->live--;
     c->warps[f->warp].live_mask &= ~(1u << f->lane);
     c->progress++;
-    swapcontext(&f->ctx, &c->sched);
+    switch_to_scheduler(c, f, true);
 }
 
 void yield()
 {
     Cta *c = g_cta;
     Fiber *f = c->cur;
-    swapcontext(&f->ctx, &c->sched);
+    switch_to_scheduler(c, f, false);
     // resumed: the scheduler has restored cur and the built-in indices
 }
 
@@ -218,9 +256,13 @@ void launch(dim3 grid, dim3 block, size_t smem, const std::function<void()> &bod
     cta.body = &body;
     cta.fibers.resize(nthreads);
     cta.warps.resize((nthreads + 31) / 32);
-    cta.smem.resize(smem + 256);
-    cta.smem_aligned = (unsigned char *)(((uintptr_t)cta.smem.data() + 127) & ~(uintptr_t)127);
-    cta.smem_aligned += 16;      // like the hardware, promise no more than 16-byte alignment of the base
+    // The window ends exactly where the allocation ends (a sanitizer build then sees every overrun), and its
+    // base promises no more than 16-byte alignment, like the hardware.
+    unsigned char *raw = nullptr;
+    if (posix_memalign((void **)&raw, 128, 128 + smem + 16) != 0) trap("out of memory");
+    cta.smem_raw = raw;
+    cta.smem_bytes = 128 + smem + 16;
+    cta.smem_aligned = raw + 128 + 16;
     for (Fiber &f : cta.fibers) f.stack.resize(kStack);
     g_blockDim = block;
     g_gridDim = grid;
@@ -234,7 +276,7 @@ void launch(dim3 grid, dim3 block, size_t smem, const std::function<void()> &bod
                 cta.bar_arrived = cta.bar_count_pred = 0;
                 cta.mbars.clear();
                 // uninitialised shared memory must not look initialised
-                memset(cta.smem.data(), 0xA5, cta.smem.size());
+                memset(cta.smem_raw, 0xA5, cta.smem_bytes);
                 for (WarpState &w : cta.warps) { w.arrived_mask = 0; w.live_mask = 0; }
                 for (int t = 0; t < nthreads; ++t) {
                     Fiber &f = cta.fibers[t];
@@ -258,7 +300,7 @@ void launch(dim3 grid, dim3 block, size_t smem, const std::function<void()> &bod
                         if (f.done) continue;
                         cta.cur = &f;
                         g_threadIdx = f.tid;
-                        swapcontext(&cta.sched, &f.ctx);
+                        switch_to_fiber(&cta, &f);
                         if (f.done) {      // an exit can complete a barrier / collective the others wait on
                             cta_barrier_check(&cta);
                             warp_check(cta.warps[f.warp]);
@@ -271,6 +313,7 @@ void launch(dim3 grid, dim3 block, size_t smem, const std::function<void()> &bod
                 }
             }
     g_cta = prev;
+    free(cta.smem_raw);
 }
 
 }  // namespace emul
@@ -288,9 +331,10 @@ cudaError_t cudaDeviceGetDefaultMemPool(cudaMemPool_t *pool, int) { *pool = null
 cudaError_t cudaMemPoolSetAttribute(cudaMemPool_t, cudaMemPoolAttr, void *) { return cudaSuccess; }
 cudaError_t cudaMalloc(void **p, size_t bytes)
 {
-    *p = aligned_alloc(256, (bytes + 255) / 256 * 256 + 256);
-    if (*p) memset(*p, 0xCD, bytes);      // device memory is not zero-initialised
-    return *p ? cudaSuccess : cudaErrorEmul;
+    *p = nullptr;
+    if (posix_memalign(p, 256, bytes ? bytes : 1) != 0) return cudaErrorEmul;      // exact size: overruns are visible to a sanitizer
+    memset(*p, 0xCD, bytes);              // device memory is not zero-initialised
+    return cudaSuccess;
 }
 cudaError_t cudaFree(void *p) { free(p); return cudaSuccess; }
 cudaError_t cudaMallocHost(void **p, size_t bytes) { return cudaMalloc(p, bytes); }
