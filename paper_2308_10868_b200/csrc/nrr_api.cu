@@ -33,6 +33,8 @@ thread_local unsigned int *t_err_flag = nullptr;      // device, sticky "a block
 thread_local void *t_pinned = nullptr;                // small pinned staging buffer
 thread_local cudaStream_t t_host_stream = nullptr;    // stream of the *_host entry points
 thread_local bool t_pool_configured = false;
+thread_local cudaStream_t t_side_stream = nullptr;    // nrr_bm_register: moving statistics run beside the selection
+thread_local cudaEvent_t t_ev_fork = nullptr, t_ev_join = nullptr;
 
 constexpr size_t kPinnedBytes = 4096;
 
@@ -189,6 +191,31 @@ int register_device(const float *fixed, const float *moving, const int dims[3], 
     const Int3 g = grid_of(dims, block, stride);
     const long long ngrid = (long long)g.x * g.y * g.z;
     if (ngrid > 0x7fffffffll) return fail(NRR_E_DIMS, "stride grid has %lld positions (limit 2^31-1)", ngrid);
+    // K = floor(0.5 + N*frac) with N <= ngrid candidates, so K <= floor(0.5 + ngrid*frac)
+    double kmax = floor(0.5 + (double)ngrid * frac);
+    if (kmax > (double)ngrid) kmax = (double)ngrid;
+    const int n_cap = (int)(kmax < (double)capacity ? kmax : (double)capacity);
+    // The moving-volume statistics do not depend on the selection: fork them onto a side stream so that both
+    // (each far from filling the GPU for long) overlap; the matching kernels join.
+    float *inv_sd = nullptr;
+    bool forked = false;
+    if (n_cap > 0) {
+        const size_t nvox = (size_t)dims[0] * dims[1] * dims[2];
+        NRR_CUDA(cudaMallocAsync((void **)&inv_sd, nvox * sizeof(float), stream));
+        if (!t_side_stream) {
+            NRR_CUDA(cudaStreamCreateWithFlags(&t_side_stream, cudaStreamNonBlocking));
+            NRR_CUDA(cudaEventCreateWithFlags(&t_ev_fork, cudaEventDisableTiming));
+            NRR_CUDA(cudaEventCreateWithFlags(&t_ev_join, cudaEventDisableTiming));
+        }
+        NRR_CUDA(cudaEventRecord(t_ev_fork, stream));
+        NRR_CUDA(cudaStreamWaitEvent(t_side_stream, t_ev_fork, 0));
+        Span s1(1, t_side_stream);
+        rc = boxstat_enqueue(moving, i3(dims), i3(block), inv_sd, t_side_stream);
+        s1.stop();
+        NRR_CUDA(cudaEventRecord(t_ev_join, t_side_stream));
+        forked = true;
+        if (rc) { cudaStreamWaitEvent(stream, t_ev_join, 0); cudaFreeAsync(inv_sd, stream); return rc; }
+    }
     void *scratch = nullptr;
     NRR_CUDA(cudaMallocAsync(&scratch, select_scratch_bytes(ngrid), stream));
     SelectState *st = nullptr;
@@ -196,28 +223,14 @@ int register_device(const float *fixed, const float *moving, const int dims[3], 
     rc = select_enqueue(fixed, i3(dims), i3(block), i3(stride), g, frac, mask, out_blocks, capacity, nullptr, scratch,
                         &st, stream);
     span.stop();
+    if (forked) NRR_CUDA(cudaStreamWaitEvent(stream, t_ev_join, 0));
     if (rc == NRR_OK && out_n_dev)
         rc = cudaMemcpyAsync(out_n_dev, &st->k, sizeof(int), cudaMemcpyDeviceToDevice, stream) == cudaSuccess
                  ? NRR_OK : fail(NRR_E_CUDA, "copy of K failed");
-    // K = floor(0.5 + N*frac) with N <= ngrid candidates, so K <= floor(0.5 + ngrid*frac)
-    double kmax = floor(0.5 + (double)ngrid * frac);
-    if (kmax > (double)ngrid) kmax = (double)ngrid;
-    const int n_cap = (int)(kmax < (double)capacity ? kmax : (double)capacity);
-    if (rc == NRR_OK && n_cap > 0) {
-        const size_t nvox = (size_t)dims[0] * dims[1] * dims[2];
-        float *inv_sd = nullptr;
-        cudaError_t e = cudaMallocAsync((void **)&inv_sd, nvox * sizeof(float), stream);
-        if (e != cudaSuccess) rc = cuda_fail(e, "cudaMallocAsync");
-        if (rc == NRR_OK) {
-            Span s1(1, stream);
-            rc = boxstat_enqueue(moving, i3(dims), i3(block), inv_sd, stream);
-            s1.stop();
-        }
-        if (rc == NRR_OK)
-            rc = match_enqueue(fixed, moving, inv_sd, i3(dims), out_blocks, n_cap, &st->k, i3(block), i3(window),
-                               out_disp, out_ncc, t_err_flag, stream);
-        if (inv_sd) cudaFreeAsync(inv_sd, stream);
-    }
+    if (rc == NRR_OK && n_cap > 0)
+        rc = match_enqueue(fixed, moving, inv_sd, i3(dims), out_blocks, n_cap, &st->k, i3(block), i3(window),
+                           out_disp, out_ncc, t_err_flag, stream);
+    if (inv_sd) cudaFreeAsync(inv_sd, stream);
     cudaError_t e = cudaFreeAsync(scratch, stream);
     if (rc == NRR_OK && e != cudaSuccess) return cuda_fail(e, "cudaFreeAsync");
     return rc;

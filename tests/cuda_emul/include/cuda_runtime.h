@@ -61,7 +61,7 @@ enum { cudaSharedmemCarveoutMaxShared = 100 };
 enum cudaMemPoolAttr { cudaMemPoolAttrReleaseThreshold = 4 };
 enum cudaDeviceAttr { cudaDevAttrMultiProcessorCount = 16 };
 enum cudaDriverEntryPointQueryResult { cudaDriverEntryPointSuccess = 0, cudaDriverEntryPointSymbolNotFound = 1 };
-enum { cudaEnableDefault = 0, cudaStreamNonBlocking = 1 };
+enum { cudaEnableDefault = 0, cudaStreamNonBlocking = 1, cudaEventDisableTiming = 2 };
 
 cudaError_t cudaGetDevice(int *dev);
 cudaError_t cudaDeviceGetAttribute(int *v, cudaDeviceAttr a, int dev);
@@ -78,6 +78,8 @@ cudaError_t cudaMemcpyAsync(void *d, const void *s, size_t bytes, cudaMemcpyKind
 cudaError_t cudaStreamSynchronize(cudaStream_t s);
 cudaError_t cudaStreamCreateWithFlags(cudaStream_t *s, unsigned flags);
 cudaError_t cudaEventCreate(cudaEvent_t *e);
+cudaError_t cudaEventCreateWithFlags(cudaEvent_t *e, unsigned flags);
+cudaError_t cudaStreamWaitEvent(cudaStream_t s, cudaEvent_t e, unsigned flags);
 cudaError_t cudaEventDestroy(cudaEvent_t e);
 cudaError_t cudaEventRecord(cudaEvent_t e, cudaStream_t s);
 cudaError_t cudaEventSynchronize(cudaEvent_t e);
