@@ -57,6 +57,9 @@ def _load():
     lib.nrr_oracle_select.restype = ctypes.c_int
     lib.nrr_oracle_select.argtypes = [c_flt_p, c_int_p, c_int_p, c_int_p, ctypes.c_double, c_u8_p,
                                       c_int_p, ctypes.c_int, c_int_p, c_dbl_p, c_int_p, c_dbl_p]
+    lib.nrr_oracle_select_pruned.restype = ctypes.c_int
+    lib.nrr_oracle_select_pruned.argtypes = [c_flt_p, c_int_p, c_int_p, c_int_p, ctypes.c_double, c_u8_p, ctypes.c_int,
+                                             c_int_p, ctypes.c_int, c_int_p, c_dbl_p, c_int_p]
     lib.nrr_oracle_match.restype = ctypes.c_int
     lib.nrr_oracle_match.argtypes = [c_flt_p, c_flt_p, c_int_p, c_int_p, ctypes.c_int, c_int_p, c_int_p,
                                      c_int_p, c_dbl_p, c_dbl_p, c_int_p, ctypes.c_int]
@@ -138,6 +141,33 @@ def select(fixed: np.ndarray, block, stride, frac: float, mask: Optional[np.ndar
     k = n.value
     return {"centres": centres[:k].copy(), "var": var[:k].copy(), "n_candidates": ncand.value,
             "margin": margin.value}
+
+
+def select_pruned(fixed: np.ndarray, block, stride, frac: float, mask: Optional[np.ndarray] = None,
+                  connectivity: int = 6):
+    """Selection under the paper's connectivity pattern (reading Q20: greedy in (variance desc,
+    index asc) order on the candidate grid).  Returns dict(centres int32 [n][3], var float64 [n], n_candidates)."""
+    fixed = _f32(fixed)
+    dims = _dims_of(fixed)
+    g = grid(dims, block, stride)
+    cap = max(1, g[0] * g[1] * g[2])
+    centres = np.empty((cap, 3), dtype=np.int32)
+    var = np.empty(cap, dtype=np.float64)
+    n = ctypes.c_int(0)
+    ncand = ctypes.c_int(0)
+    mptr = None
+    if mask is not None:
+        mask = np.ascontiguousarray(mask, dtype=np.uint8)
+        if mask.shape != fixed.shape:
+            raise ValueError("mask shape mismatch")
+        mptr = _ptr(mask, ctypes.c_ubyte)
+    rc = _load().nrr_oracle_select_pruned(_ptr(fixed, ctypes.c_float), _i3(dims), _i3(block), _i3(stride),
+                                          float(frac), mptr, int(connectivity), _ptr(centres, ctypes.c_int), cap,
+                                          ctypes.byref(n), _ptr(var, ctypes.c_double), ctypes.byref(ncand))
+    if rc != 0:
+        raise RuntimeError("nrr_oracle_select_pruned failed: %d" % rc)
+    k = n.value
+    return {"centres": centres[:k].copy(), "var": var[:k].copy(), "n_candidates": ncand.value}
 
 
 def match(fixed: np.ndarray, moving: np.ndarray, centres: np.ndarray, block, window, nthreads: int = 0):

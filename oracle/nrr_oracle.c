@@ -25,6 +25,7 @@
  *   - skip rule for candidates whose block leaves the moving volume (Q11)           PARITY UNPINNED
  *   - zero-variance block or candidate => NCC := 0 (Q12)                            PARITY UNPINNED
  *   - output order of the selected set = ascending candidate index (Q8)             PARITY UNPINNED
+ *   - the pruning rule behind the paper's connectivity patterns (Q20)               PARITY UNPINNED
  * Everything else is pinned by tests/test_oracle_*.py (closed forms, numpy.corrcoef, translation
  * recovery, affine invariance, an independent naive evaluator in oracle/naive.py).
  *
@@ -208,6 +209,86 @@ int nrr_oracle_select(const float *fixed, const int dims[3], const int block[3],
         if (out_var) out_var[t] = cand[t].var;
     }
     free(cand);
+    return NRR_ORACLE_OK;
+}
+
+/*
+ * Selection with the connectivity pattern ("The method also uses a connectivity pattern to avoid
+ * selecting blocks that are too close to each other ... Three simplex patterns are available: vertex (26
+ * connectivity), edge (18 connectivity), face (6 connectivity)").  The paper names the patterns but not the
+ * pruning algorithm; reading Q20, PARITY UNPINNED by the paper:
+ *   candidates, variances, N and K = floor(0.5 + N*frac) exactly as in nrr_oracle_select;
+ *   walk the candidates by (variance descending, candidate index ascending); KEEP a candidate iff none of its
+ *   neighbours ON THE CANDIDATE GRID (grid offsets (di,dj,dk) in {-1,0,1}^3 \ {0} with |di|+|dj|+|dk| <= 1 for
+ *   connectivity 6, <= 2 for 18, <= 3 for 26) has been kept already; stop once K are kept or the list ends;
+ *   output the kept centres in ascending candidate index.  connectivity 0 = no pruning.
+ * With stride 1 the grid neighbours are the voxel neighbours of the block centre (the paper's setting: every
+ * intracranial voxel is a feature candidate).  Out-of-mask grid positions are not candidates and block nothing.
+ */
+int nrr_oracle_select_pruned(const float *fixed, const int dims[3], const int block[3], const int stride[3],
+                             double frac, const unsigned char *mask, int connectivity, int *out_centres,
+                             int capacity, int *out_n, double *out_var, int *out_ncand)
+{
+    for (int a = 0; a < 3; ++a)
+        if (dims[a] < 1 || block[a] < 1 || (block[a] & 1) == 0 || stride[a] < 1) return NRR_ORACLE_E_ARG;
+    if (!(frac > 0.0 && frac <= 1.0)) return NRR_ORACLE_E_ARG;
+    if (connectivity != 0 && connectivity != 6 && connectivity != 18 && connectivity != 26) return NRR_ORACLE_E_ARG;
+    const int reach = connectivity == 6 ? 1 : connectivity == 18 ? 2 : connectivity == 26 ? 3 : 0;
+    int g[3];
+    nrr_oracle_grid(dims, block, stride, g);
+    size_t ngrid = (size_t)g[0] * (size_t)g[1] * (size_t)g[2];
+    long nb = (long)block[0] * block[1] * block[2];
+    cand_t *cand = (cand_t *)malloc(sizeof(cand_t) * (ngrid ? ngrid : 1));
+    int *gpos = (int *)malloc(sizeof(int) * 3 * (ngrid ? ngrid : 1));          /* grid coordinates per candidate */
+    unsigned char *kept = (unsigned char *)calloc(ngrid ? ngrid : 1, 1);       /* per GRID position */
+    double *buf = (double *)malloc(sizeof(double) * (size_t)nb);
+    if (!cand || !gpos || !kept || !buf) { free(cand); free(gpos); free(kept); free(buf); return NRR_ORACLE_E_NOMEM; }
+    int n = 0;
+    for (int k = 0; k < g[2]; ++k)
+        for (int j = 0; j < g[1]; ++j)
+            for (int i = 0; i < g[0]; ++i) {
+                int o[3] = { i * stride[0], j * stride[1], k * stride[2] };
+                int c[3] = { o[0] + (block[0] - 1) / 2, o[1] + (block[1] - 1) / 2, o[2] + (block[2] - 1) / 2 };
+                if (mask && mask[vox(dims, c[0], c[1], c[2])] == 0) continue;
+                gather_block(fixed, dims, o, block, buf);
+                cand[n].var = nrr_oracle_variance(buf, nb);
+                cand[n].q = n;
+                cand[n].c[0] = c[0]; cand[n].c[1] = c[1]; cand[n].c[2] = c[2];
+                gpos[3 * n + 0] = i; gpos[3 * n + 1] = j; gpos[3 * n + 2] = k;
+                ++n;
+            }
+    free(buf);
+    int K = nrr_oracle_count(n, frac);
+    if (K > n) K = n;
+    if (out_ncand) *out_ncand = n;
+    qsort(cand, (size_t)n, sizeof(cand_t), cmp_var_desc_q_asc);
+    int nk = 0;                                   /* kept candidates are moved to the front of cand[] */
+    for (int t = 0; t < n && nk < K; ++t) {
+        const int *gp = gpos + 3 * cand[t].q;
+        int blocked = 0;
+        for (int dk = -1; dk <= 1 && !blocked; ++dk)
+            for (int dj = -1; dj <= 1 && !blocked; ++dj)
+                for (int di = -1; di <= 1 && !blocked; ++di) {
+                    int m = abs(di) + abs(dj) + abs(dk);
+                    if (m == 0 || m > reach) continue;
+                    int i = gp[0] + di, j = gp[1] + dj, k = gp[2] + dk;
+                    if (i < 0 || j < 0 || k < 0 || i >= g[0] || j >= g[1] || k >= g[2]) continue;
+                    if (kept[((size_t)k * g[1] + j) * g[0] + i]) blocked = 1;
+                }
+        if (blocked) continue;
+        kept[((size_t)gp[2] * g[1] + gp[1]) * g[0] + gp[0]] = 1;
+        cand[nk++] = cand[t];
+    }
+    *out_n = nk;
+    if (nk > capacity) { free(cand); free(gpos); free(kept); return NRR_ORACLE_E_CAPACITY; }
+    qsort(cand, (size_t)nk, sizeof(cand_t), cmp_q_asc);
+    for (int t = 0; t < nk; ++t) {
+        out_centres[3 * t + 0] = cand[t].c[0];
+        out_centres[3 * t + 1] = cand[t].c[1];
+        out_centres[3 * t + 2] = cand[t].c[2];
+        if (out_var) out_var[t] = cand[t].var;
+    }
+    free(cand); free(gpos); free(kept);
     return NRR_ORACLE_OK;
 }
 

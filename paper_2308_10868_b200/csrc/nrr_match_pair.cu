@@ -48,6 +48,7 @@
 namespace nrr {
 
 extern float g_tie_band;
+extern int g_disable_tma;
 int g_pair_g = 0;             // experiment knob: force the number of blocks per CTA (0 = planner's choice)
 
 namespace {
@@ -665,7 +666,7 @@ int launch_pair(const float *fixed, const float *moving, const float *inv_sd, In
     PairGeom g;
     if (!pair_plan<B, R>(rz, &g)) return NRR_OK;
     if (plan_only) {
-        if (!tma_eligible(dims, moving, B + 2 * rz) && moving) return NRR_OK;
+        if (g_disable_tma || dims.x % 4 != 0 || B + 2 * rz > 256) return NRR_OK;      // what the volume shape alone decides
         *handled = true;
         plan_only->fast = 2;
         plan_only->threads = g.threads;

@@ -348,3 +348,89 @@ def test_tiny_config_exact_recovery_with_noise():
     assert inside.sum() >= 200
     assert np.all(res["disp"][inside] == np.asarray(cfg.shift))
     assert np.all(res["ncc"][inside] > 0.9)
+
+
+# ------------------------------------------------------------------------- selection with a connectivity pattern
+def _pruned_bruteforce(vol, block, stride, frac, mask, connectivity):
+    """Independent restatement (numpy + python sets) of reading Q20: greedy by (variance desc, index asc)."""
+    nz, ny, nx = vol.shape
+    g = [(n - b) // s + 1 for n, b, s in zip((nx, ny, nz), block, stride)]
+    reach = {0: 0, 6: 1, 18: 2, 26: 3}[connectivity]
+    cands = []
+    for k in range(g[2]):
+        for j in range(g[1]):
+            for i in range(g[0]):
+                o = (i * stride[0], j * stride[1], k * stride[2])
+                c = tuple(o[a] + (block[a] - 1) // 2 for a in range(3))
+                if mask is not None and mask[c[2], c[1], c[0]] == 0:
+                    continue
+                blk = vol[o[2]:o[2] + block[2], o[1]:o[1] + block[1], o[0]:o[0] + block[0]].astype(np.float64)
+                # the variance itself is pinned elsewhere; taking the oracle's keeps exact ties exact here
+                cands.append((oracle.variance(blk.ravel()), len(cands), (i, j, k), c))
+    K = min(len(cands), int(math.floor(0.5 + len(cands) * frac)))
+    kept, kept_pos = [], set()
+    for var, q, gp, c in sorted(cands, key=lambda t: (-t[0], t[1])):
+        if len(kept) == K:
+            break
+        nb = [(gp[0] + di, gp[1] + dj, gp[2] + dk) for di in (-1, 0, 1) for dj in (-1, 0, 1) for dk in (-1, 0, 1)
+              if 0 < abs(di) + abs(dj) + abs(dk) <= reach]
+        if any(p in kept_pos for p in nb):
+            continue
+        kept.append((q, c))
+        kept_pos.add(gp)
+    kept.sort()
+    return np.asarray([c for _, c in kept], dtype=np.int32).reshape(-1, 3), len(cands)
+
+
+def test_select_pruned_without_pattern_equals_plain_selection():
+    vol = np.random.default_rng(3).uniform(0, 1000, (14, 13, 12)).astype(np.float32)
+    a = oracle.select(vol, (3, 3, 3), (1, 1, 1), 0.2)
+    b = oracle.select_pruned(vol, (3, 3, 3), (1, 1, 1), 0.2, None, 0)
+    assert np.array_equal(a["centres"], b["centres"]) and np.array_equal(a["var"], b["var"])
+
+
+def test_select_pruned_uniform_image_closed_forms():
+    """All variances equal -> candidates are walked in index order, so the kept set has a closed form:
+    face (6): i+j+k even; vertex (26): i, j, k all even; on a line every other candidate."""
+    vol = np.full((9, 9, 9), 5.0, np.float32)                     # 7x7x7 grid of 3^3 blocks at stride 1
+    c = oracle.select_pruned(vol, (3, 3, 3), (1, 1, 1), 1.0, None, 6)["centres"] - 1        # grid coordinates
+    want = [(i, j, k) for k in range(7) for j in range(7) for i in range(7) if (i + j + k) % 2 == 0]
+    assert c.tolist() == [list(t) for t in want]
+    c = oracle.select_pruned(vol, (3, 3, 3), (1, 1, 1), 1.0, None, 26)["centres"] - 1
+    want = [(i, j, k) for k in range(0, 7, 2) for j in range(0, 7, 2) for i in range(0, 7, 2)]
+    assert c.tolist() == [list(t) for t in want]
+    line = np.full((3, 3, 12), 5.0, np.float32)                   # a 10x1x1 grid
+    for conn in (6, 18, 26):
+        c = oracle.select_pruned(line, (3, 3, 3), (1, 1, 1), 1.0, None, conn)["centres"]
+        assert c[:, 0].tolist() == [1, 3, 5, 7, 9]
+    # the count rule stops the walk: K = floor(0.5 + 10 * 0.25) = 3 kept, the first three of the pattern
+    c = oracle.select_pruned(line, (3, 3, 3), (1, 1, 1), 0.25, None, 6)["centres"]
+    assert c[:, 0].tolist() == [1, 3, 5]
+
+
+@pytest.mark.parametrize("conn", [6, 18, 26])
+@pytest.mark.parametrize("stride,frac,use_mask", [((1, 1, 1), 0.1, False), ((1, 1, 1), 0.6, True), ((2, 1, 3), 0.5, False)])
+def test_select_pruned_matches_bruteforce_and_is_an_independent_set(conn, stride, frac, use_mask):
+    rng = np.random.default_rng(40 + conn)
+    vol = rng.uniform(0, 1000, (11, 12, 13)).astype(np.float32)
+    vol[:4] = np.round(vol[:4] / 250.0) * 250.0                   # many exact variance ties
+    mask = (rng.uniform(size=vol.shape) < 0.7).astype(np.uint8) if use_mask else None
+    got = oracle.select_pruned(vol, (3, 3, 3), stride, frac, mask, conn)
+    want, ncand = _pruned_bruteforce(vol, (3, 3, 3), stride, frac, mask, conn)
+    assert got["n_candidates"] == ncand
+    assert np.array_equal(got["centres"], want)
+    # invariant: no two kept centres are neighbours under the pattern (grid coordinates)
+    gp = (got["centres"] - 1) // np.asarray(stride)
+    d = np.abs(gp[:, None, :] - gp[None, :, :])
+    near = (d.max(axis=2) <= 1) & (d.sum(axis=2) <= {6: 1, 18: 2, 26: 3}[conn]) & (d.sum(axis=2) > 0)
+    assert not near.any()
+    assert len(got["centres"]) <= oracle.count(ncand, frac)
+
+
+def test_select_pruned_isolated_candidates_are_untouched():
+    vol = np.random.default_rng(9).uniform(0, 1000, (12, 12, 12)).astype(np.float32)
+    mask = np.zeros(vol.shape, np.uint8)
+    mask[1::3, 1::3, 1::3] = 1                                    # candidates three voxels apart: never neighbours
+    a = oracle.select(vol, (3, 3, 3), (1, 1, 1), 0.5, mask)
+    b = oracle.select_pruned(vol, (3, 3, 3), (1, 1, 1), 0.5, mask, 26)
+    assert np.array_equal(a["centres"], b["centres"])
