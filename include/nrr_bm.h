@@ -86,6 +86,27 @@ NRR_BM_API int nrr_bm_select_blocks(const float *fixed, const int dims[3], const
                          double *out_var, int *out_ncand, void *stream);
 
 /*
+ * Selection under the paper's connectivity pattern  --  PAPER.md:376 (section 4.1): "The method also uses a
+ * connectivity pattern to avoid selecting blocks that are too close to each other ... vertex (26 connectivity),
+ * edge (18 connectivity), face (6 connectivity)".  The paper names the patterns, not the algorithm; this library
+ * reads it (Q20) as the greedy walk by (variance descending, candidate index ascending) that keeps a
+ * candidate iff none of its pattern neighbours ON THE CANDIDATE GRID (grid offsets with |di|+|dj|+|dk| <= 1 / 2
+ * / 3 for 6 / 18 / 26) is kept already, and stops at K = floor(0.5 + N*frac) kept or at the end of the list.
+ * With stride 1 (the paper's setting: every intracranial voxel is a candidate) the grid neighbours are the voxel
+ * neighbours of the block centre.  connectivity = 0 is nrr_bm_select_blocks.  Everything else (candidates,
+ * variance, outputs in ascending candidate index, *out_n on the HOST) as in nrr_bm_select_blocks; *out_n can be
+ * below K when the pattern leaves fewer candidates.  The call synchronises `stream` several times (it polls
+ * the device between batches of pruning rounds); selection is pre-operative.
+ */
+NRR_BM_API int nrr_bm_select_blocks_pruned(const float *fixed, const int dims[3], const int block[3],
+                                const int stride[3], double frac, const unsigned char *mask, int connectivity,
+                                int *out_blocks, int capacity, int *out_n, double *out_var, int *out_ncand,
+                                void *stream);
+NRR_BM_API int nrr_bm_select_blocks_pruned_host(const float *fixed, const int dims[3], const int block[3],
+                                     const int stride[3], double frac, const unsigned char *mask, int connectivity,
+                                     int *out_blocks, int capacity, int *out_n, double *out_var, int *out_ncand);
+
+/*
  * Exhaustive NCC block matching  --  PAPER.md:236-246 (section 3: for each registration point, the block
  * displacement "that maximizes the intensity-based similarity metric", NCC equation) and the listing
  * PAPER.md:659-667 (section 4.3: for each block, each candidate block in the window, similarity, maximum

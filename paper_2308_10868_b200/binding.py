@@ -20,7 +20,7 @@ NRR_E_NULL, NRR_E_DIMS, NRR_E_BLOCK, NRR_E_STRIDE, NRR_E_WINDOW, NRR_E_FRAC = -1
 NRR_E_CAPACITY, NRR_E_BOUNDS, NRR_E_SMEM, NRR_E_CUDA, NRR_E_ARG = -7, -8, -9, -10, -11
 
 EXPORTS = [
-    "nrr_bm_select_blocks", "nrr_bm_match", "nrr_bm_register", "nrr_bm_check_async_error", "nrr_bm_moving_stats", "nrr_bm_moving_stats_host",
+    "nrr_bm_select_blocks", "nrr_bm_select_blocks_pruned", "nrr_bm_select_blocks_pruned_host", "nrr_bm_match", "nrr_bm_register", "nrr_bm_check_async_error", "nrr_bm_moving_stats", "nrr_bm_moving_stats_host",
     "nrr_bm_select_blocks_host", "nrr_bm_match_host", "nrr_bm_register_host",
     "nrr_bm_profile_enable", "nrr_bm_profile_read", "nrr_bm_launch_count", "nrr_bm_match_info",
     "nrr_bm_fp32_peak", "nrr_bm_set_option", "nrr_bm_last_error", "nrr_bm_status_string", "nrr_bm_version",
@@ -51,6 +51,10 @@ def lib() -> ctypes.CDLL:
     L.nrr_bm_select_blocks.argtypes = [vp, i3, i3, i3, cd, vp, vp, ci, i3, vp, i3, vp]
     L.nrr_bm_match.restype = ci
     L.nrr_bm_match.argtypes = [vp, vp, i3, vp, ci, i3, i3, vp, vp, vp]
+    L.nrr_bm_select_blocks_pruned.restype = ci
+    L.nrr_bm_select_blocks_pruned.argtypes = [vp, i3, i3, i3, cd, vp, ci, vp, ci, ctypes.POINTER(ci), vp, ctypes.POINTER(ci), vp]
+    L.nrr_bm_select_blocks_pruned_host.restype = ci
+    L.nrr_bm_select_blocks_pruned_host.argtypes = [vp, i3, i3, i3, cd, vp, ci, vp, ci, ctypes.POINTER(ci), vp, ctypes.POINTER(ci)]
     L.nrr_bm_register.restype = ci
     L.nrr_bm_register.argtypes = [vp, vp, i3, i3, i3, i3, cd, vp, vp, ci, vp, vp, vp, vp]
     L.nrr_bm_moving_stats.restype = ci
@@ -150,6 +154,37 @@ def nrr_bm_select_blocks(fixed, block, stride, frac: float, mask=None, capacity:
                                           mask.data_ptr() if mask is not None else None, out_blocks.data_ptr(),
                                           int(capacity), ctypes.byref(n), out_var.data_ptr() if want_var else None,
                                           ctypes.byref(ncand), _stream_ptr(stream)))
+    k = n.value
+    if want_var:
+        return out_blocks[:k], k, ncand.value, out_var[:k]
+    return out_blocks[:k], k, ncand.value
+
+
+def nrr_bm_select_blocks_pruned(fixed, block, stride, frac: float, mask=None, connectivity: int = 6,
+                                capacity: Optional[int] = None, want_var: bool = False, stream=None):
+    """Device form of the selection under a connectivity pattern (0, 6, 18, 26). Same returns as nrr_bm_select_blocks."""
+    import torch
+    fixed = _dev(fixed, torch.float32, "fixed")
+    dims = _dims_of(fixed)
+    if mask is not None:
+        mask = _dev(mask, torch.uint8, "mask")
+        if tuple(mask.shape) != tuple(fixed.shape):
+            raise ValueError("mask shape mismatch")
+    if capacity is None:
+        capacity = 1
+        for a in range(3):
+            capacity *= max(0, (dims[a] - int(block[a])) // max(1, int(stride[a])) + 1)
+        capacity = max(1, capacity)
+    out_blocks = torch.empty((capacity, 3), dtype=torch.int32, device=fixed.device)
+    out_var = torch.empty((capacity,), dtype=torch.float64, device=fixed.device) if want_var else None
+    n = ctypes.c_int(0)
+    ncand = ctypes.c_int(0)
+    with torch.cuda.device(fixed.device):
+        _check(lib().nrr_bm_select_blocks_pruned(fixed.data_ptr(), _i3(dims), _i3(block), _i3(stride), float(frac),
+                                                 mask.data_ptr() if mask is not None else None, int(connectivity),
+                                                 out_blocks.data_ptr(), int(capacity), ctypes.byref(n),
+                                                 out_var.data_ptr() if want_var else None, ctypes.byref(ncand),
+                                                 _stream_ptr(stream)))
     k = n.value
     if want_var:
         return out_blocks[:k], k, ncand.value, out_var[:k]

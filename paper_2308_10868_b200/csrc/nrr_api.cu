@@ -129,7 +129,7 @@ Int3 grid_of(const int dims[3], const int block[3], const int stride[3])
 // Device select; returns K through *out_n after one synchronisation.
 int select_device(const float *fixed, const int dims[3], const int block[3], const int stride[3], double frac,
                   const unsigned char *mask, int *out_blocks, int capacity, int *out_n, double *out_var,
-                  int *out_ncand, cudaStream_t stream)
+                  int *out_ncand, cudaStream_t stream, int connectivity = 0)
 {
     int rc = ensure_thread_state();
     if (rc) return rc;
@@ -141,7 +141,7 @@ int select_device(const float *fixed, const int dims[3], const int block[3], con
     SelectState *st = nullptr;
     Span span(0, stream);
     rc = select_enqueue(fixed, i3(dims), i3(block), i3(stride), g, frac, mask, out_blocks, capacity, out_var, scratch,
-                        &st, stream);
+                        &st, stream, connectivity, (SelectState *)((char *)t_pinned + 3072));
     span.stop();
     if (rc) { cudaFreeAsync(scratch, stream); return rc; }
     SelectState *h = (SelectState *)t_pinned;
@@ -321,6 +321,45 @@ int nrr_bm_select_blocks(const float *fixed, const int dims[3], const int block[
     if (rc) return rc;
     return select_device(fixed, dims, block, stride, frac, mask, out_blocks, capacity, out_n, out_var, out_ncand,
                          (cudaStream_t)stream);
+}
+
+int nrr_bm_select_blocks_pruned(const float *fixed, const int dims[3], const int block[3], const int stride[3],
+                                double frac, const unsigned char *mask, int connectivity, int *out_blocks,
+                                int capacity, int *out_n, double *out_var, int *out_ncand, void *stream)
+{
+    int rc = check_select_args(fixed, dims, block, stride, frac, out_blocks, capacity, out_n);
+    if (rc) return rc;
+    if (connectivity != 0 && connectivity != 6 && connectivity != 18 && connectivity != 26)
+        return fail(NRR_E_ARG, "connectivity = %d (0, 6, 18 or 26)", connectivity);
+    return select_device(fixed, dims, block, stride, frac, mask, out_blocks, capacity, out_n, out_var, out_ncand,
+                         (cudaStream_t)stream, connectivity);
+}
+
+int nrr_bm_select_blocks_pruned_host(const float *fixed, const int dims[3], const int block[3], const int stride[3],
+                                     double frac, const unsigned char *mask, int connectivity, int *out_blocks,
+                                     int capacity, int *out_n, double *out_var, int *out_ncand)
+{
+    int rc = check_select_args(fixed, dims, block, stride, frac, out_blocks, capacity, out_n);
+    if (rc) return rc;
+    if (connectivity != 0 && connectivity != 6 && connectivity != 18 && connectivity != 26)
+        return fail(NRR_E_ARG, "connectivity = %d (0, 6, 18 or 26)", connectivity);
+    if ((rc = ensure_thread_state())) return rc;
+    cudaStream_t s;
+    if ((rc = host_stream(&s))) return rc;
+    const size_t nvox = (size_t)dims[0] * dims[1] * dims[2];
+    DevBuf d_fixed(s), d_mask(s), d_blocks(s), d_var(s);
+    NRR_CUDA(d_fixed.upload(fixed, nvox * sizeof(float)));
+    if (mask) NRR_CUDA(d_mask.upload(mask, nvox));
+    NRR_CUDA(d_blocks.alloc((size_t)capacity * 3 * sizeof(int)));
+    if (out_var) NRR_CUDA(d_var.alloc((size_t)capacity * sizeof(double)));
+    rc = select_device((const float *)d_fixed.p, dims, block, stride, frac, (const unsigned char *)d_mask.p,
+                       (int *)d_blocks.p, capacity, out_n, (double *)d_var.p, out_ncand, s, connectivity);
+    if (rc != NRR_OK && rc != NRR_E_CAPACITY) return rc;
+    const size_t k = (size_t)(*out_n < capacity ? *out_n : capacity);
+    NRR_CUDA(cudaMemcpyAsync(out_blocks, d_blocks.p, k * 3 * sizeof(int), cudaMemcpyDeviceToHost, s));
+    if (out_var) NRR_CUDA(cudaMemcpyAsync(out_var, d_var.p, k * sizeof(double), cudaMemcpyDeviceToHost, s));
+    NRR_CUDA(cudaStreamSynchronize(s));
+    return rc;
 }
 
 int nrr_bm_match(const float *fixed, const float *moving, const int dims[3], const int *blocks, int n,

@@ -51,13 +51,19 @@ struct SelectState {
     unsigned int k_remaining;       // still to take inside the current prefix bucket
     unsigned int ticket[8];         // last-CTA-done counters, one per kernel of the sequence
     unsigned int total_selected;    // written by the compaction scan (== K)
+    unsigned int undecided;         // connectivity pruning: candidates neither kept nor removed yet
+    unsigned int kept;              // connectivity pruning: members of the greedy independent set
 };
 
 size_t select_scratch_bytes(long long ngrid);
+// connectivity: 0 = none, 6 / 18 / 26 = the paper's face / edge / vertex pattern (reading Q20).
+// With a pattern the call polls the device (host_poll: pinned, >= sizeof(SelectState)) between batches of
+// pruning rounds, i.e. it synchronises `stream`; selection is pre-operative.
 // Enqueues the whole selection sequence. `scratch` must hold select_scratch_bytes(ngrid) bytes.
 int select_enqueue(const float *fixed, Int3 dims, Int3 block, Int3 stride, Int3 grid, double frac,
                    const unsigned char *mask, int *out_blocks, int capacity, double *out_var,
-                   void *scratch, SelectState **state_out, cudaStream_t stream);
+                   void *scratch, SelectState **state_out, cudaStream_t stream, int connectivity = 0,
+                   SelectState *host_poll = nullptr);
 
 // ---- moving-volume statistics (nrr_boxstat.cu) ------------------------------------------------------
 // inv_sd[p] = 1/sqrt(sum over the block with ORIGIN p of (m - mean)^2), 0 for zero-variance blocks,

@@ -377,12 +377,13 @@ constexpr long long kSmallLimit = 1ll << 20;      // grid positions up to which 
 
 __global__ void __launch_bounds__(kSmallThreads)
 select_small_kernel(const double *__restrict__ var, long long ngrid, Int3 block, Int3 stride, Int3 grid,
-                    SelectState *st, int *__restrict__ out_blocks, double *__restrict__ out_var, int capacity)
+                    SelectState *st, int *__restrict__ out_blocks, double *__restrict__ out_var, int capacity,
+                    int first_pass)
 {
     __shared__ unsigned int s_hist[kRadixBins];
     __shared__ unsigned long long s_carry;
     const int tid = threadIdx.x;
-    for (int pass = 1; pass < kNumPasses; ++pass) {
+    for (int pass = first_pass; pass < kNumPasses; ++pass) {
         for (int b = tid; b < kRadixBins; b += kSmallThreads) s_hist[b] = 0;
         __syncthreads();
         const unsigned long long prefix = st->prefix, mask = st->mask;
@@ -441,8 +442,86 @@ select_small_kernel(const double *__restrict__ var, long long ngrid, Int3 block,
     }
 }
 
+// ---- connectivity pruning (reading Q20): the greedy walk by (variance desc, index asc) that keeps a
+// candidate iff no kept candidate is among its pattern neighbours on the candidate grid.  A candidate's fate
+// depends only on its HIGHER-priority neighbours, so the walk is the unique fixed point of a local rule that all
+// candidates can apply at once, round after round: removed if a higher-priority neighbour is kept, kept if every
+// higher-priority neighbour is removed, undecided otherwise.  States only move from undecided to a final value
+// and final values are what the rule reads, so in-place, unordered updates reach the same fixed point as the
+// sequential walk; the highest-priority undecided candidate always decides, so the rounds terminate.  Taking the
+// K highest-priority members of the resulting set (the radix select below) is the walk stopped at K kept.
+constexpr unsigned char kUndecided = 0, kKept = 1, kRemoved = 2;
+constexpr int kPruneThreads = 256;
+
+__global__ void __launch_bounds__(kPruneThreads)
+prune_init_kernel(const double *__restrict__ var, long long ngrid, unsigned char *__restrict__ state, SelectState *st)
+{
+    const long long g = (long long)blockIdx.x * kPruneThreads + threadIdx.x;
+    const bool cand = g < ngrid && var[g] >= 0.0;
+    if (g < ngrid) state[g] = cand ? kUndecided : kRemoved;
+    const int cnt = __syncthreads_count(cand ? 1 : 0);
+    if (threadIdx.x == 0 && cnt) atomicAdd(&st->undecided, (unsigned int)cnt);
+}
+
+__global__ void __launch_bounds__(kPruneThreads)
+prune_round_kernel(const double *__restrict__ var, long long ngrid, Int3 grid, int reach,
+                   unsigned char *state, SelectState *st)
+{
+    const long long g = (long long)blockIdx.x * kPruneThreads + threadIdx.x;
+    int decided = 0, keep = 0;
+    if (g < ngrid && ((volatile unsigned char *)state)[g] == kUndecided) {
+        const int i = (int)(g % grid.x);
+        const int j = (int)((g / grid.x) % grid.y);
+        const int k = (int)(g / ((long long)grid.x * grid.y));
+        const unsigned long long key = key_of(var[g]);
+        bool kept_above = false, undecided_above = false;
+        for (int dk = -1; dk <= 1; ++dk)
+            for (int dj = -1; dj <= 1; ++dj)
+                for (int di = -1; di <= 1; ++di) {
+                    const int m = abs(di) + abs(dj) + abs(dk);
+                    if (m == 0 || m > reach) continue;
+                    const int ni = i + di, nj = j + dj, nk = k + dk;
+                    if (ni < 0 || nj < 0 || nk < 0 || ni >= grid.x || nj >= grid.y || nk >= grid.z) continue;
+                    const long long n = ((long long)nk * grid.y + nj) * grid.x + ni;
+                    const unsigned char s = ((volatile unsigned char *)state)[n];
+                    if (s == kRemoved) continue;
+                    const unsigned long long nkey = key_of(var[n]);
+                    if (!(nkey > key || (nkey == key && n < g))) continue;      // lower priority: irrelevant
+                    if (s == kKept) kept_above = true;
+                    else undecided_above = true;
+                }
+        if (kept_above) { state[g] = kRemoved; decided = 1; }
+        else if (!undecided_above) { state[g] = kKept; decided = 1; keep = 1; }
+    }
+    const int nd = __syncthreads_count(decided);
+    const int nk = __syncthreads_count(keep);
+    if (threadIdx.x == 0) {
+        if (nd) atomicSub(&st->undecided, (unsigned int)nd);
+        if (nk) atomicAdd(&st->kept, (unsigned int)nk);
+    }
+}
+
+// Candidates outside the independent set drop out of the ranking (variance -1 = key 0).
+__global__ void __launch_bounds__(kPruneThreads)
+prune_apply_kernel(double *__restrict__ var, long long ngrid, const unsigned char *__restrict__ state)
+{
+    const long long g = (long long)blockIdx.x * kPruneThreads + threadIdx.x;
+    if (g < ngrid && state[g] != kKept) var[g] = -1.0;
+}
+
+// K := min(K, |set|); the radix select starts over on the pruned keys.
+__global__ void prune_finish_kernel(SelectState *st)
+{
+    const unsigned int k = st->k < st->kept ? st->k : st->kept;
+    st->k = k;
+    st->k_remaining = k;
+    st->prefix = 0ull;
+    st->mask = 0ull;
+    st->ticket[0] = 0u;
+}
+
 struct ScratchLayout {
-    size_t state, hist, var, counts, offsets, total;
+    size_t state, hist, var, counts, offsets, prune, total;
 };
 
 ScratchLayout layout(long long ngrid)
@@ -455,6 +534,7 @@ ScratchLayout layout(long long ngrid)
     L.var = off;     off += sizeof(double) * (size_t)(ngrid > 0 ? ngrid : 1);
     L.counts = off;  off += sizeof(unsigned long long) * nchunks;
     L.offsets = off; off += sizeof(unsigned long long) * nchunks;
+    L.prune = off;   off += ((size_t)(ngrid > 0 ? ngrid : 1) + 15) / 16 * 16;             // one state byte per grid position
     L.total = off;
     return L;
 }
@@ -465,7 +545,7 @@ size_t select_scratch_bytes(long long ngrid) { return layout(ngrid).total; }
 
 int select_enqueue(const float *fixed, Int3 dims, Int3 block, Int3 stride, Int3 grid, double frac,
                    const unsigned char *mask, int *out_blocks, int capacity, double *out_var, void *scratch,
-                   SelectState **state_out, cudaStream_t stream)
+                   SelectState **state_out, cudaStream_t stream, int connectivity, SelectState *host_poll)
 {
     static_assert(sizeof(SelectState) <= 256, "SelectState must fit its scratch slot");
     const long long ngrid = (long long)grid.x * grid.y * grid.z;
@@ -493,14 +573,39 @@ int select_enqueue(const float *fixed, Int3 dims, Int3 block, Int3 stride, Int3 
     NRR_LAUNCH(stats, stats_ctas, kStatsThreads, 0, stream, fixed, dims, block, stride, grid, ngrid, frac, mask, var,
                hist, st);
     NRR_LAUNCH_CHECK("stats_kernel");
+    int first_pass = 1;                 // pass 0 is fused into the statistics kernel
+    const unsigned int chunks = (unsigned int)((ngrid + kChunk - 1) / kChunk);
+    if (connectivity != 0) {
+        if (!host_poll) { set_error("connectivity pruning needs a host polling buffer"); return NRR_E_ARG; }
+        const int reach = connectivity == 6 ? 1 : connectivity == 18 ? 2 : 3;
+        unsigned char *state = (unsigned char *)(base + L.prune);
+        const unsigned int pctas = (unsigned int)((ngrid + kPruneThreads - 1) / kPruneThreads);
+        NRR_LAUNCH(prune_init_kernel, pctas, kPruneThreads, 0, stream, var, ngrid, state, st);
+        NRR_LAUNCH_CHECK("prune_init_kernel");
+        for (long long rounds = 0;; rounds += 8) {
+            if (rounds > 4 * ngrid + 64) { set_error("connectivity pruning did not converge"); return NRR_E_CUDA; }
+            for (int r = 0; r < 8; ++r) {
+                NRR_LAUNCH(prune_round_kernel, pctas, kPruneThreads, 0, stream, var, ngrid, grid, reach, state, st);
+                NRR_LAUNCH_CHECK("prune_round_kernel");
+            }
+            NRR_CUDA(cudaMemcpyAsync(host_poll, st, sizeof(SelectState), cudaMemcpyDeviceToHost, stream));
+            NRR_CUDA(cudaStreamSynchronize(stream));
+            if (host_poll->undecided == 0) break;
+        }
+        NRR_LAUNCH(prune_apply_kernel, pctas, kPruneThreads, 0, stream, var, ngrid, state);
+        NRR_LAUNCH_CHECK("prune_apply_kernel");
+        NRR_LAUNCH(prune_finish_kernel, 1, 1, 0, stream, st);
+        NRR_LAUNCH_CHECK("prune_finish_kernel");
+        NRR_CUDA(cudaMemsetAsync(hist, 0, sizeof(unsigned int) * kRadixBins, stream));
+        first_pass = 0;
+    }
     if (!g_select_generic && ngrid <= kSmallLimit) {
         NRR_LAUNCH(select_small_kernel, 1, kSmallThreads, 0, stream, var, ngrid, block, stride, grid, st, out_blocks,
-                   out_var, capacity);
+                   out_var, capacity, first_pass);
         NRR_LAUNCH_CHECK("select_small_kernel");
         return NRR_OK;
     }
-    const unsigned int chunks = (unsigned int)((ngrid + kChunk - 1) / kChunk);
-    for (int pass = 1; pass < kNumPasses; ++pass) {
+    for (int pass = first_pass; pass < kNumPasses; ++pass) {
         NRR_LAUNCH(radix_pass_kernel, chunks, kScanThreads, 0, stream, var, ngrid, hist + (size_t)pass * kRadixBins, st, pass);
         NRR_LAUNCH_CHECK("radix_pass_kernel");
     }

@@ -24,6 +24,7 @@ def lib():
         vp, ci, cd = ctypes.c_void_p, ctypes.c_int, ctypes.c_double
         i3 = ctypes.POINTER(ctypes.c_int)
         L.nrr_bm_select_blocks_host.argtypes = [vp, i3, i3, i3, cd, vp, vp, ci, ctypes.POINTER(ci), vp, ctypes.POINTER(ci)]
+        L.nrr_bm_select_blocks_pruned_host.argtypes = [vp, i3, i3, i3, cd, vp, ci, vp, ci, ctypes.POINTER(ci), vp, ctypes.POINTER(ci)]
         L.nrr_bm_match_host.argtypes = [vp, vp, i3, vp, ci, i3, i3, vp, vp]
         L.nrr_bm_match_info.argtypes = [i3, i3, i3, i3]
         L.nrr_bm_moving_stats_host.argtypes = [vp, i3, i3, vp]
@@ -92,3 +93,16 @@ def register(fixed, moving, block, stride, window, frac, mask=None):
                                       _i3(window), float(frac), None if mask is None else mask.ctypes.data,
                                       blocks.ctypes.data, cap, ctypes.byref(n), disp.ctypes.data, ncc.ctypes.data))
     return blocks[:n.value], disp[:n.value], ncc[:n.value]
+
+
+def select_pruned(fixed, block, stride, frac, mask, connectivity):
+    nz, ny, nx = fixed.shape
+    cap = max(1, int(np.prod([max(0, ((nx, ny, nz)[a] - block[a]) // stride[a] + 1) for a in range(3)])))
+    blocks = np.empty((cap, 3), np.int32)
+    var = np.empty((cap,), np.float64)
+    n, ncand = ctypes.c_int(0), ctypes.c_int(0)
+    _check(lib().nrr_bm_select_blocks_pruned_host(fixed.ctypes.data, _i3((nx, ny, nz)), _i3(block), _i3(stride),
+                                                  float(frac), None if mask is None else mask.ctypes.data,
+                                                  int(connectivity), blocks.ctypes.data, cap, ctypes.byref(n),
+                                                  var.ctypes.data, ctypes.byref(ncand)))
+    return blocks[:n.value], n.value, ncand.value, var[:n.value]

@@ -208,3 +208,31 @@ def test_emulated_pair_kernel_every_candidate_row_can_win(b, r, rz):
     assert np.all(np.abs(ncc - 1.0) < 1e-5)
     om = oracle.match(fixed, moving, centres, block, window)
     assert_match_parity(disp, ncc, om, "planted displacements")
+
+
+@pytest.mark.parametrize("conn", [6, 18, 26])
+@pytest.mark.parametrize("dims,block,stride,frac,mask_r,generic", [
+    ((24, 22, 20), (3, 3, 3), (1, 1, 1), 0.10, None, 0),        # the paper's setting: every voxel a candidate
+    ((24, 22, 20), (3, 3, 3), (1, 1, 1), 0.90, 8.0, 0),         # K above what the pattern leaves: the whole set
+    ((30, 28, 26), (5, 5, 5), (2, 1, 3), 0.30, 11.0, 1),        # anisotropic grid, multi-launch radix select
+])
+def test_emulated_pruned_selection_matches_the_oracle(conn, dims, block, stride, frac, mask_r, generic):
+    """PAPER.md:376 connectivity patterns (reading Q20): the parallel fixed-point rounds against the oracle's
+    sequential greedy walk, bit-exact set, order and variances."""
+    vol = _smooth(dims, 300 + conn)
+    vol[:5] = np.round(vol[:5] / 100.0) * 100.0                  # exact variance ties: the index rule decides
+    mask = None if mask_r is None else spherical_mask(dims, mask_r)
+    ora = oracle.select_pruned(vol, block, stride, frac, mask, conn)
+    _emul.set_option("select_generic", generic)
+    blocks, n, ncand, var = _emul.select_pruned(vol, block, stride, frac, mask, conn)
+    _emul.set_option("select_generic", 0)
+    assert_select_parity(blocks, n, ncand, ora, var)
+
+
+def test_emulated_pruned_selection_uniform_image_closed_form():
+    vol = np.full((9, 9, 9), 5.0, np.float32)
+    blocks, n, ncand, var = _emul.select_pruned(vol, (3, 3, 3), (1, 1, 1), 1.0, None, 6)
+    want = [[i + 1, j + 1, k + 1] for k in range(7) for j in range(7) for i in range(7) if (i + j + k) % 2 == 0]
+    assert ncand == 343 and blocks.tolist() == want
+    blocks, n, ncand, var = _emul.select_pruned(vol, (3, 3, 3), (1, 1, 1), 1.0, None, 0)
+    assert n == 343                                              # no pattern: plain selection

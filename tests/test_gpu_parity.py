@@ -104,6 +104,32 @@ def test_select_parity_configs(name):
     print("%s: N=%d K=%d oracle K/K+1 variance margin %.3g" % (name, ncand, n, ora["margin"]))
 
 
+@pytest.mark.parametrize("conn", [6, 18, 26])
+@pytest.mark.parametrize("dims,block,stride,frac,mask_r", [
+    ((48, 44, 40), (3, 3, 3), (1, 1, 1), 0.05, None),          # the paper's setting: every voxel a candidate
+    ((48, 44, 40), (5, 5, 5), (1, 1, 1), 0.90, 17.0),          # K above what the pattern leaves: the whole set
+    ((64, 60, 33), (5, 5, 5), (2, 1, 3), 0.30, 20.0),
+])
+def test_pruned_selection_parity(conn, dims, block, stride, frac, mask_r):
+    """PAPER.md:376 connectivity patterns (reading Q20): parallel fixed-point rounds vs the oracle's greedy walk."""
+    vol = _smooth(dims, 300 + conn)
+    vol[:5] = np.round(vol[:5] / 100.0) * 100.0                 # exact variance ties: the index rule decides
+    mask = None if mask_r is None else spherical_mask(dims, mask_r)
+    ora = oracle.select_pruned(vol, block, stride, frac, mask, conn)
+    blocks, n, ncand, var = nrr.nrr_bm_select_blocks_pruned(_cuda(vol), block, stride, frac, _cuda(mask), conn, want_var=True)
+    assert_select_parity(blocks.cpu().numpy(), n, ncand, ora, var.cpu().numpy())
+
+
+def test_pruned_selection_dense_grid_multi_launch_path():
+    """More than 2^20 grid positions: the multi-launch radix select after the pruning rounds."""
+    dims = (128, 112, 80)
+    vol = _smooth(dims, 55, sigma=2.0)
+    ora = oracle.select_pruned(vol, (3, 3, 3), (1, 1, 1), 0.04, None, 6)
+    blocks, n, ncand = nrr.nrr_bm_select_blocks_pruned(_cuda(vol), (3, 3, 3), (1, 1, 1), 0.04, None, 6)
+    assert ncand > (1 << 20)
+    assert_select_parity(blocks.cpu().numpy(), n, ncand, ora)
+
+
 # ------------------------------------------------------------------------------------------- matching
 def _match_case(dims, block, window, shift, noise, seed, stride=None, frac=1.0, expect_fast=None):
     vol = _smooth(dims, seed)
