@@ -60,6 +60,23 @@ def valid_candidates(blocks: np.ndarray, cfg) -> np.ndarray:
     return out
 
 
+def rank_config(cfg, rank: int):
+    """Every rank matches its OWN seeded pair (independent units): no data-path collective."""
+    import dataclasses
+    return dataclasses.replace(cfg, seed=cfg.seed + 17 * rank)
+
+
+def reduce_over_ranks(total_ms: float, units: float, world: int, device=None, dist=None):
+    """Whole-job figures: time = MAX over ranks, units = SUM over ranks (the only collectives of the run)."""
+    import torch
+    t = torch.tensor([float(total_ms)], dtype=torch.float64, device=device)
+    u = torch.tensor([float(units)], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
 class ClockSampler(threading.Thread):
     """Samples SM clock and throttle reasons through NVML while the timed region runs."""
 
@@ -186,8 +203,7 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
 
-    import dataclasses
-    cfg = dataclasses.replace(CONFIGS[args.workload], seed=CONFIGS[args.workload].seed + 17 * rank)
+    cfg = rank_config(CONFIGS[args.workload], rank)
     fixed_h, moving_h, mask_h = make_pair(cfg)
     fixed = torch.from_numpy(fixed_h).to(dev)
     moving = torch.from_numpy(moving_h).to(dev)
@@ -244,13 +260,8 @@ def main():
     nrr.nrr_bm_profile_enable(False)
     clocks = sampler.stop()
     total_ms = float(sum(step_ms))
-    t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-    nb = torch.tensor([float(n) * args.steps], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dist.all_reduce(nb, op=dist.ReduceOp.SUM)
-    total_ms_max = float(t.item())
-    value = float(nb.item()) / (total_ms_max * 1e-3)
+    total_ms_max, blocks_all = reduce_over_ranks(total_ms, float(n) * args.steps, world, dev, dist)
+    value = blocks_all / (total_ms_max * 1e-3)
 
     # ---- end-to-end leg: the same step through the host-buffer C-ABI call, copies inside the timed region
     e2e_steps = args.e2e_steps if args.e2e_steps is not None else max(3, min(args.steps, 30))
@@ -271,10 +282,8 @@ def main():
         rb, rd, rs = nrr.nrr_bm_register_host(fixed_p, moving_p, cfg.block, cfg.stride, cfg.window, cfg.frac, mask_p, ob, od, on)
         e2e_t += time.perf_counter() - t0
     barrier()
-    te = torch.tensor([e2e_t], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e_value = float(len(rb)) * e2e_steps * world / float(te.item())
+    e2e_t_max, e2e_blocks = reduce_over_ranks(e2e_t, float(len(rb)) * e2e_steps, world, dev, dist)
+    e2e_value = e2e_blocks / e2e_t_max
     assert np.array_equal(rd.numpy(), disp.cpu().numpy()), "host and device forms disagree"
     h2d = fixed_h.nbytes + moving_h.nbytes + (mask_h.nbytes if mask_h is not None else 0)
     d2h = int(len(rb)) * (12 + 12 + 4) + 4
@@ -341,7 +350,7 @@ def main():
         "roofline": roofline,
         "cpu_baseline": cpu_baseline,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                "steps": e2e_steps, "ms_per_step": 1e3 * float(te.item()) / e2e_steps},
+                "steps": e2e_steps, "ms_per_step": 1e3 * e2e_t_max / e2e_steps},
         "gpu_launches": int(launches),
         "clocks": clocks,
     }

@@ -1,0 +1,52 @@
+"""N > 1 host logic on the CPU (gloo, world_size 2): blocks are independent units, so every
+rank matches its own seeded pair and the only collectives are the MAX over ranks of the time and the SUM of the
+blocks (bench.py).  The per-rank work runs on the emulated library (tests/cuda_emul), not on a GPU."""
+import json
+import os
+import socket
+import sys
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def _worker(rank, world, port, outdir):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    sys.path.insert(0, ROOT)
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    import dataclasses
+    import torch.distributed as dist
+    import bench
+    import _emul
+    from nrr_inputs import CONFIGS, make_pair
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    small = dataclasses.replace(CONFIGS["tiny"], dims=(32, 32, 16))
+    cfg = bench.rank_config(small, rank)
+    fixed, moving, mask = make_pair(cfg)
+    blocks, disp, ncc = _emul.register(fixed, moving, cfg.block, cfg.stride, cfg.window, cfg.frac, mask)
+    my_ms = 10.0 + 5.0 * rank                                   # rank 1 is the slow one
+    t_max, n_all = bench.reduce_over_ranks(my_ms, float(len(blocks)), world, None, dist)
+    with open(os.path.join(outdir, "rank%d.json" % rank), "w") as f:
+        json.dump({"seed": cfg.seed, "n": int(len(blocks)), "t_max": t_max, "n_all": n_all,
+                   "checksum": float(np.asarray(disp, np.int64).sum())}, f)
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_two_ranks_shard_pairs_and_reduce(tmp_path):
+    import torch.multiprocessing as mp
+    port = _free_port()
+    mp.spawn(_worker, args=(2, port, str(tmp_path)), nprocs=2, join=True)
+    r = [json.load(open(tmp_path / ("rank%d.json" % k))) for k in range(2)]
+    assert r[0]["seed"] != r[1]["seed"]                          # independent pairs
+    assert r[0]["t_max"] == r[1]["t_max"] == 15.0                # MAX over ranks
+    assert r[0]["n_all"] == r[1]["n_all"] == r[0]["n"] + r[1]["n"]      # SUM over ranks
+    assert r[0]["n"] > 0 and r[1]["n"] > 0
