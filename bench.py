@@ -37,7 +37,7 @@ SM_COUNT, FP32_LANES, SM_MAX_GHZ = 148, 128, 1.965
 FP32_PEAK_TFLOPS = SM_COUNT * FP32_LANES * 2 * SM_MAX_GHZ / 1e3
 
 
-def parse_args():
+def parse_args(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=200)
@@ -46,7 +46,7 @@ def parse_args():
     ap.add_argument("--workload", default="fullres", choices=sorted(CONFIGS))
     ap.add_argument("--e2e-steps", type=int, default=None, help="steps of the host-buffer (end-to-end) leg")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    return ap.parse_args()
+    return ap.parse_args(argv)
 
 
 def valid_candidates(blocks: np.ndarray, cfg) -> np.ndarray:
@@ -181,8 +181,41 @@ def run_reference(args, rank):
     print(json.dumps(line), flush=True)
 
 
-def main():
-    args = parse_args()
+class CudaBackend:
+    """The real thing: cuda:<local_rank>, the product library, CUDA events.  (tests/test_bench_dryrun.py passes a
+    stand-in with the same five members to run main() end to end on the CPU emulation of the kernels.)"""
+
+    flush_bytes = 256 * 1024 * 1024          # > 126 MB L2
+    collective_backend = "nccl"
+
+    def __init__(self, local_rank: int):
+        import torch
+        import paper_2308_10868_b200 as nrr
+        if not torch.cuda.is_available():
+            raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+        nrr.lib()
+        torch.cuda.set_device(local_rank)
+        self.nrr = nrr
+        self.dev = torch.device("cuda", local_rank)
+
+    def sync(self):
+        import torch
+        torch.cuda.synchronize()
+
+    def event(self):
+        import torch
+        return torch.cuda.Event(enable_timing=True)
+
+    def stream(self):
+        import torch
+        return torch.cuda.current_stream()
+
+    def pin(self, t):
+        return t.pin_memory()
+
+
+def main(argv=None, backend_factory=CudaBackend):
+    args = parse_args(argv)
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -193,23 +226,19 @@ def main():
 
     import torch
     import torch.distributed as dist
-    import paper_2308_10868_b200 as nrr
 
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
-    nrr.lib()
-    torch.cuda.set_device(local_rank)
-    dev = torch.device("cuda", local_rank)
+    be = backend_factory(local_rank)
+    nrr, dev = be.nrr, be.dev
     if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
+        dist.init_process_group(be.collective_backend, device_id=dev if dev.type == "cuda" else None)
 
     cfg = rank_config(CONFIGS[args.workload], rank)
     fixed_h, moving_h, mask_h = make_pair(cfg)
     fixed = torch.from_numpy(fixed_h).to(dev)
     moving = torch.from_numpy(moving_h).to(dev)
     mask = torch.from_numpy(mask_h).to(dev) if mask_h is not None else None
-    flush = torch.empty(256 * 1024 * 1024 // 4, dtype=torch.float32, device=dev)   # 256 MB > 126 MB L2
-    stream = torch.cuda.current_stream()
+    flush = torch.empty(be.flush_bytes // 4, dtype=torch.float32, device=dev)      # 256 MB > 126 MB L2
+    stream = be.stream()
 
     ngrid = 1
     for a in range(3):
@@ -225,10 +254,10 @@ def main():
                             out_blocks=o_blocks, out_n=o_n, out_disp=o_disp, out_ncc=o_ncc)
 
     def barrier():
-        torch.cuda.synchronize()
+        be.sync()
         if world > 1:
             dist.barrier()
-        torch.cuda.synchronize()
+        be.sync()
 
     for _ in range(args.warmup):
         flush.zero_()
@@ -246,7 +275,7 @@ def main():
     nrr.nrr_bm_profile_enable(True)
     nrr.nrr_bm_profile_read()
     nrr.nrr_bm_launch_count(reset=True)
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    ev = [(be.event(), be.event()) for _ in range(args.steps)]
     barrier()
     for i in range(args.steps):
         flush.zero_()
@@ -265,19 +294,19 @@ def main():
 
     # ---- end-to-end leg: the same step through the host-buffer C-ABI call, copies inside the timed region
     e2e_steps = args.e2e_steps if args.e2e_steps is not None else max(3, min(args.steps, 30))
-    fixed_p = torch.from_numpy(fixed_h).pin_memory()
-    moving_p = torch.from_numpy(moving_h).pin_memory()
-    mask_p = torch.from_numpy(mask_h).pin_memory() if mask_h is not None else None
-    ob = torch.empty((cap, 3), dtype=torch.int32).pin_memory()
-    od = torch.empty((cap, 3), dtype=torch.int32).pin_memory()
-    on = torch.empty((cap,), dtype=torch.float32).pin_memory()
+    fixed_p = be.pin(torch.from_numpy(fixed_h))
+    moving_p = be.pin(torch.from_numpy(moving_h))
+    mask_p = be.pin(torch.from_numpy(mask_h)) if mask_h is not None else None
+    ob = be.pin(torch.empty((cap, 3), dtype=torch.int32))
+    od = be.pin(torch.empty((cap, 3), dtype=torch.int32))
+    on = be.pin(torch.empty((cap,), dtype=torch.float32))
     for _ in range(3):
         nrr.nrr_bm_register_host(fixed_p, moving_p, cfg.block, cfg.stride, cfg.window, cfg.frac, mask_p, ob, od, on)
     barrier()
     e2e_t = 0.0
     for _ in range(e2e_steps):
         flush.zero_()
-        torch.cuda.synchronize()
+        be.sync()
         t0 = time.perf_counter()
         rb, rd, rs = nrr.nrr_bm_register_host(fixed_p, moving_p, cfg.block, cfg.stride, cfg.window, cfg.frac, mask_p, ob, od, on)
         e2e_t += time.perf_counter() - t0

@@ -1,0 +1,114 @@
+"""bench.py end to end on the CPU: main() runs unchanged, with a stand-in backend whose `nrr` adapter forwards the
+calls bench.py makes to the emulated library (tests/cuda_emul) and whose events read the host clock.  This checks
+the bench's own logic (step, phases, counting of useful FMAs, e2e leg, JSON contract keys) without a GPU; every
+number it prints is meaningless as a measurement."""
+import io
+import json
+import time
+from contextlib import redirect_stdout
+
+import numpy as np
+import torch
+
+import _emul
+import bench
+
+
+class _Event:
+    def record(self, stream=None):
+        self.t = time.perf_counter()
+
+    def elapsed_time(self, other):
+        return (other.t - self.t) * 1e3
+
+
+class _EmulNrr:
+    """The subset of the binding bench.py uses, on CPU tensors."""
+
+    def __init__(self):
+        self.launches = 0
+
+    def lib(self):
+        return _emul.lib()
+
+    def nrr_bm_register(self, fixed, moving, block, stride, window, frac, mask, capacity, out_blocks, out_n, out_disp, out_ncc):
+        b, d, s = _emul.register(fixed.numpy(), moving.numpy(), block, stride, window, frac, None if mask is None else mask.numpy())
+        n = min(len(b), capacity)
+        out_blocks[:n] = torch.from_numpy(b[:n])
+        out_disp[:n] = torch.from_numpy(d[:n])
+        out_ncc[:n] = torch.from_numpy(s[:n])
+        out_n.fill_(len(b))
+        self.launches += 5
+        return out_blocks, out_n, out_disp, out_ncc
+
+    def nrr_bm_register_host(self, fixed, moving, block, stride, window, frac, mask, out_blocks, out_disp, out_ncc):
+        b, d, s = _emul.register(fixed.numpy(), moving.numpy(), block, stride, window, frac, None if mask is None else mask.numpy())
+        k = len(b)
+        out_blocks[:k] = torch.from_numpy(b)
+        out_disp[:k] = torch.from_numpy(d)
+        out_ncc[:k] = torch.from_numpy(s)
+        return out_blocks[:k], out_disp[:k], out_ncc[:k]
+
+    def nrr_bm_check_async_error(self):
+        pass
+
+    def nrr_bm_profile_enable(self, on):
+        pass
+
+    def nrr_bm_profile_read(self):
+        return {"select_ms": 1.0, "moving_stats_ms": 1.0, "match_ms": 2.0, "prep_ms": 0.5,
+                "select_calls": 1, "moving_stats_calls": 1, "match_calls": 1, "prep_calls": 1}
+
+    def nrr_bm_launch_count(self, reset=False):
+        v, self.launches = self.launches, 0 if reset else self.launches
+        return v
+
+    def nrr_bm_match_info(self, dims, block, window):
+        i = _emul.match_info(dims, block, window)
+        return {"fast": bool(i["kernel"]), "kernel": i["kernel"], "threads": i["threads"], "smem_bytes": i["smem_bytes"],
+                "tma": bool(i["tma"]), "candidates": i["candidates"], "blocks_per_cta": 0}
+
+    def nrr_bm_fp32_peak(self):
+        return 70.0
+
+
+class _Backend:
+    flush_bytes = 1 << 20
+    collective_backend = "gloo"
+
+    def __init__(self, local_rank):
+        self.nrr = _EmulNrr()
+        self.dev = torch.device("cpu")
+
+    def sync(self):
+        pass
+
+    def event(self):
+        return _Event()
+
+    def stream(self):
+        return None
+
+    def pin(self, t):
+        return t
+
+
+def test_bench_main_runs_end_to_end_on_the_emulated_library():
+    out = io.StringIO()
+    with redirect_stdout(out):
+        bench.main(["--workload", "tiny", "--steps", "2", "--warmup", "3", "--e2e-steps", "1", "--no-cpu-baseline"],
+                   backend_factory=_Backend)
+    line = json.loads(out.getvalue().strip().splitlines()[-1])
+    for key in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+                "vs_baseline", "dtype", "data", "config", "roofline", "cpu_baseline", "e2e", "gpu_launches", "clocks"):
+        assert key in line, key
+    assert line["metric"] == "blocks_per_sec" and line["unit"] == "blocks/s" and line["steps"] == 2
+    assert line["config"]["workload"] == "tiny" and line["config"]["blocks_per_pair"] == 259
+    rf = line["roofline"]
+    assert rf["bound"] == "alu" and rf["kernel"] == "match_pair_kernel" and rf["unit"] == "TFLOP/s"
+    # useful FMAs = sum over blocks of valid candidates x block voxels: at most 259 x 343 x 125, and most of it
+    assert 0.7 * 259 * 343 * 125 < rf["useful_fma_per_launch"] <= 259 * 343 * 125
+    assert abs(rf["frac"] - rf["achieved"] / rf["peak"]) < 1e-12
+    e2e = line["e2e"]
+    assert e2e["h2d_bytes_per_step"] == 2 * 64 * 64 * 32 * 4 and e2e["d2h_bytes_per_step"] == 259 * 28 + 4
+    assert line["gpu_launches"] == 10 and line["value"] > 0 and e2e["value"] > 0
