@@ -60,6 +60,8 @@ def _load():
     lib.nrr_oracle_select_pruned.restype = ctypes.c_int
     lib.nrr_oracle_select_pruned.argtypes = [c_flt_p, c_int_p, c_int_p, c_int_p, ctypes.c_double, c_u8_p, ctypes.c_int,
                                              c_int_p, ctypes.c_int, c_int_p, c_dbl_p, c_int_p]
+    lib.nrr_oracle_warp.restype = ctypes.c_int
+    lib.nrr_oracle_warp.argtypes = [c_flt_p, c_int_p, c_flt_p, c_flt_p]
     lib.nrr_oracle_match.restype = ctypes.c_int
     lib.nrr_oracle_match.argtypes = [c_flt_p, c_flt_p, c_int_p, c_int_p, ctypes.c_int, c_int_p, c_int_p,
                                      c_int_p, c_dbl_p, c_dbl_p, c_int_p, ctypes.c_int]
@@ -190,6 +192,21 @@ def match(fixed: np.ndarray, moving: np.ndarray, centres: np.ndarray, block, win
     if rc != 0:
         raise RuntimeError("nrr_oracle_match failed: %d" % rc)
     return {"disp": disp, "ncc": val, "gap": gap, "nvalid": nvalid}
+
+
+def warp(image: np.ndarray, field: np.ndarray) -> np.ndarray:
+    """out(p) = trilinear(image, clamp(p + v(p))); field is float32 [3][nz][ny][nx], components (vx, vy, vz) in voxels
+    (reading Q21)."""
+    image = _f32(image)
+    field = np.ascontiguousarray(field, dtype=np.float32)
+    if field.shape != (3,) + image.shape:
+        raise ValueError("field must be [3][nz][ny][nx]")
+    out = np.empty_like(image)
+    rc = _load().nrr_oracle_warp(_ptr(image, ctypes.c_float), _i3(_dims_of(image)), _ptr(field, ctypes.c_float),
+                                 _ptr(out, ctypes.c_float))
+    if rc != 0:
+        raise RuntimeError("nrr_oracle_warp failed: %d" % rc)
+    return out
 
 
 def ncc_at(fixed: np.ndarray, moving: np.ndarray, centre, block, d) -> float:

@@ -26,6 +26,7 @@
  *   - zero-variance block or candidate => NCC := 0 (Q12)                            PARITY UNPINNED
  *   - output order of the selected set = ascending candidate index (Q8)             PARITY UNPINNED
  *   - the pruning rule behind the paper's connectivity patterns (Q20)               PARITY UNPINNED
+ *   - direction, interpolation and boundary rule of the dense-field warp (Q21)      PARITY UNPINNED
  * Everything else is pinned by tests/test_oracle_*.py (closed forms, numpy.corrcoef, translation
  * recovery, affine invariance, an independent naive evaluator in oracle/naive.py).
  *
@@ -391,6 +392,53 @@ double nrr_oracle_ncc_at(const float *fixed, const float *moving, const int dims
     free(fb);
     return s;
 }
+
+/*
+ * Warp of an image by a dense displacement field (the registration derives a "dense
+ * deformation field that defines transformation for each point in the image space", which is then applied to the
+ * pre-operative image; the APBNRR loop of PAPER.md:286 re-registers the warped image).  The paper gives no
+ * formula; reading Q21, PARITY UNPINNED by the paper: backward warp on the output grid with trilinear
+ * interpolation and edge clamping,
+ *     out(p) = T[image](p + v(p)),   v(p) = (field[0][p], field[1][p], field[2][p])  in voxels, (x, y, z) order,
+ * where the sample position is clamped to [0, n_a - 1] per axis and T interpolates linearly along x, then y,
+ * then z between the two neighbouring voxels.  Arithmetic in double; the result is rounded to float once.
+ */
+int nrr_oracle_warp(const float *image, const int dims[3], const float *field, float *out)
+{
+    for (int a = 0; a < 3; ++a)
+        if (dims[a] < 1) return NRR_ORACLE_E_ARG;
+    const size_t nvox = (size_t)dims[0] * dims[1] * dims[2];
+    for (int z = 0; z < dims[2]; ++z)
+        for (int y = 0; y < dims[1]; ++y)
+            for (int x = 0; x < dims[0]; ++x) {
+                const size_t p = vox(dims, x, y, z);
+                const int pos[3] = { x, y, z };
+                int i0[3], i1[3];
+                double t[3];
+                for (int a = 0; a < 3; ++a) {
+                    double s = (double)pos[a] + (double)field[(size_t)a * nvox + p];
+                    if (s < 0.0) s = 0.0;
+                    if (s > (double)(dims[a] - 1)) s = (double)(dims[a] - 1);
+                    double f = floor(s);
+                    i0[a] = (int)f;
+                    i1[a] = i0[a] + 1 < dims[a] ? i0[a] + 1 : i0[a];
+                    t[a] = s - f;
+                }
+                double c[2][2];
+                for (int kz = 0; kz < 2; ++kz)
+                    for (int ky = 0; ky < 2; ++ky) {
+                        const int zz = kz ? i1[2] : i0[2], yy = ky ? i1[1] : i0[1];
+                        const double a0 = (double)image[vox(dims, i0[0], yy, zz)];
+                        const double a1 = (double)image[vox(dims, i1[0], yy, zz)];
+                        c[kz][ky] = a0 + t[0] * (a1 - a0);
+                    }
+                const double c0 = c[0][0] + t[1] * (c[0][1] - c[0][0]);
+                const double c1 = c[1][0] + t[1] * (c[1][1] - c[1][0]);
+                out[p] = (float)(c0 + t[2] * (c1 - c0));
+            }
+    return NRR_ORACLE_OK;
+}
+
 
 int nrr_oracle_max_threads(void)
 {

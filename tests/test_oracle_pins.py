@@ -434,3 +434,38 @@ def test_select_pruned_isolated_candidates_are_untouched():
     a = oracle.select(vol, (3, 3, 3), (1, 1, 1), 0.5, mask)
     b = oracle.select_pruned(vol, (3, 3, 3), (1, 1, 1), 0.5, mask, 26)
     assert np.array_equal(a["centres"], b["centres"])
+
+
+# ------------------------------------------------------------------------------------ dense-field warp (Q21)
+def test_warp_identity_and_integer_translation_are_exact():
+    rng = np.random.default_rng(5)
+    img = rng.uniform(0, 1000, (9, 10, 11)).astype(np.float32)
+    zero = np.zeros((3,) + img.shape, np.float32)
+    assert np.array_equal(oracle.warp(img, zero), img)
+    f = zero.copy()
+    f[0], f[1], f[2] = 2.0, -1.0, 3.0                             # out(p) = img(clamp(p + (2,-1,3)))
+    nz, ny, nx = img.shape
+    iz = np.clip(np.arange(nz) + 3, 0, nz - 1)
+    iy = np.clip(np.arange(ny) - 1, 0, ny - 1)
+    ix = np.clip(np.arange(nx) + 2, 0, nx - 1)
+    assert np.array_equal(oracle.warp(img, f), img[np.ix_(iz, iy, ix)])
+
+
+def test_warp_reproduces_affine_images_and_matches_scipy():
+    from scipy import ndimage
+    rng = np.random.default_rng(6)
+    nz, ny, nx = 12, 13, 14
+    z, y, x = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    field = rng.uniform(-1.5, 1.5, (3, nz, ny, nx)).astype(np.float32)
+    # trilinear interpolation reproduces affine functions wherever the sample stays inside the volume
+    img = (3.0 * x - 2.0 * y + 0.5 * z + 7.0).astype(np.float32)
+    sx, sy, sz = x + field[0].astype(np.float64), y + field[1].astype(np.float64), z + field[2].astype(np.float64)
+    inside = (sx >= 0) & (sx <= nx - 1) & (sy >= 0) & (sy <= ny - 1) & (sz >= 0) & (sz <= nz - 1)
+    got = oracle.warp(img, field).astype(np.float64)
+    want = 3.0 * sx - 2.0 * sy + 0.5 * sz + 7.0
+    assert np.max(np.abs(got - want)[inside]) < 1e-5
+    # a library routine with the same definition: order-1 spline, coordinates clamped to the edge
+    img2 = rng.uniform(0, 1000, (nz, ny, nx)).astype(np.float32)
+    ref = ndimage.map_coordinates(img2.astype(np.float64), [sz, sy, sx], order=1, mode="nearest")
+    # the oracle rounds its double result to float once: half an ulp at 1000 is 3.1e-5
+    assert np.max(np.abs(oracle.warp(img2, field).astype(np.float64) - ref)) < 1e-4
