@@ -162,6 +162,21 @@ NRR_BM_API int nrr_bm_moving_stats(const float *moving, const int dims[3], const
                         void *stream);
 NRR_BM_API int nrr_bm_moving_stats_host(const float *moving, const int dims[3], const int block[3], float *out_inv_sd);
 
+/*
+ * Warp of an image by a dense displacement field  --  PAPER.md:225-229 (section 3: the registration derives a
+ * "dense deformation field that defines transformation for each point in the image space") and PAPER.md:286
+ * (APBNRR re-registers the warped image in every iteration).  The paper gives no formula; this library reads it
+ * (Q21) as the backward warp on the output grid with trilinear interpolation and edge clamping:
+ *     out(p) = T[image](p + v(p)),   v(p) = (field[0][p], field[1][p], field[2][p]) in voxels, (x, y, z) order,
+ * the sample position clamped to [0, n_a - 1] per axis, T linear along x, then y, then z.
+ *   image [in]  device fp32 [nz][ny][nx]          field [in] device fp32 [3][nz][ny][nx] (component-major)
+ *   out   [out] device fp32 [nz][ny][nx], must not alias image
+ * Asynchronous on `stream`.  fp32 arithmetic: |out - exact| <= 8 * 2^-24 * max|image|.  nrr_bm_warp_host: HOST
+ * buffers, synchronises.
+ */
+NRR_BM_API int nrr_bm_warp(const float *image, const int dims[3], const float *field, float *out, void *stream);
+NRR_BM_API int nrr_bm_warp_host(const float *image, const int dims[3], const float *field, float *out);
+
 /* Synchronises `stream` and returns NRR_E_BOUNDS if any nrr_bm_match enqueued on this thread since the last
  * check saw a block leaving the volume (and clears the flag), NRR_E_CUDA on a CUDA error, else NRR_OK. */
 NRR_BM_API int nrr_bm_check_async_error(void *stream);

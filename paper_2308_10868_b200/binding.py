@@ -20,7 +20,7 @@ NRR_E_NULL, NRR_E_DIMS, NRR_E_BLOCK, NRR_E_STRIDE, NRR_E_WINDOW, NRR_E_FRAC = -1
 NRR_E_CAPACITY, NRR_E_BOUNDS, NRR_E_SMEM, NRR_E_CUDA, NRR_E_ARG = -7, -8, -9, -10, -11
 
 EXPORTS = [
-    "nrr_bm_select_blocks", "nrr_bm_select_blocks_pruned", "nrr_bm_select_blocks_pruned_host", "nrr_bm_match", "nrr_bm_register", "nrr_bm_check_async_error", "nrr_bm_moving_stats", "nrr_bm_moving_stats_host",
+    "nrr_bm_select_blocks", "nrr_bm_select_blocks_pruned", "nrr_bm_select_blocks_pruned_host", "nrr_bm_match", "nrr_bm_register", "nrr_bm_check_async_error", "nrr_bm_moving_stats", "nrr_bm_moving_stats_host", "nrr_bm_warp", "nrr_bm_warp_host",
     "nrr_bm_select_blocks_host", "nrr_bm_match_host", "nrr_bm_register_host",
     "nrr_bm_profile_enable", "nrr_bm_profile_read", "nrr_bm_launch_count", "nrr_bm_match_info",
     "nrr_bm_fp32_peak", "nrr_bm_set_option", "nrr_bm_last_error", "nrr_bm_status_string", "nrr_bm_version",
@@ -57,6 +57,10 @@ def lib() -> ctypes.CDLL:
     L.nrr_bm_select_blocks_pruned_host.argtypes = [vp, i3, i3, i3, cd, vp, ci, vp, ci, ctypes.POINTER(ci), vp, ctypes.POINTER(ci)]
     L.nrr_bm_register.restype = ci
     L.nrr_bm_register.argtypes = [vp, vp, i3, i3, i3, i3, cd, vp, vp, ci, vp, vp, vp, vp]
+    L.nrr_bm_warp.restype = ci
+    L.nrr_bm_warp.argtypes = [vp, i3, vp, vp, vp]
+    L.nrr_bm_warp_host.restype = ci
+    L.nrr_bm_warp_host.argtypes = [vp, i3, vp, vp]
     L.nrr_bm_moving_stats.restype = ci
     L.nrr_bm_moving_stats.argtypes = [vp, i3, i3, vp, vp]
     L.nrr_bm_moving_stats_host.restype = ci
@@ -243,6 +247,21 @@ def nrr_bm_register(fixed, moving, block, stride, window, frac: float, mask=None
                                      int(capacity), out_n.data_ptr(), out_disp.data_ptr(), out_ncc.data_ptr(),
                                      _stream_ptr(stream)))
     return out_blocks, out_n, out_disp, out_ncc
+
+
+def nrr_bm_warp(image, field, out=None, stream=None):
+    """Device form, asynchronous: out(p) = trilinear(image, clamp(p + v(p))); field is CUDA fp32 [3][nz][ny][nx]."""
+    import torch
+    image = _dev(image, torch.float32, "image")
+    field = _dev(field, torch.float32, "field")
+    if tuple(field.shape) != (3,) + tuple(image.shape):
+        raise ValueError("field must be [3][nz][ny][nx]")
+    if out is None:
+        out = torch.empty_like(image)
+    out = _dev(out, torch.float32, "out")
+    with torch.cuda.device(image.device):
+        _check(lib().nrr_bm_warp(image.data_ptr(), _i3(_dims_of(image)), field.data_ptr(), out.data_ptr(), _stream_ptr(stream)))
+    return out
 
 
 def nrr_bm_moving_stats(moving, block, out_inv_sd=None, stream=None):

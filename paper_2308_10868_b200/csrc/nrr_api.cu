@@ -413,6 +413,38 @@ int nrr_bm_register(const float *fixed, const float *moving, const int dims[3], 
                            out_ncc, (cudaStream_t)stream);
 }
 
+int nrr_bm_warp(const float *image, const int dims[3], const float *field, float *out, void *stream)
+{
+    if (!image || !field || !out || !dims) return fail(NRR_E_NULL, "image/dims/field/out is NULL");
+    for (int a = 0; a < 3; ++a)
+        if (dims[a] < 1) return fail(NRR_E_DIMS, "dims[%d] = %d < 1", a, dims[a]);
+    if (image == out) return fail(NRR_E_ARG, "the warp cannot run in place");
+    int rc = ensure_thread_state();
+    if (rc) return rc;
+    return warp_enqueue(image, i3(dims), field, out, (cudaStream_t)stream);
+}
+
+int nrr_bm_warp_host(const float *image, const int dims[3], const float *field, float *out)
+{
+    if (!image || !field || !out || !dims) return fail(NRR_E_NULL, "image/dims/field/out is NULL");
+    for (int a = 0; a < 3; ++a)
+        if (dims[a] < 1) return fail(NRR_E_DIMS, "dims[%d] = %d < 1", a, dims[a]);
+    int rc = ensure_thread_state();
+    if (rc) return rc;
+    cudaStream_t s;
+    if ((rc = host_stream(&s))) return rc;
+    const size_t nvox = (size_t)dims[0] * dims[1] * dims[2];
+    DevBuf d_img(s), d_field(s), d_out(s);
+    NRR_CUDA(d_img.upload(image, nvox * sizeof(float)));
+    NRR_CUDA(d_field.upload(field, 3 * nvox * sizeof(float)));
+    NRR_CUDA(d_out.alloc(nvox * sizeof(float)));
+    rc = warp_enqueue((const float *)d_img.p, i3(dims), (const float *)d_field.p, (float *)d_out.p, s);
+    if (rc) return rc;
+    NRR_CUDA(cudaMemcpyAsync(out, d_out.p, nvox * sizeof(float), cudaMemcpyDeviceToHost, s));
+    NRR_CUDA(cudaStreamSynchronize(s));
+    return NRR_OK;
+}
+
 int nrr_bm_check_async_error(void *stream) { return check_async((cudaStream_t)stream); }
 
 int nrr_bm_select_blocks_host(const float *fixed, const int dims[3], const int block[3], const int stride[3],

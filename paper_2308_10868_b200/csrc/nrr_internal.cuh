@@ -93,6 +93,9 @@ int match_pair_dispatch(const float *fixed, const float *moving, const float *in
                         int n, Int3 block, Int3 window, int *out_disp, float *out_ncc, unsigned int *err_flag,
                         cudaStream_t stream, MatchPlan *plan_only, bool *handled);
 
+// ---- dense-field warp (nrr_warp.cu) -----------------------------------------------------------------
+int warp_enqueue(const float *image, Int3 dims, const float *field, float *out, cudaStream_t stream);
+
 // ---- FFMA microbenchmark (nrr_fma_peak.cu) ----------------------------------------------------------
 int fp32_peak_measure(double *out_tflops, cudaStream_t stream);
 

@@ -25,6 +25,7 @@ def lib():
         i3 = ctypes.POINTER(ctypes.c_int)
         L.nrr_bm_select_blocks_host.argtypes = [vp, i3, i3, i3, cd, vp, vp, ci, ctypes.POINTER(ci), vp, ctypes.POINTER(ci)]
         L.nrr_bm_select_blocks_pruned_host.argtypes = [vp, i3, i3, i3, cd, vp, ci, vp, ci, ctypes.POINTER(ci), vp, ctypes.POINTER(ci)]
+        L.nrr_bm_warp_host.argtypes = [vp, i3, vp, vp]
         L.nrr_bm_match_host.argtypes = [vp, vp, i3, vp, ci, i3, i3, vp, vp]
         L.nrr_bm_match_info.argtypes = [i3, i3, i3, i3]
         L.nrr_bm_moving_stats_host.argtypes = [vp, i3, i3, vp]
@@ -106,3 +107,11 @@ def select_pruned(fixed, block, stride, frac, mask, connectivity):
                                                   int(connectivity), blocks.ctypes.data, cap, ctypes.byref(n),
                                                   var.ctypes.data, ctypes.byref(ncand)))
     return blocks[:n.value], n.value, ncand.value, var[:n.value]
+
+
+def warp(image, field):
+    nz, ny, nx = image.shape
+    field = np.ascontiguousarray(field, np.float32)
+    out = np.empty_like(image)
+    _check(lib().nrr_bm_warp_host(image.ctypes.data, _i3((nx, ny, nz)), field.ctypes.data, out.ctypes.data))
+    return out

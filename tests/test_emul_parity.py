@@ -236,3 +236,22 @@ def test_emulated_pruned_selection_uniform_image_closed_form():
     assert ncand == 343 and blocks.tolist() == want
     blocks, n, ncand, var = _emul.select_pruned(vol, (3, 3, 3), (1, 1, 1), 1.0, None, 0)
     assert n == 343                                              # no pattern: plain selection
+
+
+def _warp_case(dims, amp, seed):
+    rng = np.random.default_rng(seed)
+    nx, ny, nz = dims
+    img = rng.uniform(0, 1000, (nz, ny, nx)).astype(np.float32)
+    field = rng.uniform(-amp, amp, (3, nz, ny, nx)).astype(np.float32)
+    field[:, 0, 0, :4] = [[-1e9, 1e9, 0.0, 2.0]] * 3             # far outside, integers: clamping / exact copies
+    return img, field
+
+
+@pytest.mark.parametrize("dims,amp", [((37, 21, 9), 2.5), ((16, 16, 16), 40.0), ((300, 3, 2), 1.0)])
+def test_emulated_warp_matches_the_oracle(dims, amp):
+    """|gpu - oracle| <= 8 * 2^-24 * max|image| (three fp32 interpolations, tolerances)."""
+    img, field = _warp_case(dims, amp, 90 + dims[0])
+    got, want = _emul.warp(img, field), oracle.warp(img, field)
+    assert np.max(np.abs(got.astype(np.float64) - want)) <= 8 * 2.0 ** -24 * 1000.0
+    zero = np.zeros_like(field)
+    assert np.array_equal(_emul.warp(img, zero), img)              # identity is exact

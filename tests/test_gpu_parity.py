@@ -375,3 +375,18 @@ def test_match_parity_batch_sampled():
         total_exempt += assert_match_parity(rd[:n].cpu().numpy()[idx], rs[:n].cpu().numpy()[idx], ora, label=str(st))
         total_blocks += n
     print("batch: 32 settings, %d blocks, %d exempt blocks among the samples" % (total_blocks, total_exempt))
+
+
+# ------------------------------------------------------------------------------------------- dense-field warp
+@pytest.mark.parametrize("dims,amp", [((37, 21, 9), 2.5), ((64, 60, 33), 40.0), ((256, 256, 124), 8.0)])
+def test_warp_parity(dims, amp):
+    """out(p) = trilinear(image, clamp(p + v(p))) (reading Q21): |gpu - oracle| <= 8 * 2^-24 * max|image|."""
+    rng = np.random.default_rng(90 + dims[0])
+    nx, ny, nz = dims
+    img = rng.uniform(0, 1000, (nz, ny, nx)).astype(np.float32)
+    field = rng.uniform(-amp, amp, (3, nz, ny, nx)).astype(np.float32)
+    field[:, 0, 0, :4] = [[-1e9, 1e9, 0.0, 2.0]] * 3
+    got = nrr.nrr_bm_warp(_cuda(img), _cuda(field)).cpu().numpy()
+    want = oracle.warp(img, field)
+    assert np.max(np.abs(got.astype(np.float64) - want)) <= 8 * 2.0 ** -24 * 1000.0
+    assert torch.equal(nrr.nrr_bm_warp(_cuda(img), torch.zeros_like(_cuda(field))), _cuda(img))
