@@ -217,6 +217,14 @@ NRR_BM_API int nrr_bm_profile_read(double ms[4], int calls[4]);
 NRR_BM_API long long nrr_bm_launch_count(int reset);
 NRR_BM_API int nrr_bm_match_info(const int dims[3], const int block[3], const int window[3], int info[6]);
 NRR_BM_API int nrr_bm_fp32_peak(double *out_tflops, void *stream);
+/*  nrr_bm_pair_task_table: the host-built lane -> task table of the pair matching kernel for a cubic block and a
+ *      window (wx == wy), one word per thread of a CTA: bit 31 = lane has a task, bit 30 = one-row warp,
+ *      bits 16..23 = block of the CTA's group, bits 8..15 = dy index, bits 0..7 = pair index p (rows dz = 2p, 2p+1;
+ *      a one-row task has dz = 2*wz).  info[0] = threads per CTA (= words written), info[1] = blocks per CTA,
+ *      info[2] = staged row pitch (floats), info[3] = staged rows per plane, info[4] = bytes between the unions of
+ *      consecutive blocks in shared memory, info[5] = dynamic shared memory bytes.  No device needed. */
+NRR_BM_API int nrr_bm_pair_task_table(const int block[3], const int window[3], unsigned int *out_table, int capacity,
+                           int info[6]);
 
 /* Tuning / experiment knobs (process-wide; results stay within the documented tolerances):
  *   "tie_band"      FP32 candidates within this NCC distance of the FP32 maximum are re-scored in FP64

@@ -23,7 +23,7 @@ EXPORTS = [
     "nrr_bm_select_blocks", "nrr_bm_select_blocks_pruned", "nrr_bm_select_blocks_pruned_host", "nrr_bm_match", "nrr_bm_register", "nrr_bm_check_async_error", "nrr_bm_moving_stats", "nrr_bm_moving_stats_host", "nrr_bm_warp", "nrr_bm_warp_host",
     "nrr_bm_select_blocks_host", "nrr_bm_match_host", "nrr_bm_register_host",
     "nrr_bm_profile_enable", "nrr_bm_profile_read", "nrr_bm_launch_count", "nrr_bm_match_info",
-    "nrr_bm_fp32_peak", "nrr_bm_set_option", "nrr_bm_last_error", "nrr_bm_status_string", "nrr_bm_version",
+    "nrr_bm_fp32_peak", "nrr_bm_pair_task_table", "nrr_bm_set_option", "nrr_bm_last_error", "nrr_bm_status_string", "nrr_bm_version",
 ]
 
 
@@ -81,6 +81,8 @@ def lib() -> ctypes.CDLL:
     L.nrr_bm_launch_count.argtypes = [ci]
     L.nrr_bm_match_info.restype = ci
     L.nrr_bm_match_info.argtypes = [i3, i3, i3, i3]
+    L.nrr_bm_pair_task_table.restype = ci
+    L.nrr_bm_pair_task_table.argtypes = [i3, i3, vp, ci, ctypes.POINTER(ci)]
     L.nrr_bm_fp32_peak.restype = ci
     L.nrr_bm_fp32_peak.argtypes = [ctypes.POINTER(cd), vp]
     L.nrr_bm_set_option.restype = ci
@@ -360,6 +362,15 @@ def nrr_bm_match_info(dims, block, window):
     _check(lib().nrr_bm_match_info(_i3(dims), _i3(block), _i3(window), info))
     return {"fast": bool(info[0]), "kernel": info[0], "threads": info[1], "smem_bytes": info[2], "tma": bool(info[3]),
             "candidates": info[4], "blocks_per_cta": info[5]}
+
+
+def nrr_bm_pair_task_table(block, window):
+    """Returns (table uint32 [threads], info dict) of the pair kernel's lane -> task assignment. No device needed."""
+    info = (ctypes.c_int * 6)()
+    tab = np.zeros(1024, dtype=np.uint32)
+    _check(lib().nrr_bm_pair_task_table(_i3(block), _i3(window), tab.ctypes.data, tab.size, info))
+    return tab[: info[0]].copy(), {"threads": info[0], "blocks_per_cta": info[1], "pitch": info[2], "rows_per_plane": info[3],
+                                   "union_stride": info[4], "smem_bytes": info[5]}
 
 
 def nrr_bm_fp32_peak(stream=None) -> float:

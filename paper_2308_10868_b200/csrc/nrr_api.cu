@@ -580,6 +580,15 @@ int nrr_bm_match_info(const int dims[3], const int block[3], const int window[3]
     return NRR_OK;
 }
 
+int nrr_bm_pair_task_table(const int block[3], const int window[3], unsigned int *out_table, int capacity, int info[6])
+{
+    if (!block || !window || !info || (capacity > 0 && !out_table)) return fail(NRR_E_NULL, "block/window/info/out_table is NULL");
+    const int n = match_pair_table(i3(block), i3(window), out_table, capacity, info);
+    if (n < 0) return fail(NRR_E_CAPACITY, "the table has %d entries, capacity is %d", -n, capacity);
+    if (n == 0) return fail(NRR_E_ARG, "the pair kernel has no plan for this block / window");
+    return NRR_OK;
+}
+
 int nrr_bm_fp32_peak(double *out_tflops, void *stream)
 {
     if (!out_tflops) return fail(NRR_E_NULL, "out_tflops is NULL");

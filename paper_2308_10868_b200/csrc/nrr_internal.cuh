@@ -93,6 +93,8 @@ int match_pair_dispatch(const float *fixed, const float *moving, const float *in
                         int n, Int3 block, Int3 window, int *out_disp, float *out_ncc, unsigned int *err_flag,
                         cudaStream_t stream, MatchPlan *plan_only, bool *handled);
 
+int match_pair_table(Int3 block, Int3 window, unsigned int *out, int capacity, int info[6]);
+
 // ---- dense-field warp (nrr_warp.cu) -----------------------------------------------------------------
 int warp_enqueue(const float *image, Int3 dims, const float *field, float *out, cudaStream_t stream);
 

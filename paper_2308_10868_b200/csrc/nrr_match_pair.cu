@@ -711,7 +711,35 @@ int launch_pair(const float *fixed, const float *moving, const float *inv_sd, In
     return NRR_OK;
 }
 
+template <int B, int R>
+int table_for(int rz, unsigned int *out, int capacity, int info[6])
+{
+    using C = PairCfg<B, R>;
+    PairGeom g;
+    if (!pair_plan<B, R>(rz, &g)) return 0;
+    info[0] = g.threads; info[1] = g.G; info[2] = C::PITCH; info[3] = C::UX; info[4] = g.union_stride; info[5] = (int)g.smem;
+    if (capacity < g.threads) return -g.threads;
+    const std::vector<uint32_t> tab = build_task_table<B, R>(rz, g);
+    for (int i = 0; i < g.threads; ++i) out[i] = tab[(size_t)i];
+    return g.threads;
+}
+
 }  // namespace
+
+// The lane -> task table of the pair kernel for (block, window): returns the number of words written (threads per
+// CTA), 0 if the pair kernel has no plan for this shape, -needed if `capacity` is too small.
+int match_pair_table(Int3 block, Int3 window, unsigned int *out, int capacity, int info[6])
+{
+    if (!(block.x == block.y && block.y == block.z && window.x == window.y)) return 0;
+#define NRR_PAIR(BB, RR) \
+    if (block.x == BB && window.x == RR) return table_for<BB, RR>(window.z, out, capacity, info);
+    NRR_PAIR(5, 3) NRR_PAIR(5, 5) NRR_PAIR(5, 7) NRR_PAIR(5, 9)
+    NRR_PAIR(7, 3) NRR_PAIR(7, 5) NRR_PAIR(7, 7) NRR_PAIR(7, 9)
+    NRR_PAIR(9, 3) NRR_PAIR(9, 5) NRR_PAIR(9, 7) NRR_PAIR(9, 9)
+    NRR_PAIR(11, 3) NRR_PAIR(11, 5) NRR_PAIR(11, 7) NRR_PAIR(11, 9)
+#undef NRR_PAIR
+    return 0;
+}
 
 // Tries the pair kernel; *handled tells whether it took the call (cubic block 5/7/9/11, in-plane window
 // 3/5/7/9 equal in x and y, TMA-eligible volume).

@@ -1,0 +1,83 @@
+"""Host logic of the pair matching kernel (no GPU): the lane -> task table must give every candidate row of every
+block of a CTA's group to exactly one lane, keep one-row warps and two-row warps apart, spread the work evenly
+over the four warp schedulers of an SM, and keep the LDS.128 row addresses of a quarter-warp on distinct 16-byte
+bank groups where the counts allow it (paper_2308_10868_b200/csrc/nrr_match_pair.cu)."""
+import numpy as np
+import pytest
+
+import paper_2308_10868_b200 as nrr
+
+SHAPES = [(b, r, rz) for b in (5, 7, 9, 11) for r in (3, 5, 7, 9) for rz in (r,)] + [(7, 5, 3), (5, 3, 0), (9, 7, 1)]
+
+
+def _decode(tab):
+    valid = (tab >> 31) & 1
+    single = (tab >> 30) & 1
+    g = (tab >> 16) & 0xFF
+    dy = (tab >> 8) & 0xFF
+    p = tab & 0xFF
+    return valid.astype(bool), single.astype(bool), g.astype(int), dy.astype(int), p.astype(int)
+
+
+@pytest.mark.parametrize("b,r,rz", SHAPES)
+def test_every_candidate_row_has_exactly_one_lane(b, r, rz):
+    tab, info = nrr.nrr_bm_pair_task_table((b, b, b), (r, r, rz))
+    valid, single, g, dy, p = _decode(tab)
+    w, wz = 2 * r + 1, 2 * rz + 1
+    assert info["threads"] == len(tab) and len(tab) % 32 == 0 and len(tab) <= 512
+    assert info["smem_bytes"] <= 227 * 1024
+    rows = []
+    for v, s, gg, d, pp in zip(valid, single, g, dy, p):
+        if not v:
+            continue
+        assert gg < info["blocks_per_cta"] and d < w
+        if s:
+            rows.append((gg, d, wz - 1))
+        else:
+            assert 2 * pp + 1 <= wz - 2 + 1 and 2 * pp + 1 < wz
+            rows += [(gg, d, 2 * pp), (gg, d, 2 * pp + 1)]
+    want = sorted((gg, d, z) for gg in range(info["blocks_per_cta"]) for d in range(w) for z in range(wz))
+    assert sorted(rows) == want                                   # each (block, dy, dz) row once, none missing
+    # the role bit is uniform over a warp (the kernel branches on it per warp)
+    for wi in range(len(tab) // 32):
+        assert len(set(single[wi * 32:(wi + 1) * 32])) == 1
+
+
+@pytest.mark.parametrize("b,r,rz", SHAPES)
+def test_schedulers_are_balanced_and_quarter_warps_mostly_conflict_free(b, r, rz):
+    tab, info = nrr.nrr_bm_pair_task_table((b, b, b), (r, r, rz))
+    valid, single, g, dy, p = _decode(tab)
+    nw = len(tab) // 32
+    wz = 2 * rz + 1
+    load = [0, 0, 0, 0]                                           # warp w issues from scheduler w % 4
+    for wi in range(nw):
+        load[wi % 4] += 1 if single[wi * 32] else 2
+    n_single = sum(1 for wi in range(nw) if single[wi * 32])
+    # no choice of warp slots for the one-row warps gives a smaller maximum (brute force over the slot sets)
+    import itertools
+    best = min(max(sum((1 if wi in sl else 2) for wi in range(nw) if wi % 4 == s) for s in range(4))
+               for sl in map(set, itertools.combinations(range(nw), n_single)))
+    assert max(load) == best
+    # shared-memory wavefronts of one LDS.128 of moving voxels: per quarter-warp, the largest number of lanes whose
+    # row address falls into the same 16-byte bank group (address in 16-byte units: base + P4*dy + PLANE4*dz)
+    p4 = info["pitch"] // 4
+    plane4 = p4 * info["rows_per_plane"]
+    assert p4 % 2 == 1 and (info["union_stride"] // 16) % 8 == 0
+    wavefronts = quarters = 0
+    for q in range(0, len(tab), 8):
+        lanes = [i for i in range(q, q + 8) if valid[i]]
+        if not lanes:
+            continue
+        res = [(p4 * dy[i] + plane4 * ((wz - 1) if single[i] else 2 * p[i])) % 8 for i in lanes]
+        wavefronts += max(np.bincount(res, minlength=8))
+        quarters += 1
+    assert wavefronts <= 1.25 * quarters, (wavefronts, quarters)
+
+
+def test_config3_numbers_quoted_in_design_md():
+    tab, info = nrr.nrr_bm_pair_task_table((7, 7, 7), (5, 5, 5))
+    valid, single, g, dy, p = _decode(tab)
+    assert info["blocks_per_cta"] == 4 and info["threads"] == 288 and info["pitch"] == 20
+    assert 2 * (info["smem_bytes"] + 1024) <= 228 * 1024          # two CTAs per SM
+    assert int(valid.sum()) == 4 * (55 + 11)
+    assert [wi for wi in range(9) if single[wi * 32]] == [0, 4]    # two of scheduler 0's three slots: 4 units each
