@@ -231,7 +231,7 @@ NRR_BM_API int nrr_bm_pair_task_table(const int block[3], const int window[3], u
  *                   (default 1e-4; 0 disables the re-score except for exact FP32 ties)
  *   "force_generic" != 0: always use the generic matching kernel
  *   "force_rows"    != 0: skip the pair kernel (one candidate row per thread instead)
- *   "disable_tma"   != 0: stage shared memory with plain loads instead of TMA (implies no pair kernel)
+ *   "disable_tma"   != 0: stage shared memory with plain loads instead of TMA
  *   "pair_blocks_per_cta"  > 0: blocks per CTA of the pair kernel (0 = the planner's choice)
  *   "boxstat_generic" / "select_generic" != 0: the runtime-shaped moving-statistics / selection kernels */
 NRR_BM_API int nrr_bm_set_option(const char *name, double value);

@@ -326,6 +326,7 @@ struct PairArgs {
     float *out_ncc;
     Int3 dims;
     int n, rz, G, n_pair_warps;
+    int use_tma;                   // 0: the unions are staged with plain loads (volumes TMA cannot address)
     int union_stride;              // bytes between the unions of consecutive blocks of a CTA (multiple of 128)
     float tie_band;
 };
@@ -372,9 +373,9 @@ match_pair_kernel(const __grid_constant__ CUtensorMap tm_moving, const PairArgs 
         const unsigned okmask = __ballot_sync(0xffffffffu, ok);
         __syncwarp();
         if (lane == 0)
-            mbar_arrive_expect_tx(&ctrl->bar, (uint32_t)__popc(okmask) * union_bytes + (uint32_t)gact * C::REC_BYTES);
+            mbar_arrive_expect_tx(&ctrl->bar, (a.use_tma ? (uint32_t)__popc(okmask) * union_bytes : 0u) + (uint32_t)gact * C::REC_BYTES);
         __syncwarp();
-        if (ok) tma_load_3d(s_unions + (size_t)lane * a.union_stride, &tm_moving, (ox - R) & ~3, oy - R, oz - rz, &ctrl->bar);
+        if (ok && a.use_tma) tma_load_3d(s_unions + (size_t)lane * a.union_stride, &tm_moving, (ox - R) & ~3, oy - R, oz - rz, &ctrl->bar);
         if (lane == 0) bulk_load(s_recs, a.records + (size_t)b0 * C::REC_FLOATS, (uint32_t)gact * C::REC_BYTES, &ctrl->bar);
     }
     // this lane's task
@@ -386,9 +387,23 @@ match_pair_kernel(const __grid_constant__ CUtensorMap tm_moving, const PairArgs 
     const int4 org = ctrl->org[g < gact ? g : 0];
     const bool active = (task >> 31) && g < gact && org.w;
 
+    if (!a.use_tma) {      // plain-load staging straight to the final position (no alignment slack to undo)
+        const int per_block = UZ * UX * UX;
+        for (int i = tid; i < gact * per_block; i += blockDim.x) {
+            const int gg = i / per_block, r = i - gg * per_block;
+            const int4 o = ctrl->org[gg];
+            if (!o.w) continue;
+            const int zz = r / (UX * UX), yy = (r / UX) % UX, xx = r % UX;
+            const int gx = o.x - R + xx, gy = o.y - R + yy, gz = o.z - rz + zz;
+            float v = 0.f;
+            if (gx >= 0 && gx < dims.x && gy >= 0 && gy < dims.y && gz >= 0 && gz < dims.z)
+                v = __ldg(a.moving + ((size_t)gz * dims.y + gy) * dims.x + gx);
+            ((float *)(s_unions + (size_t)gg * a.union_stride))[((size_t)zz * UX + yy) * PITCH + xx] = v;
+        }
+    }
     mbar_wait(&ctrl->bar, 0);
     // ---- undo the TMA alignment slack: shift every staged row left by its block's 0..3 floats
-    {
+    if (a.use_tma) {
         const int rows_per_block = UZ * UX;
         for (int r = tid; r < gact * rows_per_block; r += blockDim.x) {
             const int gg = r / rows_per_block, rr = r - gg * rows_per_block;
@@ -666,19 +681,17 @@ int launch_pair(const float *fixed, const float *moving, const float *inv_sd, In
     PairGeom g;
     if (!pair_plan<B, R>(rz, &g)) return NRR_OK;
     if (plan_only) {
-        if (g_disable_tma || dims.x % 4 != 0 || B + 2 * rz > 256) return NRR_OK;      // what the volume shape alone decides
         *handled = true;
         plan_only->fast = 2;
         plan_only->threads = g.threads;
         plan_only->smem_bytes = (int)g.smem;
-        plan_only->tma = 1;
+        plan_only->tma = (g_disable_tma || dims.x % 4 != 0 || B + 2 * rz > 256) ? 0 : 1;      // what the shape alone decides
         plan_only->blocks_per_cta = g.G;
         return NRR_OK;
     }
-    if (!tma_eligible(dims, moving, B + 2 * rz)) return NRR_OK;
     CUtensorMap tm_m;
     memset(&tm_m, 0, sizeof(tm_m));
-    if (!make_volume_map(&tm_m, moving, dims, C::PITCH, C::UX, B + 2 * rz)) return NRR_OK;
+    const int use_tma = tma_eligible(dims, moving, B + 2 * rz) && make_volume_map(&tm_m, moving, dims, C::PITCH, C::UX, B + 2 * rz);
     *handled = true;
     const uint32_t *tab = nullptr;
     int rc = task_table_device<B, R>(rz, g, stream, &tab);
@@ -702,6 +715,7 @@ int launch_pair(const float *fixed, const float *moving, const float *inv_sd, In
     PairArgs a;
     a.fixed = fixed; a.moving = moving; a.inv_sd = inv_sd; a.records = records; a.blocks = blocks; a.task_tab = tab;
     a.out_disp = out_disp; a.out_ncc = out_ncc; a.dims = dims; a.n = n; a.rz = rz; a.G = g.G; a.n_dev = t_match_n_dev;
+    a.use_tma = use_tma;
     a.n_pair_warps = g.n_pair_warps; a.union_stride = g.union_stride; a.tie_band = g_tie_band;
     profile_begin(2, stream);
     NRR_LAUNCH(kern, (n + g.G - 1) / g.G, g.threads, g.smem, stream, tm_m, a);

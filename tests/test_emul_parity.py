@@ -105,6 +105,7 @@ def _grid_blocks(dims, block, stride):
     ((36, 34, 30), 9, 7, 7, (13, 12, 10), 0),     # the config-4 shape
     ((28, 28, 24), 5, 5, 0, (11, 11, 9), 0),      # rz = 0: only the single-row warps work
     ((32, 30, 30), 11, 3, 3, (10, 9, 9), 0),
+    ((29, 27, 25), 5, 3, 3, (6, 7, 8), 0),        # nx not a multiple of 4: TMA cannot address it, plain staging
 ])
 def test_emulated_pair_kernel_matches_the_oracle(dims, b, r, rz, stride, g):
     fixed = _smooth(dims, 7 + b + r)
@@ -116,6 +117,11 @@ def test_emulated_pair_kernel_matches_the_oracle(dims, b, r, rz, stride, g):
     om = oracle.match(fixed, moving, blocks, block, window)
     disp, ncc = _emul.match(fixed, moving, blocks, block, window)
     assert_match_parity(disp, ncc, om, "pair %s" % (dims,))
+    _emul.set_option("disable_tma", 1)                     # plain-load staging must not change a bit
+    assert _emul.match_info(dims, block, window)["kernel"] == 2
+    disp2, ncc2 = _emul.match(fixed, moving, blocks, block, window)
+    _emul.set_option("disable_tma", 0)
+    assert np.array_equal(disp, disp2) and np.array_equal(ncc, ncc2)
     _emul.set_option("force_rows", 1)                      # the one-row-per-thread kernel on the same input
     disp, ncc = _emul.match(fixed, moving, blocks, block, window)
     assert_match_parity(disp, ncc, om, "rows %s" % (dims,))
