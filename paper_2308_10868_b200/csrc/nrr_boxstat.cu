@@ -97,7 +97,7 @@ boxstat_kernel(const float *__restrict__ vol, Int3 dims, Int3 block, float *__re
 
 
 // ------------------------------------------------------------------------------------------ sliding kernel
-// Cubic blocks B in {5,7,9,11}.  One CTA owns a TX x TY tile of ORIGINS and marches over a chunk of z.
+// Blocks B x B x bz with B in {5,7,9,11} (any bz).  One CTA owns a TX x TY tile of ORIGINS and marches over a chunk of z.
 //   z : every thread owns NCOL input columns (x,y) of the haloed tile and keeps, per column, the running FP64
 //       sums of m and m^2 over the last B planes (the plane that leaves the window is read again: an L2 hit);
 //   x : the z-summed plane goes to shared memory; a thread per (row, 8 origins) slides the B-wide window;
@@ -121,7 +121,7 @@ struct SlideCfg {
 
 template <int B>
 __global__ void __launch_bounds__(256, 2)
-boxstat_slide_kernel(const float *__restrict__ vol, Int3 dims, int zchunk, float *__restrict__ inv_sd)
+boxstat_slide_kernel(const float *__restrict__ vol, Int3 dims, int bz, int zchunk, float *__restrict__ inv_sd)
 {
     using C = SlideCfg<B>;
     constexpr int TX = C::TX, TY = C::TY, HX = C::HX, HY = C::HY, NCOL = C::NCOL, ZP = C::ZP, RP = C::RP;
@@ -131,12 +131,12 @@ boxstat_slide_kernel(const float *__restrict__ vol, Int3 dims, int zchunk, float
 
     const int tid = threadIdx.x;
     const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY, z0 = blockIdx.z * zchunk;
-    const int nzo = dims.z - B + 1;
+    const int nzo = dims.z - bz + 1;
     const int zo_end = min(z0 + zchunk, nzo);
     if (z0 >= zo_end) return;                    // uniform over the CTA
-    const int zi_end = zo_end + B - 1;
+    const int zi_end = zo_end + bz - 1;
     const size_t plane = (size_t)dims.x * dims.y;
-    const double nvox = (double)(B * B * B);
+    const double nvox = (double)(B * B * bz);
 
     int gofs[NCOL], sidx[NCOL];                  // global offset inside a plane (-1: outside the volume), s_z slot (-1: none)
 #pragma unroll
@@ -153,13 +153,13 @@ boxstat_slide_kernel(const float *__restrict__ vol, Int3 dims, int zchunk, float
 
     for (int zi = z0; zi < zi_end; ++zi) {
         {
-            const bool emit = zi - z0 >= B - 1;  // uniform: the window is full, plane zo = zi - (B-1) is due
-            const bool drop = zi - z0 >= B;      // uniform: plane zi - B leaves the window (re-read: an L2 hit)
+            const bool emit = zi - z0 >= bz - 1; // uniform: the window is full, plane zo = zi - (bz-1) is due
+            const bool drop = zi - z0 >= bz;     // uniform: plane zi - bz leaves the window (re-read: an L2 hit)
             float vn[NCOL], vl[NCOL];
 #pragma unroll
             for (int c = 0; c < NCOL; ++c) {
                 vn[c] = gofs[c] >= 0 ? __ldg(vol + (size_t)zi * plane + gofs[c]) : 0.f;
-                vl[c] = (drop && gofs[c] >= 0) ? __ldg(vol + (size_t)(zi - B) * plane + gofs[c]) : 0.f;
+                vl[c] = (drop && gofs[c] >= 0) ? __ldg(vol + (size_t)(zi - bz) * plane + gofs[c]) : 0.f;
             }
 #pragma unroll
             for (int c = 0; c < NCOL; ++c) {
@@ -192,7 +192,7 @@ boxstat_slide_kernel(const float *__restrict__ vol, Int3 dims, int zchunk, float
             if (tid < TX * 2) {
                 const int x = tid % TX, ys = (tid / TX) * C::YS;
                 const double2 *col = s_row + (size_t)x * RP + ys;
-                const int gx = x0 + x, zo = zi - (B - 1);
+                const int gx = x0 + x, zo = zi - (bz - 1);
                 const bool x_ok = gx <= dims.x - B;
                 double a = 0.0, b = 0.0;
 #pragma unroll
@@ -220,14 +220,14 @@ boxstat_slide_kernel(const float *__restrict__ vol, Int3 dims, int zchunk, float
 }
 
 template <int B>
-int launch_slide(const float *moving, Int3 dims, float *inv_sd, cudaStream_t stream)
+int launch_slide(const float *moving, Int3 dims, int bz, float *inv_sd, cudaStream_t stream)
 {
     using C = SlideCfg<B>;
-    const int nxo = dims.x - B + 1, nyo = dims.y - B + 1, nzo = dims.z - B + 1;
+    const int nxo = dims.x - B + 1, nyo = dims.y - B + 1, nzo = dims.z - bz + 1;
     const int gx = (nxo + C::TX - 1) / C::TX, gy = (nyo + C::TY - 1) / C::TY;
     // enough CTAs for two per SM; chunks of at least 2B planes keep the z halo below 50 %
     int zsplit = (2 * 148 + gx * gy - 1) / (gx * gy);
-    const int max_split = (nzo + 2 * B - 1) / (2 * B);
+    const int max_split = (nzo + 2 * bz - 1) / (2 * bz);
     if (zsplit > max_split) zsplit = max_split;
     if (zsplit < 1) zsplit = 1;
     const int zchunk = (nzo + zsplit - 1) / zsplit;
@@ -242,7 +242,7 @@ int launch_slide(const float *moving, Int3 dims, float *inv_sd, cudaStream_t str
         NRR_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM));
         configured = true;
     }
-    NRR_LAUNCH(kern, dim3(gx, gy, zsplit), C::NT, C::SMEM, stream, moving, dims, zchunk, inv_sd);
+    NRR_LAUNCH(kern, dim3(gx, gy, zsplit), C::NT, C::SMEM, stream, moving, dims, bz, zchunk, inv_sd);
     NRR_LAUNCH_CHECK("boxstat_slide_kernel");
     return NRR_OK;
 }
@@ -253,12 +253,12 @@ int boxstat_enqueue(const float *moving, Int3 dims, Int3 block, float *inv_sd, c
 {
     const int nxo = dims.x - block.x + 1, nyo = dims.y - block.y + 1, nzo = dims.z - block.z + 1;
     if (nxo < 1 || nyo < 1 || nzo < 1) return NRR_OK;
-    if (!g_boxstat_generic && block.x == block.y && block.y == block.z) {
+    if (!g_boxstat_generic && block.x == block.y) {      // in-plane square, any extent along z
         switch (block.x) {
-        case 5: return launch_slide<5>(moving, dims, inv_sd, stream);
-        case 7: return launch_slide<7>(moving, dims, inv_sd, stream);
-        case 9: return launch_slide<9>(moving, dims, inv_sd, stream);
-        case 11: return launch_slide<11>(moving, dims, inv_sd, stream);
+        case 5: return launch_slide<5>(moving, dims, block.z, inv_sd, stream);
+        case 7: return launch_slide<7>(moving, dims, block.z, inv_sd, stream);
+        case 9: return launch_slide<9>(moving, dims, block.z, inv_sd, stream);
+        case 11: return launch_slide<11>(moving, dims, block.z, inv_sd, stream);
         default: break;
         }
     }

@@ -68,12 +68,13 @@ struct PairCfg {
     static constexpr int NF = FP / 4;
     static constexpr int FPP = (2 * B + 3) / 4 * 4;     // floats per row of the pair table
     static constexpr int NFP = FPP / 4;
-    static constexpr int PLAIN_FLOATS = B * B * FP;
-    static constexpr int PAIR_FLOATS = (B - 1) * B * FPP;
     static constexpr int HDR_FLOATS = 4;                // isd_f, valid, 0, 0
-    static constexpr int REC_FLOATS = PLAIN_FLOATS + PAIR_FLOATS + HDR_FLOATS;
-    static constexpr int REC_BYTES = REC_FLOATS * 4;
-    static_assert(REC_BYTES % 16 == 0, "records are moved by 16-byte bulk copies");
+    // record of one block of B x B x bz voxels (in-plane edge B at compile time, bz at run time)
+    __host__ __device__ static constexpr int plain_floats(int bz) { return bz * B * FP; }
+    __host__ __device__ static constexpr int pair_floats(int bz) { return (bz - 1) * B * FPP; }
+    __host__ __device__ static constexpr int rec_floats(int bz) { return plain_floats(bz) + pair_floats(bz) + HDR_FLOATS; }
+    __host__ __device__ static constexpr int rec_bytes(int bz) { return rec_floats(bz) * 4; }      // multiple of 16
+    static_assert(FP % 4 == 0 && FPP % 4 == 0 && HDR_FLOATS % 4 == 0, "records are moved by 16-byte bulk copies");
     static_assert(PITCH >= NV * 4, "row pitch must cover the vector loads");
 };
 
@@ -148,26 +149,28 @@ __device__ __forceinline__ float unorder_bits(uint32_t k)
 
 // ------------------------------------------------------------------------------------------ prep kernel
 constexpr int kPrepWarps = 4;
+constexpr int kMaxBZ = 11;          // largest block extent along z the pair kernel takes
 
 template <int B, int R>
 __global__ void __launch_bounds__(kPrepWarps * 32)
-prep_kernel(const float *__restrict__ fixed, Int3 dims, const int *__restrict__ blocks, int n,
+prep_kernel(const float *__restrict__ fixed, Int3 dims, const int *__restrict__ blocks, int n, int bz,
             const unsigned int *__restrict__ n_dev, float *__restrict__ records, int *__restrict__ out_disp,
             float *__restrict__ out_ncc, unsigned int *err_flag)
 {
     if (n_dev) n = min(n, (int)*n_dev);               // the launch was sized for an upper bound
     using C = PairCfg<B, R>;
-    constexpr int NVOX = B * B * B;
-    __shared__ float s_f[kPrepWarps][NVOX];
+    const int NVOX = B * B * bz;
+    const int REC_FLOATS = C::rec_floats(bz), PLAIN_FLOATS = C::plain_floats(bz), PAIR_FLOATS = C::pair_floats(bz);
+    __shared__ float s_f[kPrepWarps][B * B * kMaxBZ];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int b = blockIdx.x * kPrepWarps + warp;
     if (b >= n) return;
-    float *rec = records + (size_t)b * C::REC_FLOATS;
-    float *hdr = rec + C::PLAIN_FLOATS + C::PAIR_FLOATS;
+    float *rec = records + (size_t)b * REC_FLOATS;
+    float *hdr = rec + PLAIN_FLOATS + PAIR_FLOATS;
     const int ox = blocks[3 * (size_t)b + 0] - (B - 1) / 2;
     const int oy = blocks[3 * (size_t)b + 1] - (B - 1) / 2;
-    const int oz = blocks[3 * (size_t)b + 2] - (B - 1) / 2;
-    if (!block_in_volume(dims, Int3{B, B, B}, ox, oy, oz)) {      // uniform over the warp
+    const int oz = blocks[3 * (size_t)b + 2] - (bz - 1) / 2;
+    if (!block_in_volume(dims, Int3{B, B, bz}, ox, oy, oz)) {      // uniform over the warp
         if (lane == 0) {
             out_disp[3 * (size_t)b + 0] = 0;
             out_disp[3 * (size_t)b + 1] = 0;
@@ -175,7 +178,7 @@ prep_kernel(const float *__restrict__ fixed, Int3 dims, const int *__restrict__ 
             out_ncc[b] = __int_as_float(0x7fc00000);
             atomicOr(err_flag, 1u);
         }
-        for (int i = lane; i < C::REC_FLOATS; i += 32) rec[i] = 0.f;      // header: isd_f = 0, valid = 0
+        for (int i = lane; i < REC_FLOATS; i += 32) rec[i] = 0.f;      // header: isd_f = 0, valid = 0
         return;
     }
     float *f = s_f[warp];
@@ -196,13 +199,13 @@ prep_kernel(const float *__restrict__ fixed, Int3 dims, const int *__restrict__ 
     const double ssf = warp_sum(q);
     __syncwarp();
     // plain centred block: rows of FP floats, zero padded
-    for (int i = lane; i < C::PLAIN_FLOATS; i += 32) {
+    for (int i = lane; i < PLAIN_FLOATS; i += 32) {
         const int zy = i / C::FP, x = i % C::FP;
         rec[i] = x < B ? f[zy * B + x] : 0.f;
     }
     // pair table: for zr = 1..B-1 and every (vy, vx): (f'[zr][vy][vx], f'[zr-1][vy][vx])
-    float *pt = rec + C::PLAIN_FLOATS;
-    for (int i = lane; i < C::PAIR_FLOATS; i += 32) {
+    float *pt = rec + PLAIN_FLOATS;
+    for (int i = lane; i < PAIR_FLOATS; i += 32) {
         const int row = i / C::FPP, k = i % C::FPP;         // row = (zr-1)*B + vy
         const int zr = row / B + 1, vy = row % B, vx = k >> 1, h = k & 1;
         pt[i] = vx < B ? f[((zr - h) * B + vy) * B + vx] : 0.f;
@@ -229,7 +232,7 @@ __device__ __forceinline__ void load_row(float (&m)[NV * 4], const float *p)
 // Two candidate rows per thread: row A at union plane offset 0, row B one plane further.
 // urow = first moving row of A; rec = this block's record; ra/rb receive the raw numerators.
 template <int B, int R>
-__device__ __forceinline__ void pair_rows(const float *urow, const float *rec, float (&ra)[2 * R + 1], float (&rb)[2 * R + 1])
+__device__ __forceinline__ void pair_rows(const float *urow, const float *rec, int bz, float (&ra)[2 * R + 1], float (&rb)[2 * R + 1])
 {
     using C = PairCfg<B, R>;
     constexpr int W = C::W, PITCH = C::PITCH, PLANE = C::UX * C::PITCH;
@@ -247,10 +250,10 @@ __device__ __forceinline__ void pair_rows(const float *urow, const float *rec, f
 #pragma unroll
             for (int j = 0; j < W; ++j) fma_lo(acc[j], f[vx], m[j + vx]);
     }
-    // planes 1..B-1: both rows, (f'[zr], f'[zr-1]) pairs
-    const float *pt = rec + C::PLAIN_FLOATS;
+    // planes 1..bz-1: both rows, (f'[zr], f'[zr-1]) pairs
+    const float *pt = rec + C::plain_floats(bz);
 #pragma unroll 1
-    for (int zr = 1; zr < B; ++zr) {
+    for (int zr = 1; zr < bz; ++zr) {
         const float *up = urow + zr * PLANE;
         const float *fp = pt + (zr - 1) * B * C::FPP;
 #pragma unroll 1
@@ -269,10 +272,10 @@ __device__ __forceinline__ void pair_rows(const float *urow, const float *rec, f
                 for (int j = 0; j < W; ++j) fma2s(acc[j], m[j + vx], f[vx]);
         }
     }
-    // plane B: row B only, fixed plane B-1
+    // plane bz: row B only, fixed plane bz-1
     {
-        const float *up = urow + B * PLANE;
-        const float *fp = rec + (B - 1) * B * C::FP;
+        const float *up = urow + bz * PLANE;
+        const float *fp = rec + (bz - 1) * B * C::FP;
 #pragma unroll 1
         for (int vy = 0; vy < B; ++vy) {
             float m[C::NV * 4], f[C::FP];
@@ -293,14 +296,14 @@ __device__ __forceinline__ void pair_rows(const float *urow, const float *rec, f
 
 // One candidate row per thread (the odd last plane of candidates).
 template <int B, int R>
-__device__ __forceinline__ void single_row(const float *urow, const float *rec, float (&ra)[2 * R + 1])
+__device__ __forceinline__ void single_row(const float *urow, const float *rec, int bz, float (&ra)[2 * R + 1])
 {
     using C = PairCfg<B, R>;
     constexpr int W = C::W, PITCH = C::PITCH, PLANE = C::UX * C::PITCH;
 #pragma unroll
     for (int j = 0; j < W; ++j) ra[j] = 0.f;
 #pragma unroll 1
-    for (int vz = 0; vz < B; ++vz) {
+    for (int vz = 0; vz < bz; ++vz) {
         const float *up = urow + vz * PLANE;
         const float *fp = rec + vz * B * C::FP;
 #pragma unroll 1
@@ -325,7 +328,7 @@ struct PairArgs {
     int *out_disp;
     float *out_ncc;
     Int3 dims;
-    int n, rz, G, n_pair_warps;
+    int n, rz, bz, G, n_pair_warps;
     int use_tma;                   // 0: the unions are staged with plain loads (volumes TMA cannot address)
     int union_stride;              // bytes between the unions of consecutive blocks of a CTA (multiple of 128)
     float tie_band;
@@ -341,14 +344,15 @@ match_pair_kernel(const __grid_constant__ CUtensorMap tm_moving, const PairArgs 
     unsigned char *s_base = s_raw + ((128u - (smem_u32(s_raw) & 127u)) & 127u);
     unsigned char *s_unions = s_base;
     float *s_recs = (float *)(s_base + (size_t)a.G * a.union_stride);
-    PairCtrl *ctrl = (PairCtrl *)((unsigned char *)s_recs + (size_t)a.G * C::REC_BYTES);
+    const int bz = a.bz, REC_FLOATS = C::rec_floats(bz);
+    PairCtrl *ctrl = (PairCtrl *)((unsigned char *)s_recs + (size_t)a.G * REC_FLOATS * 4);
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int n = a.n_dev ? min(a.n, (int)*a.n_dev) : a.n;
     const int b0 = blockIdx.x * a.G;
     if (b0 >= n) return;                               // uniform: the launch was sized for an upper bound
     const int gact = min(a.G, n - b0);
-    const int rz = a.rz, WZ = 2 * rz + 1, UZ = B + 2 * rz;
+    const int rz = a.rz, WZ = 2 * rz + 1, UZ = bz + 2 * rz;
     const Int3 dims = a.dims;
     const uint32_t union_bytes = (uint32_t)(sizeof(float) * UZ * UX * PITCH);
 
@@ -362,8 +366,8 @@ match_pair_kernel(const __grid_constant__ CUtensorMap tm_moving, const PairArgs 
         if (lane < gact) {
             ox = a.blocks[3 * (size_t)(b0 + lane) + 0] - (B - 1) / 2;
             oy = a.blocks[3 * (size_t)(b0 + lane) + 1] - (B - 1) / 2;
-            oz = a.blocks[3 * (size_t)(b0 + lane) + 2] - (B - 1) / 2;
-            ok = block_in_volume(dims, Int3{B, B, B}, ox, oy, oz) ? 1 : 0;
+            oz = a.blocks[3 * (size_t)(b0 + lane) + 2] - (bz - 1) / 2;
+            ok = block_in_volume(dims, Int3{B, B, bz}, ox, oy, oz) ? 1 : 0;
         }
         if (lane < kGMax) {
             ctrl->org[lane] = make_int4(ox, oy, oz, ok);
@@ -373,10 +377,10 @@ match_pair_kernel(const __grid_constant__ CUtensorMap tm_moving, const PairArgs 
         const unsigned okmask = __ballot_sync(0xffffffffu, ok);
         __syncwarp();
         if (lane == 0)
-            mbar_arrive_expect_tx(&ctrl->bar, (a.use_tma ? (uint32_t)__popc(okmask) * union_bytes : 0u) + (uint32_t)gact * C::REC_BYTES);
+            mbar_arrive_expect_tx(&ctrl->bar, (a.use_tma ? (uint32_t)__popc(okmask) * union_bytes : 0u) + (uint32_t)gact * REC_FLOATS * 4u);
         __syncwarp();
         if (ok && a.use_tma) tma_load_3d(s_unions + (size_t)lane * a.union_stride, &tm_moving, (ox - R) & ~3, oy - R, oz - rz, &ctrl->bar);
-        if (lane == 0) bulk_load(s_recs, a.records + (size_t)b0 * C::REC_FLOATS, (uint32_t)gact * C::REC_BYTES, &ctrl->bar);
+        if (lane == 0) bulk_load(s_recs, a.records + (size_t)b0 * REC_FLOATS, (uint32_t)gact * REC_FLOATS * 4u, &ctrl->bar);
     }
     // this lane's task
     const uint32_t task = a.task_tab[tid];
@@ -421,24 +425,24 @@ match_pair_kernel(const __grid_constant__ CUtensorMap tm_moving, const PairArgs 
     // ---- M3: cross terms
     float ra[W], rb[W];
     const float *urow = (const float *)(s_unions + (size_t)g * a.union_stride) + (size_t)dzA * PLANE + dyi * PITCH;
-    const float *rec = s_recs + (size_t)g * C::REC_FLOATS;
+    const float *rec = s_recs + (size_t)g * REC_FLOATS;
     if (is_pair) {
-        if (active) pair_rows<B, R>(urow, rec, ra, rb);
+        if (active) pair_rows<B, R>(urow, rec, bz, ra, rb);
     } else {
-        if (active) single_row<B, R>(urow, rec, ra);
+        if (active) single_row<B, R>(urow, rec, bz, ra);
     }
 
     // ---- M4: NCC and the per-block arg-max
     float bv = -INFINITY;
     int bi = 0x7fffffff;
     if (active) {
-        const float isd_f = rec[C::PLAIN_FLOATS + C::PAIR_FLOATS];
+        const float isd_f = rec[REC_FLOATS - C::HDR_FLOATS];
         const int py = org.y + dyi - R;
         const bool y_ok = py >= 0 && py + B <= dims.y;
         const int jlo = max(0, R - org.x), jhi = min(W - 1, dims.x - B - org.x + R);      // valid j range
         {
             const int pz = org.z + dzA - rz;
-            const bool row_ok = y_ok && pz >= 0 && pz + B <= dims.z;
+            const bool row_ok = y_ok && pz >= 0 && pz + bz <= dims.z;
             const float *ip = a.inv_sd + ((size_t)pz * dims.y + py) * dims.x + org.x - R;
 #pragma unroll
             for (int j = 0; j < W; ++j) {
@@ -450,7 +454,7 @@ match_pair_kernel(const __grid_constant__ CUtensorMap tm_moving, const PairArgs 
         }
         if (is_pair) {
             const int pz = org.z + dzA + 1 - rz;
-            const bool row_ok = y_ok && pz >= 0 && pz + B <= dims.z;
+            const bool row_ok = y_ok && pz >= 0 && pz + bz <= dims.z;
             const float *ip = a.inv_sd + ((size_t)pz * dims.y + py) * dims.x + org.x - R;
 #pragma unroll
             for (int j = 0; j < W; ++j) {
@@ -497,7 +501,7 @@ match_pair_kernel(const __grid_constant__ CUtensorMap tm_moving, const PairArgs 
     __syncthreads();
 
     // ---- M5: write, with the FP64 photo finish where needed
-    const Int3 block = {B, B, B}, window = {R, R, rz};
+    const Int3 block = {B, B, bz}, window = {R, R, rz};
     for (int gg = 0; gg < gact; ++gg) {
         const int4 o = ctrl->org[gg];
         if (!o.w) continue;                              // flagged by the prep kernel
@@ -529,10 +533,10 @@ struct PairGeom {
 constexpr size_t kMaxSmemPerCta = 227 * 1024, kSmemPerSm = 228 * 1024;
 
 template <int B, int R>
-bool pair_geometry(int rz, int G, PairGeom *out)
+bool pair_geometry(int rz, int bz, int G, PairGeom *out)
 {
     using C = PairCfg<B, R>;
-    const int WZ = 2 * rz + 1, UZ = B + 2 * rz, NP = WZ / 2;
+    const int WZ = 2 * rz + 1, UZ = bz + 2 * rz, NP = WZ / 2;
     PairGeom g;
     g.G = G;
     g.pair_lanes_per_block = (C::W * NP + 7) / 8 * 8;
@@ -541,7 +545,7 @@ bool pair_geometry(int rz, int G, PairGeom *out)
     g.n_single_warps = (G * g.single_lanes_per_block + 31) / 32;
     g.threads = (g.n_pair_warps + g.n_single_warps) * 32;
     g.union_stride = (int)align_up(sizeof(float) * (size_t)UZ * C::UX * C::PITCH, 128);
-    g.smem = (size_t)G * g.union_stride + (size_t)G * C::REC_BYTES + align_up(sizeof(PairCtrl), 16) + 128;
+    g.smem = (size_t)G * g.union_stride + (size_t)G * C::rec_bytes(bz) + align_up(sizeof(PairCtrl), 16) + 128;
     if (g.threads > kPairMaxThreads || g.smem > kMaxSmemPerCta) return false;
     g.efficiency = (double)G * C::W * WZ / 32.0 / (2.0 * g.n_pair_warps + g.n_single_warps);
     const int by_smem = (int)(kSmemPerSm / (g.smem + 1024));
@@ -553,14 +557,14 @@ bool pair_geometry(int rz, int G, PairGeom *out)
 }
 
 template <int B, int R>
-bool pair_plan(int rz, PairGeom *best)
+bool pair_plan(int rz, int bz, PairGeom *best)
 {
     bool found = false;
     double best_score = 0.0;
     for (int G = 1; G <= kGMax; ++G) {
         if (g_pair_g && G != g_pair_g) continue;
         PairGeom g;
-        if (!pair_geometry<B, R>(rz, G, &g)) continue;
+        if (!pair_geometry<B, R>(rz, bz, G, &g)) continue;
         // a lone CTA per SM cannot overlap its staging with another CTA's arithmetic
         const double score = g.efficiency * (g.ctas_per_sm >= 2 ? 1.0 : 0.85);
         if (!found || score > best_score + 1e-9) { found = true; best_score = score; *best = g; }
@@ -656,7 +660,7 @@ int task_table_device(int rz, const PairGeom &g, cudaStream_t stream, const uint
 {
     int dev = 0;
     NRR_CUDA(cudaGetDevice(&dev));
-    const long long key = ((((long long)dev * 32 + B) * 32 + R) * 512 + rz) * 16 + g.G;
+    const long long key = ((((long long)dev * 32 + B) * 32 + R) * 512 + rz) * 16 + g.G;      // the table does not depend on bz
     std::lock_guard<std::mutex> lock(g_tab_mutex);
     auto it = g_tab_cache.find(key);
     if (it != g_tab_cache.end()) { *out = it->second; return NRR_OK; }
@@ -673,34 +677,34 @@ int task_table_device(int rz, const PairGeom &g, cudaStream_t stream, const uint
 
 template <int B, int R>
 int launch_pair(const float *fixed, const float *moving, const float *inv_sd, Int3 dims, const int *blocks, int n,
-                int rz, int *out_disp, float *out_ncc, unsigned int *err_flag, cudaStream_t stream,
+                int rz, int bz, int *out_disp, float *out_ncc, unsigned int *err_flag, cudaStream_t stream,
                 MatchPlan *plan_only, bool *handled)
 {
     using C = PairCfg<B, R>;
     *handled = false;
     PairGeom g;
-    if (!pair_plan<B, R>(rz, &g)) return NRR_OK;
+    if (bz < 1 || bz > kMaxBZ || !pair_plan<B, R>(rz, bz, &g)) return NRR_OK;
     if (plan_only) {
         *handled = true;
         plan_only->fast = 2;
         plan_only->threads = g.threads;
         plan_only->smem_bytes = (int)g.smem;
-        plan_only->tma = (g_disable_tma || dims.x % 4 != 0 || B + 2 * rz > 256) ? 0 : 1;      // what the shape alone decides
+        plan_only->tma = (g_disable_tma || dims.x % 4 != 0 || bz + 2 * rz > 256) ? 0 : 1;      // what the shape alone decides
         plan_only->blocks_per_cta = g.G;
         return NRR_OK;
     }
     CUtensorMap tm_m;
     memset(&tm_m, 0, sizeof(tm_m));
-    const int use_tma = tma_eligible(dims, moving, B + 2 * rz) && make_volume_map(&tm_m, moving, dims, C::PITCH, C::UX, B + 2 * rz);
+    const int use_tma = tma_eligible(dims, moving, bz + 2 * rz) && make_volume_map(&tm_m, moving, dims, C::PITCH, C::UX, bz + 2 * rz);
     *handled = true;
     const uint32_t *tab = nullptr;
     int rc = task_table_device<B, R>(rz, g, stream, &tab);
     if (rc) return rc;
     float *records = nullptr;
-    NRR_CUDA(cudaMallocAsync((void **)&records, (size_t)n * C::REC_BYTES, stream));
+    NRR_CUDA(cudaMallocAsync((void **)&records, (size_t)n * C::rec_bytes(bz), stream));
     auto prep = prep_kernel<B, R>;
     profile_begin(3, stream);
-    NRR_LAUNCH(prep, (n + kPrepWarps - 1) / kPrepWarps, kPrepWarps * 32, 0, stream, fixed, dims, blocks, n,
+    NRR_LAUNCH(prep, (n + kPrepWarps - 1) / kPrepWarps, kPrepWarps * 32, 0, stream, fixed, dims, blocks, n, bz,
                t_match_n_dev, records, out_disp, out_ncc, err_flag);
     profile_end(3, stream);
     NRR_LAUNCH_CHECK("prep_kernel");
@@ -714,7 +718,7 @@ int launch_pair(const float *fixed, const float *moving, const float *inv_sd, In
     }
     PairArgs a;
     a.fixed = fixed; a.moving = moving; a.inv_sd = inv_sd; a.records = records; a.blocks = blocks; a.task_tab = tab;
-    a.out_disp = out_disp; a.out_ncc = out_ncc; a.dims = dims; a.n = n; a.rz = rz; a.G = g.G; a.n_dev = t_match_n_dev;
+    a.out_disp = out_disp; a.out_ncc = out_ncc; a.dims = dims; a.n = n; a.rz = rz; a.bz = bz; a.G = g.G; a.n_dev = t_match_n_dev;
     a.use_tma = use_tma;
     a.n_pair_warps = g.n_pair_warps; a.union_stride = g.union_stride; a.tie_band = g_tie_band;
     profile_begin(2, stream);
@@ -726,11 +730,11 @@ int launch_pair(const float *fixed, const float *moving, const float *inv_sd, In
 }
 
 template <int B, int R>
-int table_for(int rz, unsigned int *out, int capacity, int info[6])
+int table_for(int rz, int bz, unsigned int *out, int capacity, int info[6])
 {
     using C = PairCfg<B, R>;
     PairGeom g;
-    if (!pair_plan<B, R>(rz, &g)) return 0;
+    if (bz < 1 || bz > kMaxBZ || !pair_plan<B, R>(rz, bz, &g)) return 0;
     info[0] = g.threads; info[1] = g.G; info[2] = C::PITCH; info[3] = C::UX; info[4] = g.union_stride; info[5] = (int)g.smem;
     if (capacity < g.threads) return -g.threads;
     const std::vector<uint32_t> tab = build_task_table<B, R>(rz, g);
@@ -744,9 +748,9 @@ int table_for(int rz, unsigned int *out, int capacity, int info[6])
 // CTA), 0 if the pair kernel has no plan for this shape, -needed if `capacity` is too small.
 int match_pair_table(Int3 block, Int3 window, unsigned int *out, int capacity, int info[6])
 {
-    if (!(block.x == block.y && block.y == block.z && window.x == window.y)) return 0;
+    if (!(block.x == block.y && window.x == window.y)) return 0;
 #define NRR_PAIR(BB, RR) \
-    if (block.x == BB && window.x == RR) return table_for<BB, RR>(window.z, out, capacity, info);
+    if (block.x == BB && window.x == RR) return table_for<BB, RR>(window.z, block.z, out, capacity, info);
     NRR_PAIR(5, 3) NRR_PAIR(5, 5) NRR_PAIR(5, 7) NRR_PAIR(5, 9)
     NRR_PAIR(7, 3) NRR_PAIR(7, 5) NRR_PAIR(7, 7) NRR_PAIR(7, 9)
     NRR_PAIR(9, 3) NRR_PAIR(9, 5) NRR_PAIR(9, 7) NRR_PAIR(9, 9)
@@ -755,18 +759,18 @@ int match_pair_table(Int3 block, Int3 window, unsigned int *out, int capacity, i
     return 0;
 }
 
-// Tries the pair kernel; *handled tells whether it took the call (cubic block 5/7/9/11, in-plane window
-// 3/5/7/9 equal in x and y, TMA-eligible volume).
+// Tries the pair kernel; *handled tells whether it took the call (blocks B x B x bz with B in 5/7/9/11 and any odd
+// bz <= 11 -- thick-slice MRI wants e.g. 7 x 7 x 3 --, in-plane window 3/5/7/9 equal in x and y, any window in z).
 int match_pair_dispatch(const float *fixed, const float *moving, const float *inv_sd, Int3 dims, const int *blocks, int n,
                         Int3 block, Int3 window, int *out_disp, float *out_ncc, unsigned int *err_flag,
                         cudaStream_t stream, MatchPlan *plan_only, bool *handled)
 {
     *handled = false;
-    if (!(block.x == block.y && block.y == block.z && window.x == window.y)) return NRR_OK;
+    if (!(block.x == block.y && window.x == window.y)) return NRR_OK;
 #define NRR_PAIR(BB, RR)                                                                                           \
     if (block.x == BB && window.x == RR)                                                                           \
-        return launch_pair<BB, RR>(fixed, moving, inv_sd, dims, blocks, n, window.z, out_disp, out_ncc, err_flag, \
-                                   stream, plan_only, handled);
+        return launch_pair<BB, RR>(fixed, moving, inv_sd, dims, blocks, n, window.z, block.z, out_disp, out_ncc,  \
+                                   err_flag, stream, plan_only, handled);
     NRR_PAIR(5, 3) NRR_PAIR(5, 5) NRR_PAIR(5, 7) NRR_PAIR(5, 9)
     NRR_PAIR(7, 3) NRR_PAIR(7, 5) NRR_PAIR(7, 7) NRR_PAIR(7, 9)
     NRR_PAIR(9, 3) NRR_PAIR(9, 5) NRR_PAIR(9, 7) NRR_PAIR(9, 9)

@@ -106,11 +106,15 @@ def _grid_blocks(dims, block, stride):
     ((28, 28, 24), 5, 5, 0, (11, 11, 9), 0),      # rz = 0: only the single-row warps work
     ((32, 30, 30), 11, 3, 3, (10, 9, 9), 0),
     ((29, 27, 25), 5, 3, 3, (6, 7, 8), 0),        # nx not a multiple of 4: TMA cannot address it, plain staging
+    ((32, 30, 20), (7, 3), 5, 2, (9, 11, 5), 0),  # thick-slice block 7 x 7 x 3
+    ((28, 28, 24), (5, 9), 3, 3, (8, 8, 5), 0),   # block 5 x 5 x 9
+    ((28, 28, 12), (5, 1), 3, 1, (8, 8, 3), 0),   # a single plane: no pair-table planes at all
 ])
 def test_emulated_pair_kernel_matches_the_oracle(dims, b, r, rz, stride, g):
+    b, bz = b if isinstance(b, tuple) else (b, b)
     fixed = _smooth(dims, 7 + b + r)
     moving = _shift_noise(fixed, (1, -2, 1), 8.0, 11)
-    block, window = (b, b, b), (r, r, rz)
+    block, window = (b, b, bz), (r, r, rz)
     blocks = _grid_blocks(dims, block, stride)
     _emul.set_option("pair_blocks_per_cta", g)
     assert _emul.match_info(dims, block, window)["kernel"] == 2
@@ -156,7 +160,8 @@ def test_emulated_degenerate_inputs():
     ((33, 29, 40), (5, 5, 5), 0),
     ((40, 38, 30), (9, 9, 9), 0),
     ((36, 30, 28), (11, 11, 11), 0),
-    ((30, 22, 21), (3, 5, 7), 0),        # non-cubic: generic kernel
+    ((30, 22, 21), (3, 5, 7), 0),        # not square in-plane: generic kernel
+    ((33, 29, 40), (7, 7, 3), 0),        # square in-plane, thin along z: sliding kernel with bz = 3
 ])
 def test_emulated_moving_stats(dims, block, generic):
     """inv_sd[p] = 1/sqrt(SS of the moving block with origin p) against a plain numpy fp64 evaluation."""

@@ -152,7 +152,8 @@ def _match_case(dims, block, window, shift, noise, seed, stride=None, frac=1.0, 
     ((44, 40, 36), (9, 9, 9), (3, 3, 2), True),
     ((40, 40, 40), (11, 11, 11), (3, 3, 3), True),
     ((36, 32, 28), (5, 5, 5), (7, 7, 1), True),
-    ((40, 36, 24), (3, 5, 3), (2, 1, 3), False),     # anisotropic: generic kernel
+    ((40, 36, 24), (3, 5, 3), (2, 1, 3), False),     # not square in-plane: generic kernel
+    ((48, 44, 24), (7, 7, 3), (5, 5, 2), True),      # thick-slice block: pair kernel with a run-time z extent
     ((33, 31, 29), (7, 7, 7), (4, 4, 4), False),     # window without a fast instantiation
     ((30, 30, 30), (5, 5, 5), (0, 0, 0), False),     # single candidate
 ])

@@ -7,7 +7,8 @@ import pytest
 
 import paper_2308_10868_b200 as nrr
 
-SHAPES = [(b, r, rz) for b in (5, 7, 9, 11) for r in (3, 5, 7, 9) for rz in (r,)] + [(7, 5, 3), (5, 3, 0), (9, 7, 1)]
+SHAPES = [(b, r, rz) for b in (5, 7, 9, 11) for r in (3, 5, 7, 9) for rz in (r,)] + [(7, 5, 3), (5, 3, 0), (9, 7, 1),
+                                                                                       ((7, 3), 5, 2), ((11, 1), 9, 9)]
 
 
 def _decode(tab):
@@ -21,7 +22,8 @@ def _decode(tab):
 
 @pytest.mark.parametrize("b,r,rz", SHAPES)
 def test_every_candidate_row_has_exactly_one_lane(b, r, rz):
-    tab, info = nrr.nrr_bm_pair_task_table((b, b, b), (r, r, rz))
+    b, bz = b if isinstance(b, tuple) else (b, b)
+    tab, info = nrr.nrr_bm_pair_task_table((b, b, bz), (r, r, rz))
     valid, single, g, dy, p = _decode(tab)
     w, wz = 2 * r + 1, 2 * rz + 1
     assert info["threads"] == len(tab) and len(tab) % 32 == 0 and len(tab) <= 512
@@ -45,7 +47,8 @@ def test_every_candidate_row_has_exactly_one_lane(b, r, rz):
 
 @pytest.mark.parametrize("b,r,rz", SHAPES)
 def test_schedulers_are_balanced_and_quarter_warps_mostly_conflict_free(b, r, rz):
-    tab, info = nrr.nrr_bm_pair_task_table((b, b, b), (r, r, rz))
+    b, bz = b if isinstance(b, tuple) else (b, b)
+    tab, info = nrr.nrr_bm_pair_task_table((b, b, bz), (r, r, rz))
     valid, single, g, dy, p = _decode(tab)
     nw = len(tab) // 32
     wz = 2 * rz + 1
