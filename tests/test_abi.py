@@ -71,6 +71,21 @@ def test_argument_validation_happens_before_cuda(nrr):
     assert L.nrr_bm_match(p, p, i3(8, 8, 8), p, -1, i3(3, 3, 3), i3(1, 1, 1), p, p, None) == -11
     assert L.nrr_bm_match(p, None, i3(8, 8, 8), p, 1, i3(3, 3, 3), i3(1, 1, 1), p, p, None) == -1
     assert L.nrr_bm_match(p, p, i3(8, 8, 8), None, 1, i3(3, 3, 3), i3(1, 1, 1), p, p, None) == -1
+    # the entry points added in r1c validate the same way
+    assert L.nrr_bm_select_blocks_pruned(p, i3(8, 8, 8), i3(3, 3, 3), i3(1, 1, 1), 0.5, None, 7, p, 4, ctypes.byref(n), None, None, None) == -11
+    assert L.nrr_bm_select_blocks_pruned(p, i3(8, 8, 8), i3(3, 2, 3), i3(1, 1, 1), 0.5, None, 6, p, 4, ctypes.byref(n), None, None, None) == -3
+    assert L.nrr_bm_register(p, p, i3(8, 8, 8), i3(3, 3, 3), i3(1, 1, 1), i3(1, -1, 1), 0.5, None, p, 4, None, p, p, None) == -5
+    assert L.nrr_bm_register(p, None, i3(8, 8, 8), i3(3, 3, 3), i3(1, 1, 1), i3(1, 1, 1), 0.5, None, p, 4, None, p, p, None) == -1
+    assert L.nrr_bm_register(p, p, i3(8, 8, 8), i3(3, 3, 3), i3(1, 1, 1), i3(1, 1, 1), 2.0, None, p, 4, None, p, p, None) == -6
+    assert L.nrr_bm_moving_stats(p, i3(8, 8, 8), i3(3, 4, 3), p, None) == -3
+    assert L.nrr_bm_moving_stats(None, i3(8, 8, 8), i3(3, 3, 3), p, None) == -1
+    assert L.nrr_bm_warp(p, i3(8, 8, 0), p, p, None) == -2
+    assert L.nrr_bm_warp(p, i3(8, 8, 8), p, None, None) == -1
+    q = ctypes.cast((ctypes.c_float * 8)(), ctypes.c_void_p)
+    assert L.nrr_bm_warp(p, i3(2, 2, 2), q, p, None) == -11           # in place
+    info = (ctypes.c_int * 6)()
+    assert L.nrr_bm_pair_task_table(i3(7, 5, 7), i3(5, 5, 5), None, 0, info) == -11      # not square in-plane: no plan
+    assert L.nrr_bm_pair_task_table(i3(7, 7, 7), i3(5, 5, 5), None, 0, info) == -7 and info[0] == 288
     assert nrr.lib().nrr_bm_status_string(-7) == b"NRR_E_CAPACITY"
     assert L.nrr_bm_set_option(b"no_such_option", 1.0) == -11
 
@@ -83,7 +98,10 @@ def test_match_info_dispatch_table(nrr):
             assert info["threads"] % 32 == 0 and 32 <= info["threads"] <= 512
             assert info["smem_bytes"] <= 227 * 1024
     assert nrr.nrr_bm_match_info((256, 256, 60), (7, 7, 7), (5, 5, 3))["fast"]
-    assert not nrr.nrr_bm_match_info((256, 256, 60), (7, 5, 7), (5, 5, 3))["fast"]
+    assert not nrr.nrr_bm_match_info((256, 256, 60), (7, 5, 7), (5, 5, 3))["fast"]       # not square in-plane
+    assert nrr.nrr_bm_match_info((256, 256, 60), (7, 7, 3), (5, 5, 2))["kernel"] == 2     # thick-slice block
+    assert nrr.nrr_bm_match_info((254, 256, 60), (7, 7, 7), (5, 5, 3)) == dict(
+        nrr.nrr_bm_match_info((256, 256, 60), (7, 7, 7), (5, 5, 3)), tma=False)            # plain-load staging
     assert not nrr.nrr_bm_match_info((256, 256, 60), (7, 7, 7), (4, 4, 4))["fast"]
     with pytest.raises(nrr.NrrError):
         nrr.nrr_bm_match_info((256, 256, 60), (7, 7, 7), (5, 5, 300))       # window beyond every kernel's limits
