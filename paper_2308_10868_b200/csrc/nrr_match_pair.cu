@@ -1,4 +1,5 @@
-// nrr_match_pair.cu -- the register-tiled matching kernel for cubic blocks.
+// nrr_match_pair.cu -- the register-tiled matching kernel for blocks B x B x bz, B in {5,7,9,11} at compile time,
+// bz (odd, <= 11) at run time.
 //
 // NCC's numerator over the centred fixed block f' = f - fbar is num(d) = sum_v f'(v) * m(o + d + v)
 // (sum f' = 0, so the moving mean drops out); NCC(d) = num(d) * inv_sd_m(o + d) * inv_sd_f with inv_sd_m
