@@ -579,29 +579,25 @@ bool pair_plan(int rz, int bz, PairGeom *best)
 void place_tasks(std::vector<uint32_t> &tab, int lane0, int lanes, int g, const std::vector<int> &dy,
                  const std::vector<int> &p, const std::vector<int> &residue)
 {
+    // Every residue class hands one task to each quarter-group in index order (so a group never sees a residue
+    // twice and never exceeds eight lanes); what a class has beyond the number of groups is overflow, and all
+    // overflow is packed into the last groups that still have room: the unavoidable two-way conflicts end up in as
+    // few quarter-warps as possible.
     const int ngroups = lanes / 8;
     std::vector<std::vector<int>> grp(ngroups);
-    std::vector<std::vector<int>> by_res(8);
-    for (size_t t = 0; t < dy.size(); ++t) by_res[residue[t]].push_back((int)t);
-    std::vector<int> order = {0, 1, 2, 3, 4, 5, 6, 7};
-    for (int i = 0; i < 8; ++i)
-        for (int j = i + 1; j < 8; ++j)
-            if (by_res[order[j]].size() > by_res[order[i]].size()) { int t = order[i]; order[i] = order[j]; order[j] = t; }
-    for (int oi = 0; oi < 8; ++oi) {
-        const int r = order[oi];
-        for (int t : by_res[r]) {
-            int pick = -1, pick_same = 0;
-            size_t pick_load = 0;
-            for (int k = 0; k < ngroups; ++k) {
-                if (grp[k].size() >= 8) continue;
-                int same = 0;
-                for (int u : grp[k]) same += residue[u] == r;
-                if (pick < 0 || same < pick_same || (same == pick_same && grp[k].size() < pick_load)) {
-                    pick = k; pick_same = same; pick_load = grp[k].size();
-                }
-            }
-            grp[pick].push_back(t);
+    std::vector<int> overflow;
+    for (int r = 0; r < 8; ++r) {
+        int k = 0;
+        for (size_t t = 0; t < dy.size(); ++t) {
+            if (residue[t] != r) continue;
+            if (k < ngroups) grp[k++].push_back((int)t);
+            else overflow.push_back((int)t);
         }
+    }
+    for (int t : overflow) {
+        int k = ngroups - 1;
+        while (k >= 0 && grp[k].size() >= 8) --k;
+        if (k >= 0) grp[k].push_back(t);      // k < 0 cannot happen: the segment holds at least dy.size() lanes
     }
     for (int k = 0; k < ngroups; ++k)
         for (size_t s = 0; s < grp[k].size(); ++s) {
