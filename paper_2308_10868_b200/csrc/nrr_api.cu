@@ -137,17 +137,16 @@ int select_device(const float *fixed, const int dims[3], const int block[3], con
     const Int3 g = grid_of(dims, block, stride);
     const long long ngrid = (long long)g.x * g.y * g.z;
     if (ngrid > 0x7fffffffll) return fail(NRR_E_DIMS, "stride grid has %lld positions (limit 2^31-1)", ngrid);
-    void *scratch = nullptr;
-    NRR_CUDA(cudaMallocAsync(&scratch, select_scratch_bytes(ngrid), stream));
+    AsyncScratch sel_buf(stream);
+    NRR_CUDA(sel_buf.alloc(select_scratch_bytes(ngrid)));
     SelectState *st = nullptr;
     Span span(0, stream);
-    rc = select_enqueue(fixed, i3(dims), i3(block), i3(stride), g, frac, mask, out_blocks, capacity, out_var, scratch,
+    rc = select_enqueue(fixed, i3(dims), i3(block), i3(stride), g, frac, mask, out_blocks, capacity, out_var, sel_buf.p,
                         &st, stream, connectivity, (SelectState *)((char *)t_pinned + 3072));
     span.stop();
-    if (rc) { cudaFreeAsync(scratch, stream); return rc; }
+    if (rc) return rc;
     SelectState *h = (SelectState *)t_pinned;
     NRR_CUDA(cudaMemcpyAsync(h, st, sizeof(SelectState), cudaMemcpyDeviceToHost, stream));
-    NRR_CUDA(cudaFreeAsync(scratch, stream));
     NRR_CUDA(cudaStreamSynchronize(stream));
     *out_n = (int)h->k;
     if (out_ncand) *out_ncand = (int)h->n_candidates;
@@ -166,16 +165,15 @@ int match_device(const float *fixed, const float *moving, const int dims[3], con
     rc = match_plan(i3(dims), i3(block), i3(window), moving, fixed, &plan);
     if (rc) return rc;
     const size_t nvox = (size_t)dims[0] * dims[1] * dims[2];
-    float *inv_sd = nullptr;
-    NRR_CUDA(cudaMallocAsync((void **)&inv_sd, nvox * sizeof(float), stream));
+    AsyncScratch inv_buf(stream);
+    NRR_CUDA(inv_buf.alloc(nvox * sizeof(float)));
+    float *inv_sd = (float *)inv_buf.p;
     Span s1(1, stream);
     rc = boxstat_enqueue(moving, i3(dims), i3(block), inv_sd, stream);
     s1.stop();
     if (rc == NRR_OK)
         rc = match_enqueue(fixed, moving, inv_sd, i3(dims), blocks, n, nullptr, i3(block), i3(window), out_disp, out_ncc,
                            t_err_flag, stream);
-    cudaError_t e = cudaFreeAsync(inv_sd, stream);
-    if (rc == NRR_OK && e != cudaSuccess) return cuda_fail(e, "cudaFreeAsync");
     return rc;
 }
 
@@ -198,11 +196,13 @@ int register_device(const float *fixed, const float *moving, const int dims[3], 
     const int n_cap = (int)(kmax < (double)capacity ? kmax : (double)capacity);
     // The moving-volume statistics do not depend on the selection: fork them onto a side stream so that both
     // (each far from filling the GPU for long) overlap; the matching kernels join.
+    AsyncScratch inv_buf(stream), sel_buf(stream);      // released in stream order on every path out of here
     float *inv_sd = nullptr;
     bool forked = false;
     if (n_cap > 0) {
         const size_t nvox = (size_t)dims[0] * dims[1] * dims[2];
-        NRR_CUDA(cudaMallocAsync((void **)&inv_sd, nvox * sizeof(float), stream));
+        NRR_CUDA(inv_buf.alloc(nvox * sizeof(float)));
+        inv_sd = (float *)inv_buf.p;
         if (!t_side_stream) {
             NRR_CUDA(cudaStreamCreateWithFlags(&t_side_stream, cudaStreamNonBlocking));
             NRR_CUDA(cudaEventCreateWithFlags(&t_ev_fork, cudaEventDisableTiming));
@@ -215,25 +215,28 @@ int register_device(const float *fixed, const float *moving, const int dims[3], 
         s1.stop();
         NRR_CUDA(cudaEventRecord(t_ev_join, t_side_stream));
         forked = true;
-        if (rc) { cudaStreamWaitEvent(stream, t_ev_join, 0); cudaFreeAsync(inv_sd, stream); return rc; }
     }
-    void *scratch = nullptr;
-    NRR_CUDA(cudaMallocAsync(&scratch, select_scratch_bytes(ngrid), stream));
+    // The join (main stream waits for the side stream) is enqueued BEHIND the selection kernels so that the two
+    // overlap, and on every path: the scratch buffers are released in the main stream's order.
+    auto join = [&]() -> int {
+        if (forked && cudaStreamWaitEvent(stream, t_ev_join, 0) != cudaSuccess) return fail(NRR_E_CUDA, "join of the side stream failed");
+        return NRR_OK;
+    };
+    if (rc) { join(); return rc; }
+    if (cudaSuccess != sel_buf.alloc(select_scratch_bytes(ngrid))) { join(); return fail(NRR_E_CUDA, "cudaMallocAsync failed"); }
     SelectState *st = nullptr;
     Span span(0, stream);
-    rc = select_enqueue(fixed, i3(dims), i3(block), i3(stride), g, frac, mask, out_blocks, capacity, nullptr, scratch,
+    rc = select_enqueue(fixed, i3(dims), i3(block), i3(stride), g, frac, mask, out_blocks, capacity, nullptr, sel_buf.p,
                         &st, stream);
     span.stop();
-    if (forked) NRR_CUDA(cudaStreamWaitEvent(stream, t_ev_join, 0));
+    const int jrc = join();
+    if (rc == NRR_OK) rc = jrc;
     if (rc == NRR_OK && out_n_dev)
         rc = cudaMemcpyAsync(out_n_dev, &st->k, sizeof(int), cudaMemcpyDeviceToDevice, stream) == cudaSuccess
                  ? NRR_OK : fail(NRR_E_CUDA, "copy of K failed");
     if (rc == NRR_OK && n_cap > 0)
         rc = match_enqueue(fixed, moving, inv_sd, i3(dims), out_blocks, n_cap, &st->k, i3(block), i3(window),
                            out_disp, out_ncc, t_err_flag, stream);
-    if (inv_sd) cudaFreeAsync(inv_sd, stream);
-    cudaError_t e = cudaFreeAsync(scratch, stream);
-    if (rc == NRR_OK && e != cudaSuccess) return cuda_fail(e, "cudaFreeAsync");
     return rc;
 }
 

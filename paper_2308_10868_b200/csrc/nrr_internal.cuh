@@ -41,6 +41,17 @@ void profile_end(int phase, cudaStream_t stream);
         ::nrr::count_launch();                                        \
     } while (0)
 
+// Stream-ordered scratch released on scope exit, error paths included.
+struct AsyncScratch {
+    void *p = nullptr;
+    cudaStream_t s;
+    explicit AsyncScratch(cudaStream_t st) : s(st) {}
+    AsyncScratch(const AsyncScratch &) = delete;
+    AsyncScratch &operator=(const AsyncScratch &) = delete;
+    ~AsyncScratch() { if (p) cudaFreeAsync(p, s); }
+    cudaError_t alloc(size_t bytes) { return cudaMallocAsync(&p, bytes ? bytes : 1, s); }
+};
+
 // ---- selection (nrr_select.cu) ----------------------------------------------------------------------
 // Device-side state of one selection call; lives in library scratch.
 struct SelectState {

@@ -750,12 +750,14 @@ int launch_pair(const float *fixed, const float *moving, const float *inv_sd, In
     const uint32_t *tab = nullptr;
     int rc = task_table_device<B, R>(rz, g, stream, &tab);
     if (rc) return rc;
-    float *records = nullptr;
-    NRR_CUDA(cudaMallocAsync((void **)&records, (size_t)n * C::rec_bytes(bz), stream));
+    AsyncScratch rec_buf(stream), perm_buf(stream);
+    NRR_CUDA(rec_buf.alloc((size_t)n * C::rec_bytes(bz)));
+    float *records = (float *)rec_buf.p;
     int *perm = nullptr;
     unsigned int *cls_count = nullptr;
     if (g_pair_xoff_classes) {
-        NRR_CUDA(cudaMallocAsync((void **)&perm, sizeof(int) * 4 * (size_t)n + 4 * sizeof(unsigned int), stream));
+        NRR_CUDA(perm_buf.alloc(sizeof(int) * 4 * (size_t)n + 4 * sizeof(unsigned int)));
+        perm = (int *)perm_buf.p;
         cls_count = (unsigned int *)(perm + 4 * (size_t)n);
         NRR_CUDA(cudaMemsetAsync(cls_count, 0, 4 * sizeof(unsigned int), stream));
     }
@@ -783,9 +785,7 @@ int launch_pair(const float *fixed, const float *moving, const float *inv_sd, In
     NRR_LAUNCH(kern, (n + g.G - 1) / g.G + (perm ? 3 : 0), g.threads, g.smem, stream, tm_m, a);
     profile_end(2, stream);
     NRR_LAUNCH_CHECK("match_pair_kernel");
-    NRR_CUDA(cudaFreeAsync(records, stream));
-    if (perm) NRR_CUDA(cudaFreeAsync(perm, stream));
-    return NRR_OK;
+    return NRR_OK;      // the scratch is released behind the kernels, in stream order
 }
 
 template <int B, int R>
