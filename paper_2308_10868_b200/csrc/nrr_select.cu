@@ -373,6 +373,7 @@ compact_kernel(const double *__restrict__ var, long long ngrid, Int3 block, Int3
 // ---- small grids: passes 1..5, the threshold counts and the compaction in ONE single-CTA launch.
 // 60,000 keys (config 3) are 59 keys per thread and pass; seven tiny launches cost more than the work.
 constexpr int kSmallThreads = 1024;
+constexpr int kSmallList = 4096;       // keys (32 KB of shared memory) the single-CTA tail may keep on the side
 constexpr long long kSmallLimit = 1ll << 20;      // grid positions up to which the single-CTA tail is used
 
 __global__ void __launch_bounds__(kSmallThreads)
@@ -382,16 +383,39 @@ select_small_kernel(const double *__restrict__ var, long long ngrid, Int3 block,
 {
     __shared__ unsigned int s_hist[kRadixBins];
     __shared__ unsigned long long s_carry;
+    // Keys that match the prefix decided so far.  A full scan collects them on the side; once they fit, the
+    // remaining passes walk this list instead of the whole grid (after two digits the bucket of the K-th key
+    // usually holds a few dozen keys).  The histograms, hence the selected set, are the same either way.
+    __shared__ unsigned long long s_list[kSmallList];
+    __shared__ unsigned int s_nlist;
     const int tid = threadIdx.x;
+    bool listed = false;                   // uniform: s_list holds exactly the keys matching (prefix, mask)
     for (int pass = first_pass; pass < kNumPasses; ++pass) {
         for (int b = tid; b < kRadixBins; b += kSmallThreads) s_hist[b] = 0;
+        const unsigned int nlist = listed ? s_nlist : 0u;
         __syncthreads();
         const unsigned long long prefix = st->prefix, mask = st->mask;
-        for (long long g = tid; g < ngrid; g += kSmallThreads) {
-            const unsigned long long key = key_of(var[g]);
-            if ((key & mask) == prefix) atomicAdd(&s_hist[digit_of(key, pass)], 1u);
+        if (listed) {
+            for (unsigned int i = tid; i < nlist; i += kSmallThreads) {
+                const unsigned long long key = s_list[i];
+                if ((key & mask) == prefix) atomicAdd(&s_hist[digit_of(key, pass)], 1u);
+            }
+        } else {
+            if (tid == 0) s_nlist = 0u;
+            __syncthreads();
+            for (long long g = tid; g < ngrid; g += kSmallThreads) {
+                const unsigned long long key = key_of(var[g]);
+                if ((key & mask) == prefix) {
+                    atomicAdd(&s_hist[digit_of(key, pass)], 1u);
+                    if (mask != 0ull) {        // with no digit decided yet everything matches: not worth listing
+                        const unsigned int slot = atomicAdd(&s_nlist, 1u);
+                        if (slot < (unsigned int)kSmallList) s_list[slot] = key;
+                    }
+                }
+            }
         }
         __syncthreads();
+        if (!listed && mask != 0ull && s_nlist <= (unsigned int)kSmallList) listed = true;      // same value in every thread
         pick_digit(s_hist, st, pass);      // thread 0 updates *st; the barrier below publishes it to the CTA
         __syncthreads();
     }
