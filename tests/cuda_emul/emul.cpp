@@ -276,7 +276,7 @@ void launch(dim3 grid, dim3 block, size_t smem, const std::function<void()> &bod
                 cta.bar_arrived = cta.bar_count_pred = 0;
                 cta.mbars.clear();
                 // uninitialised shared memory must not look initialised
-                memset(cta.smem_raw, 0xA5, cta.smem_bytes);
+                memset(cta.smem_raw, 0xFF, cta.smem_bytes);      // NaN as float, -1 as int: a use shows up in the results
                 for (WarpState &w : cta.warps) { w.arrived_mask = 0; w.live_mask = 0; }
                 for (int t = 0; t < nthreads; ++t) {
                     Fiber &f = cta.fibers[t];
@@ -333,7 +333,7 @@ cudaError_t cudaMalloc(void **p, size_t bytes)
 {
     *p = nullptr;
     if (posix_memalign(p, 256, bytes ? bytes : 1) != 0) return cudaErrorEmul;      // exact size: overruns are visible to a sanitizer
-    memset(*p, 0xCD, bytes);              // device memory is not zero-initialised
+    memset(*p, 0xFF, bytes);              // device memory is not zero-initialised: NaN as float, -1 as int
     return cudaSuccess;
 }
 cudaError_t cudaFree(void *p) { free(p); return cudaSuccess; }
