@@ -264,6 +264,18 @@ void launch(dim3 grid, dim3 block, size_t smem, const std::function<void()> &bod
     cta.smem_bytes = 128 + smem + 16;
     cta.smem_aligned = raw + 128 + 16;
     for (Fiber &f : cta.fibers) f.stack.resize(kStack);
+    // scheduling order of the runnable threads inside a CTA (default: ascending thread index)
+    int sched_mode = 0;
+    unsigned long long rng = 0x9E3779B97F4A7C15ull;
+    if (const char *e = getenv("NRR_EMUL_SCHED")) {
+        if (!strcmp(e, "reverse")) sched_mode = 1;
+        else if (!strncmp(e, "random", 6)) { sched_mode = 2; if (e[6] == ':') rng ^= strtoull(e + 7, nullptr, 10); }
+    }
+    std::vector<int> order;
+    if (sched_mode) {
+        order.resize((size_t)nthreads);
+        for (int i = 0; i < nthreads; ++i) order[(size_t)i] = sched_mode == 1 ? nthreads - 1 - i : i;
+    }
     g_blockDim = block;
     g_gridDim = grid;
     Cta *prev = g_cta;
@@ -295,7 +307,16 @@ void launch(dim3 grid, dim3 block, size_t smem, const std::function<void()> &bod
                 int idle_passes = 0;
                 while (cta.live > 0) {
                     const unsigned long long before = cta.progress;
-                    for (int t = 0; t < nthreads; ++t) {
+                    if (sched_mode == 2) {
+                        for (int i = nthreads - 1; i > 0; --i) {
+                            rng = rng * 6364136223846793005ull + 1442695040888963407ull;
+                            std::swap(order[(size_t)i], order[(size_t)((rng >> 33) % (unsigned long long)(i + 1))]);
+                        }
+                    }
+                    for (int tt = 0; tt < nthreads; ++tt) {
+                        // NRR_EMUL_SCHED=reverse|random: another order in which runnable threads take their turns; a
+                        // result that depends on it is a missing barrier (a race) in the kernel
+                        const int t = order.empty() ? tt : order[(size_t)tt];
                         Fiber &f = cta.fibers[t];
                         if (f.done) continue;
                         cta.cur = &f;
