@@ -3,7 +3,8 @@
 // A kernel launch runs its CTAs one after another on the calling OS thread.  Inside a CTA every CUDA thread is
 // a ucontext fiber; fibers run round-robin and switch only inside the emulated collectives (__syncthreads, warp
 // shuffles/votes/reductions, mbarrier waits), so shared-memory atomics are plain operations.  A full pass over
-// the fibers without any progress is reported as a deadlock.  TMA copies are performed at issue time; the
+// the fibers without any progress is reported as a deadlock.  TMA copies are performed when a thread first waits on
+// their mbarrier (until then the destination holds the 0xFF fill, as an unwaited-for read would see garbage); the
 // hardware rules this project measured on B200 are asserted (16-byte aligned inner start coordinate and box
 // row, 128-byte aligned shared destination, 16-byte granularity of bulk copies).
 #include <stdio.h>
@@ -46,7 +47,9 @@ struct WarpState {
     unsigned live_mask = 0;      // lanes that exist and have not exited
 };
 
-struct MBar { long long pending; long long tx_expected, tx_done; unsigned phase; };
+// Copies are asynchronous on the hardware: the emulation performs them only when a thread first WAITS on their
+// barrier, so a kernel that touches the destination without waiting reads the 0xFF fill, not the data.
+struct MBar { long long pending; long long tx_expected, tx_done; unsigned phase; std::vector<std::function<void()>> copies; };
 
 struct Cta {
     std::vector<Fiber> fibers;
@@ -188,7 +191,7 @@ void syncwarp(unsigned mask)
 }
 
 // ---- mbarrier / TMA
-void mbar_init(void *bar, unsigned count) { g_cta->mbars[bar] = MBar{(long long)count, 0, 0, 0}; g_cta->progress++; }
+void mbar_init(void *bar, unsigned count) { g_cta->mbars[bar] = MBar{(long long)count, 0, 0, 0, {}}; g_cta->progress++; }
 
 static MBar &mbar_of(void *bar)
 {
@@ -209,6 +212,11 @@ bool mbar_try_wait(void *bar, unsigned parity)
 {
     MBar &m = mbar_of(bar);
     if (parity != 0) trap("the emulation models single-phase mbarriers only");
+    if (!m.copies.empty()) {
+        for (auto &c : m.copies) c();
+        m.copies.clear();
+        g_cta->progress++;
+    }
     if (m.pending < 0 || m.tx_done > m.tx_expected) trap("mbarrier over-arrived / more bytes than expected");
     if (m.pending == 0 && m.tx_done == m.tx_expected) return true;
     yield();
@@ -221,28 +229,33 @@ void tma_load_3d(void *dst, const void *map_, int x, int y, int z, void *bar)
     if (map->rank != 3) trap("tensor map of rank != 3");
     if ((x & 3) != 0) trap("TMA inner start coordinate not a multiple of 16 bytes (faults on B200)");
     if (((uintptr_t)dst & 127) != 0) trap("TMA shared destination not 128-byte aligned");
-    float *d = (float *)dst;
-    const long long nx = (long long)map->dim[0], ny = (long long)map->dim[1], nz = (long long)map->dim[2];
-    for (unsigned c = 0; c < map->box[2]; ++c)
-        for (unsigned b = 0; b < map->box[1]; ++b)
-            for (unsigned a = 0; a < map->box[0]; ++a) {
-                const long long gx = (long long)x + a, gy = (long long)y + b, gz = (long long)z + c;
-                float v = 0.f;
-                if (gx >= 0 && gx < nx && gy >= 0 && gy < ny && gz >= 0 && gz < nz)
-                    v = *(const float *)((const char *)map->base + gz * map->stride_bytes[1] + gy * map->stride_bytes[0] + gx * 4);
-                *d++ = v;
-            }
+    const CUtensorMap mp = *map;
     MBar &m = mbar_of(bar);
-    m.tx_done += (long long)map->box[0] * map->box[1] * map->box[2] * 4;
+    m.copies.push_back([mp, dst, x, y, z, &m]() {
+        float *d = (float *)dst;
+        const long long nx = (long long)mp.dim[0], ny = (long long)mp.dim[1], nz = (long long)mp.dim[2];
+        for (unsigned c = 0; c < mp.box[2]; ++c)
+            for (unsigned b = 0; b < mp.box[1]; ++b)
+                for (unsigned a = 0; a < mp.box[0]; ++a) {
+                    const long long gx = (long long)x + a, gy = (long long)y + b, gz = (long long)z + c;
+                    float v = 0.f;
+                    if (gx >= 0 && gx < nx && gy >= 0 && gy < ny && gz >= 0 && gz < nz)
+                        v = *(const float *)((const char *)mp.base + gz * mp.stride_bytes[1] + gy * mp.stride_bytes[0] + gx * 4);
+                    *d++ = v;
+                }
+        m.tx_done += (long long)mp.box[0] * mp.box[1] * mp.box[2] * 4;
+    });
     g_cta->progress++;
 }
 
 void bulk_load(void *dst, const void *src, unsigned bytes, void *bar)
 {
     if ((bytes & 15) || ((uintptr_t)dst & 15) || ((uintptr_t)src & 15)) trap("bulk copy not 16-byte aligned / sized");
-    memcpy(dst, src, bytes);
     MBar &m = mbar_of(bar);
-    m.tx_done += bytes;
+    m.copies.push_back([dst, src, bytes, &m]() {
+        memcpy(dst, src, bytes);
+        m.tx_done += bytes;
+    });
     g_cta->progress++;
 }
 
