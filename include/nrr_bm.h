@@ -54,7 +54,10 @@ typedef enum nrr_status {
                             synchronising host entry points and by nrr_bm_check_async_error) */
     NRR_E_SMEM = -9,     /* block / window too large for the kernels' shared-memory or index limits */
     NRR_E_CUDA = -10,    /* a CUDA runtime call failed (message in nrr_bm_last_error) */
-    NRR_E_ARG = -11      /* other invalid argument (n < 0, capacity < 0, ...) */
+    NRR_E_ARG = -11,     /* other invalid argument (n < 0, capacity < 0, ...) */
+    NRR_E_DEVICE = -12   /* a staged copy of a matching kernel did not complete within its time bound; the blocks
+                            of that CTA get out_disp = (0,0,0), out_ncc = NaN.  Reported like NRR_E_BOUNDS (sticky
+                            device flag); the kernel leaves in an orderly way and never faults the GPU */
 } nrr_status;
 
 /*
@@ -177,8 +180,9 @@ NRR_BM_API int nrr_bm_moving_stats_host(const float *moving, const int dims[3], 
 NRR_BM_API int nrr_bm_warp(const float *image, const int dims[3], const float *field, float *out, void *stream);
 NRR_BM_API int nrr_bm_warp_host(const float *image, const int dims[3], const float *field, float *out);
 
-/* Synchronises `stream` and returns NRR_E_BOUNDS if any nrr_bm_match enqueued on this thread since the last
- * check saw a block leaving the volume (and clears the flag), NRR_E_CUDA on a CUDA error, else NRR_OK. */
+/* Synchronises `stream` and returns NRR_E_DEVICE if a staged copy of a matching kernel enqueued on this thread since
+ * the last check did not complete, NRR_E_BOUNDS if one saw a block leaving the volume (and clears the flag),
+ * NRR_E_CUDA on a CUDA error, else NRR_OK. */
 NRR_BM_API int nrr_bm_check_async_error(void *stream);
 
 /*

@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libnrr_bm.so")
 
 NRR_OK = 0
 NRR_E_NULL, NRR_E_DIMS, NRR_E_BLOCK, NRR_E_STRIDE, NRR_E_WINDOW, NRR_E_FRAC = -1, -2, -3, -4, -5, -6
-NRR_E_CAPACITY, NRR_E_BOUNDS, NRR_E_SMEM, NRR_E_CUDA, NRR_E_ARG = -7, -8, -9, -10, -11
+NRR_E_CAPACITY, NRR_E_BOUNDS, NRR_E_SMEM, NRR_E_CUDA, NRR_E_ARG, NRR_E_DEVICE = -7, -8, -9, -10, -11, -12
 
 EXPORTS = [
     "nrr_bm_select_blocks", "nrr_bm_select_blocks_pruned", "nrr_bm_select_blocks_pruned_host", "nrr_bm_match", "nrr_bm_register", "nrr_bm_check_async_error", "nrr_bm_moving_stats", "nrr_bm_moving_stats_host", "nrr_bm_warp", "nrr_bm_warp_host",

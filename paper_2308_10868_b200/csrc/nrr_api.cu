@@ -6,6 +6,7 @@
 #include <stdio.h>
 #include <string.h>
 
+#include <mutex>
 #include <vector>
 
 #include "nrr_internal.cuh"
@@ -18,6 +19,7 @@ extern int g_disable_tma;
 extern int g_force_rows;
 extern int g_pair_g;
 extern int g_pair_xoff_classes;
+extern int g_debug_tx_extra;
 extern int g_boxstat_generic;
 extern int g_select_generic;
 
@@ -30,26 +32,29 @@ thread_local int t_profile = 0;
 struct TimedSpan { int phase; cudaEvent_t e0, e1; };
 thread_local std::vector<TimedSpan> *t_spans = nullptr;
 
-thread_local unsigned int *t_err_flag = nullptr;      // device, sticky "a block left the volume"
-thread_local void *t_pinned = nullptr;                // small pinned staging buffer
-thread_local cudaStream_t t_host_stream = nullptr;    // stream of the *_host entry points
-thread_local bool t_pool_configured = false;
-thread_local cudaStream_t t_side_stream = nullptr;    // nrr_bm_register: moving statistics run beside the selection
-thread_local cudaEvent_t t_ev_fork = nullptr, t_ev_join = nullptr;
+// Per-thread, per-device state: a second GPU in the same process gets its own flag, streams and events.
+struct DevState {
+    unsigned int *err_flag = nullptr;      // device, sticky error bits (kErrBounds | kErrStaging of the kernels)
+    cudaStream_t host_stream = nullptr;    // stream of the *_host entry points
+    cudaStream_t side_stream = nullptr;    // nrr_bm_register: moving statistics run beside the selection
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+};
+thread_local DevState t_dev[kMaxDevices];
+thread_local void *t_pinned = nullptr;     // small pinned staging buffer (host memory: one per thread)
+DevState &ds() { return t_dev[current_device()]; }
+#define t_err_flag (ds().err_flag)
+#define t_host_stream (ds().host_stream)
+#define t_side_stream (ds().side_stream)
+#define t_ev_fork (ds().ev_fork)
+#define t_ev_join (ds().ev_join)
 
 constexpr size_t kPinnedBytes = 4096;
 
+std::mutex g_pool_mutex;
+cudaMemPool_t g_pools[kMaxDevices] = {};
+
 int ensure_thread_state()
 {
-    if (!t_pool_configured) {
-        int dev = 0;
-        NRR_CUDA(cudaGetDevice(&dev));
-        cudaMemPool_t pool;
-        NRR_CUDA(cudaDeviceGetDefaultMemPool(&pool, dev));
-        unsigned long long keep = ~0ull;      // keep freed scratch cached in the pool: reuse without re-mapping
-        NRR_CUDA(cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep));
-        t_pool_configured = true;
-    }
     if (!t_err_flag) {
         NRR_CUDA(cudaMalloc((void **)&t_err_flag, sizeof(unsigned int)));
         NRR_CUDA(cudaMemset(t_err_flag, 0, sizeof(unsigned int)));
@@ -248,7 +253,8 @@ int check_async(cudaStream_t stream)
     NRR_CUDA(cudaMemcpyAsync(h, t_err_flag, sizeof(unsigned int), cudaMemcpyDeviceToHost, stream));
     NRR_CUDA(cudaMemsetAsync(t_err_flag, 0, sizeof(unsigned int), stream));
     NRR_CUDA(cudaStreamSynchronize(stream));
-    if (*h) return fail(NRR_E_BOUNDS, "a supplied block leaves the volume");
+    if (*h & 2u) return fail(NRR_E_DEVICE, "a staged copy (TMA / bulk) of a matching kernel did not complete");
+    if (*h & 1u) return fail(NRR_E_BOUNDS, "a supplied block leaves the volume");
     return NRR_OK;
 }
 
@@ -264,7 +270,7 @@ struct DevBuf {     // stream-ordered device buffer released on scope exit
     cudaStream_t s;
     explicit DevBuf(cudaStream_t st) : s(st) {}
     ~DevBuf() { if (p) cudaFreeAsync(p, s); }
-    cudaError_t alloc(size_t bytes) { return cudaMallocAsync(&p, bytes ? bytes : 1, s); }
+    cudaError_t alloc(size_t bytes) { return scratch_alloc(&p, bytes, s); }
     cudaError_t upload(const void *h, size_t bytes)
     {
         cudaError_t e = alloc(bytes);
@@ -274,6 +280,35 @@ struct DevBuf {     // stream-ordered device buffer released on scope exit
 };
 
 }  // namespace
+
+// Library scratch comes from a PRIVATE stream-ordered pool per device (the process-wide default pool is left as the
+// application configured it); freed scratch stays cached in it, so steady-state calls re-map nothing.
+cudaMemPool_t scratch_pool()
+{
+    const int dev = current_device();
+    std::lock_guard<std::mutex> lock(g_pool_mutex);
+    if (!g_pools[dev]) {
+        cudaMemPoolProps props;
+        memset(&props, 0, sizeof(props));
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        cudaMemPool_t pool = nullptr;
+        if (cudaMemPoolCreate(&pool, &props) != cudaSuccess) { (void)cudaGetLastError(); return nullptr; }
+        unsigned long long keep = ~0ull;
+        (void)cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+        g_pools[dev] = pool;
+    }
+    return g_pools[dev];
+}
+
+cudaError_t scratch_alloc(void **p, size_t bytes, cudaStream_t s)
+{
+    cudaMemPool_t pool = scratch_pool();
+    if (!pool) return cudaMallocAsync(p, bytes ? bytes : 1, s);
+    return cudaMallocFromPoolAsync(p, bytes ? bytes : 1, pool, s);
+}
 
 void set_error(const char *fmt, ...)
 {
@@ -610,6 +645,7 @@ int nrr_bm_set_option(const char *name, double value)
     if (!strcmp(name, "force_rows")) { g_force_rows = value != 0.0; return NRR_OK; }
     if (!strcmp(name, "pair_xoff_classes")) { g_pair_xoff_classes = value != 0.0; return NRR_OK; }
     if (!strcmp(name, "pair_blocks_per_cta")) { g_pair_g = (int)value; return NRR_OK; }
+    if (!strcmp(name, "debug_expect_tx_extra")) { g_debug_tx_extra = (int)value & ~15; return NRR_OK; }
     return fail(NRR_E_ARG, "unknown option '%s'", name);
 }
 
@@ -630,6 +666,7 @@ const char *nrr_bm_status_string(int status)
     case NRR_E_SMEM: return "NRR_E_SMEM";
     case NRR_E_CUDA: return "NRR_E_CUDA";
     case NRR_E_ARG: return "NRR_E_ARG";
+    case NRR_E_DEVICE: return "NRR_E_DEVICE";
     default: return "NRR_E_UNKNOWN";
     }
 }

@@ -237,10 +237,11 @@ int launch_slide(const float *moving, Int3 dims, int bz, float *inv_sd, cudaStre
         return NRR_E_DIMS;
     }
     auto kern = boxstat_slide_kernel<B>;
-    static bool configured = false;
-    if (!configured) {
+    static bool configured[kMaxDevices] = {};     // per instantiation and device
+    bool &conf = configured[current_device()];
+    if (!conf) {
         NRR_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM));
-        configured = true;
+        conf = true;
     }
     NRR_LAUNCH(kern, dim3(gx, gy, zsplit), C::NT, C::SMEM, stream, moving, dims, bz, zchunk, inv_sd);
     NRR_LAUNCH_CHECK("boxstat_slide_kernel");

@@ -41,6 +41,18 @@ void profile_end(int phase, cudaStream_t stream);
         ::nrr::count_launch();                                        \
     } while (0)
 
+// Per-device caches (function attributes, streams, flags) are indexed by the current device ordinal.
+constexpr int kMaxDevices = 64;
+inline int current_device()
+{
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) dev = 0;
+    return dev;
+}
+
+// Library scratch: a private stream-ordered memory pool per device (nrr_api.cu).
+cudaError_t scratch_alloc(void **p, size_t bytes, cudaStream_t s);
+
 // Stream-ordered scratch released on scope exit, error paths included.
 struct AsyncScratch {
     void *p = nullptr;
@@ -49,7 +61,7 @@ struct AsyncScratch {
     AsyncScratch(const AsyncScratch &) = delete;
     AsyncScratch &operator=(const AsyncScratch &) = delete;
     ~AsyncScratch() { if (p) cudaFreeAsync(p, s); }
-    cudaError_t alloc(size_t bytes) { return cudaMallocAsync(&p, bytes ? bytes : 1, s); }
+    cudaError_t alloc(size_t bytes) { return scratch_alloc(&p, bytes, s); }
 };
 
 // ---- selection (nrr_select.cu) ----------------------------------------------------------------------

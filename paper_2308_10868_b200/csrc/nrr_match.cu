@@ -61,6 +61,7 @@ struct FastSmem {      // tail of the dynamic shared memory, after the union and
     int am_i[32];
     TieScratch ts;
     float isd_f;
+    int stage_failed;
 };
 
 
@@ -120,6 +121,7 @@ __global__ void __launch_bounds__(kFastMaxThreads) match_rows_kernel(const __gri
     const int xoff = x0 - x0a;                // 0..3 floats of slack at the start of every staged row
     if (use_tma) {
         if (tid == 0) {
+            sm->stage_failed = 0;
             mbar_init(&sm->bar_union, 1);
             mbar_fence_init();
             mbar_arrive_expect_tx(&sm->bar_union, (uint32_t)(sizeof(float) * (size_t)UZ * PROWS * PITCH));
@@ -178,7 +180,7 @@ __global__ void __launch_bounds__(kFastMaxThreads) match_rows_kernel(const __gri
     }
 
     if (use_tma) {
-        mbar_wait(&sm->bar_union, 0);
+        if (!mbar_wait(&sm->bar_union, 0)) sm->stage_failed = 1;
         if (xoff != 0) {                      // uniform over the CTA
             const int nstaged = UZ * C::UX;   // rows that are read later: (z, y < UX)
             for (int r = tid; r < nstaged; r += blockDim.x) {
@@ -189,6 +191,10 @@ __global__ void __launch_bounds__(kFastMaxThreads) match_rows_kernel(const __gri
             }
         }
         __syncthreads();
+        if (sm->stage_failed) {      // uniform: the copy did not land in time -- report, never fault (NRR_E_DEVICE)
+            write_error_result(b, out_disp, out_ncc, err_flag, kErrStaging);
+            return;
+        }
     }
 
     // ---- M3: cross terms
@@ -403,10 +409,11 @@ int launch_fast(const float *fixed, const float *moving, const float *inv_sd, In
     int use_tma = 0;
     if (tma && make_volume_map(&tm_m, moving, dims, C::PITCH, C::PROWS, B + 2 * rz)) use_tma = 1;
     auto kern = match_rows_kernel<B, R>;
-    static int configured_smem = 0;     // per instantiation
-    if ((int)smem > configured_smem) {
+    static int configured_smem[kMaxDevices] = {};     // per instantiation and device
+    int &conf = configured_smem[current_device()];
+    if ((int)smem > conf) {
         NRR_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        configured_smem = (int)smem;
+        conf = (int)smem;
     }
     profile_begin(2, stream);
     NRR_LAUNCH(kern, n, threads, smem, stream, tm_m, use_tma, fixed, moving, inv_sd, dims, blocks, rz, g_tie_band,
@@ -482,10 +489,11 @@ int dispatch(const float *fixed, const float *moving, const float *inv_sd, Int3 
         plan_only->tma = 0;
         return NRR_OK;
     }
-    static int configured_smem = 48 * 1024;
-    if ((int)smem > configured_smem) {
+    static int configured_smem[kMaxDevices] = {};     // per device (0: the 48 KB default)
+    int &conf = configured_smem[current_device()];
+    if ((int)smem > 48 * 1024 && (int)smem > conf) {
         NRR_CUDA(cudaFuncSetAttribute(match_generic_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        configured_smem = (int)smem;
+        conf = (int)smem;
     }
     profile_begin(2, stream);
     NRR_LAUNCH(match_generic_kernel, n, 128, smem, stream, fixed, moving, inv_sd, dims, blocks, block, window,

@@ -21,9 +21,12 @@ __device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count) { emul:
 __device__ __forceinline__ void mbar_fence_init() {}
 __device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t *bar, uint32_t bytes) { emul::mbar_arrive_expect_tx(bar, bytes); }
 __device__ __forceinline__ bool mbar_try_wait(uint64_t *bar, uint32_t parity) { return emul::mbar_try_wait(bar, parity); }
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+__device__ __forceinline__ bool mbar_wait(uint64_t *bar, uint32_t parity)
 {
-    while (!mbar_try_wait(bar, parity)) {}
+    for (int spin = 0; spin < 3; ++spin)
+        if (mbar_try_wait(bar, parity)) return true;
+    emul::mbar_timeout();
+    return false;
 }
 __device__ __forceinline__ void tma_load_3d(void *dst, const CUtensorMap *map, int x, int y, int z, uint64_t *bar)
 {
@@ -53,11 +56,24 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t *bar, uint32_t parity)
         : "memory");
     return ok != 0;
 }
-// Bounded wait: a mis-programmed copy must abort the kernel, never hang the GPU.
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+__device__ __forceinline__ uint64_t global_timer_ns()
 {
-    for (uint32_t spin = 0; !mbar_try_wait(bar, parity); ++spin)
-        if (spin > (1u << 24)) __trap();
+    uint64_t t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+// Bounded wait: a mis-programmed copy must neither hang the GPU nor fault it.  Returns false when the barrier has
+// not completed after kMbarTimeoutNs of wall time (bounded by time, not by polls: time-slicing, a debugger or a long
+// TMA queue must not fire it on a healthy copy); the caller then reports NRR_E_DEVICE through the sticky error
+// flag and leaves the kernel in an orderly way -- no __trap(), no Xid.
+constexpr uint64_t kMbarTimeoutNs = 4000000000ull;
+__device__ __forceinline__ bool mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    if (mbar_try_wait(bar, parity)) return true;
+    const uint64_t t0 = global_timer_ns();
+    while (!mbar_try_wait(bar, parity))
+        if (global_timer_ns() - t0 > kMbarTimeoutNs) return false;
+    return true;
 }
 __device__ __forceinline__ void tma_load_3d(void *dst, const CUtensorMap *map, int x, int y, int z, uint64_t *bar)
 {
@@ -194,15 +210,23 @@ __device__ __forceinline__ bool block_in_volume(Int3 dims, Int3 block, int ox, i
     return ox >= 0 && oy >= 0 && oz >= 0 && ox + block.x <= dims.x && oy + block.y <= dims.y && oz + block.z <= dims.z;
 }
 
-__device__ void write_bounds_error(int b, int *out_disp, float *out_ncc, unsigned int *err_flag)
+// Sticky device-side error flag bits (read and cleared by nrr_bm_check_async_error)
+constexpr unsigned int kErrBounds = 1u;      // a supplied block leaves the volume       -> NRR_E_BOUNDS
+constexpr unsigned int kErrStaging = 2u;     // a staged (TMA / bulk) copy did not land  -> NRR_E_DEVICE
+
+__device__ void write_error_result(int b, int *out_disp, float *out_ncc, unsigned int *err_flag, unsigned int bit)
 {
     if (threadIdx.x == 0) {
         out_disp[3 * (size_t)b + 0] = 0;
         out_disp[3 * (size_t)b + 1] = 0;
         out_disp[3 * (size_t)b + 2] = 0;
         out_ncc[b] = __int_as_float(0x7fc00000);
-        atomicOr(err_flag, 1u);
+        atomicOr(err_flag, bit);
     }
+}
+__device__ __forceinline__ void write_bounds_error(int b, int *out_disp, float *out_ncc, unsigned int *err_flag)
+{
+    write_error_result(b, out_disp, out_ncc, err_flag, kErrBounds);
 }
 
 // row[k] = row[k + S] for k < UX, in place, one thread per row: whole row to registers, then vector stores.

@@ -52,6 +52,7 @@ extern float g_tie_band;
 extern int g_disable_tma;
 int g_pair_xoff_classes = 0;   // experiment knob: CTAs of equal TMA alignment slack, no row shift (see PairArgs)
 int g_pair_g = 0;             // experiment knob: force the number of blocks per CTA (0 = planner's choice)
+int g_debug_tx_extra = 0;     // test hook: over-programs the staging barrier so that its wait must time out
 
 namespace {
 
@@ -86,6 +87,7 @@ struct PairCtrl {              // tail of the dynamic shared memory
     u64 best[kGMax];           // (ordered NCC bits << 32) | ~index
     int4 org[kGMax];           // block origin (x, y, z), w = 1 if the block is inside the volume
     int count[kGMax];          // near ties besides the FP32 best
+    int stage_failed;          // a thread's bounded wait for the staged copies gave up
     TieScratch ts;
 };
 
@@ -352,6 +354,8 @@ struct PairArgs {
     int n_cap;
     int union_stride;              // bytes between the unions of consecutive blocks of a CTA (multiple of 128)
     float tie_band;
+    unsigned int *err_flag;        // sticky device flag (kErrStaging when the staged copies do not land)
+    unsigned int debug_tx_extra;   // test hook (option "debug_expect_tx_extra"): bytes added to the expected copy size
 };
 
 template <int B, int R>
@@ -397,6 +401,7 @@ match_pair_kernel(const __grid_constant__ CUtensorMap tm_moving, const PairArgs 
     // ---- M1: stage. Warp 0: lane g owns block b0 + g.
     if (warp == 0) {
         if (lane == 0) {
+            ctrl->stage_failed = 0;
             mbar_init(&ctrl->bar, 1);
             mbar_fence_init();
         }
@@ -417,7 +422,7 @@ match_pair_kernel(const __grid_constant__ CUtensorMap tm_moving, const PairArgs 
         const unsigned okmask = __ballot_sync(0xffffffffu, ok);
         __syncwarp();
         if (lane == 0)
-            mbar_arrive_expect_tx(&ctrl->bar, (a.use_tma ? (uint32_t)__popc(okmask) * union_bytes : 0u) + (uint32_t)gact * REC_FLOATS * 4u);
+            mbar_arrive_expect_tx(&ctrl->bar, (a.use_tma ? (uint32_t)__popc(okmask) * union_bytes : 0u) + (uint32_t)gact * REC_FLOATS * 4u + a.debug_tx_extra);
         __syncwarp();
         if (ok && a.use_tma) tma_load_3d(s_unions + (size_t)lane * a.union_stride, &tm_moving, (ox - R) & ~3, oy - R, oz - rz, &ctrl->bar);
         if (blist) {       // the records of a class are scattered: one bulk copy per block
@@ -449,7 +454,7 @@ match_pair_kernel(const __grid_constant__ CUtensorMap tm_moving, const PairArgs 
             ((float *)(s_unions + (size_t)gg * a.union_stride))[((size_t)zz * UX + yy) * PITCH + xx] = v;
         }
     }
-    mbar_wait(&ctrl->bar, 0);
+    if (!mbar_wait(&ctrl->bar, 0)) ctrl->stage_failed = 1;
     // ---- undo the TMA alignment slack: shift every staged row left by its block's 0..3 floats
     if (a.use_tma && !blist) {
         const int rows_per_block = UZ * UX;
@@ -464,7 +469,12 @@ match_pair_kernel(const __grid_constant__ CUtensorMap tm_moving, const PairArgs 
             else shift_row_left<3, UX, PITCH>(row);
         }
     }
-    if (!blist || !a.use_tma) __syncthreads();      // class mode with TMA: nothing was rewritten, the mbarrier wait orders the reads
+    __syncthreads();
+    if (ctrl->stage_failed) {      // uniform: the copies did not land in time -- report, never fault (NRR_E_DEVICE)
+        for (int gg = 0; gg < gact; ++gg)
+            if (ctrl->org[gg].w) write_error_result(ctrl->bidx[gg], a.out_disp, a.out_ncc, a.err_flag, kErrStaging);
+        return;
+    }
 
     // ---- M3: cross terms
     float ra[W], rb[W];
@@ -768,12 +778,13 @@ int launch_pair(const float *fixed, const float *moving, const float *inv_sd, In
     profile_end(3, stream);
     NRR_LAUNCH_CHECK("prep_kernel");
     auto kern = match_pair_kernel<B, R>;
-    static size_t configured_smem = 0;     // per instantiation
-    if (g.smem > configured_smem) {
+    static size_t configured_smem[kMaxDevices] = {};     // per instantiation and device
+    size_t &conf = configured_smem[current_device()];
+    if (g.smem > conf) {
         NRR_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem));
         // two CTAs per SM only fit if the L1/shared split is at its shared-memory maximum
         NRR_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared));
-        configured_smem = g.smem;
+        conf = g.smem;
     }
     PairArgs a;
     a.fixed = fixed; a.moving = moving; a.inv_sd = inv_sd; a.records = records; a.blocks = blocks; a.task_tab = tab;
@@ -781,6 +792,7 @@ int launch_pair(const float *fixed, const float *moving, const float *inv_sd, In
     a.use_tma = use_tma;
     a.perm = perm; a.cls_count = cls_count; a.n_cap = n;
     a.n_pair_warps = g.n_pair_warps; a.union_stride = g.union_stride; a.tie_band = g_tie_band;
+    a.err_flag = err_flag; a.debug_tx_extra = (unsigned int)g_debug_tx_extra;
     profile_begin(2, stream);
     NRR_LAUNCH(kern, (n + g.G - 1) / g.G + (perm ? 3 : 0), g.threads, g.smem, stream, tm_m, a);
     profile_end(2, stream);

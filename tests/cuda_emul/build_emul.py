@@ -16,7 +16,8 @@ LIB = os.path.join(HERE, "libnrr_bm_emul_asan.so" if ASAN else "libnrr_bm_emul.s
 FLAGS = ["-std=c++17", "-O1", "-g", "-ffp-contract=off", "-fPIC", "-fvisibility=hidden", "-fno-strict-aliasing",
          "-Wno-attributes", "-Wno-unknown-pragmas", "-I", os.path.join(HERE, "include")]
 if ASAN:
-    FLAGS += ["-fsanitize=address", "-fno-omit-frame-pointer"]
+    # alignment: a misaligned float4 / double2 / ulonglong2 access (a misaligned-address fault on the GPU) aborts here
+    FLAGS += ["-fsanitize=address", "-fsanitize=alignment", "-fno-sanitize-recover=alignment", "-fno-omit-frame-pointer"]
 
 
 def needs_build() -> bool:
@@ -54,7 +55,7 @@ def build(force: bool = False) -> str:
     if failed:
         raise RuntimeError("g++ failed building the CUDA emulation")
     tmp = LIB + ".tmp.%d" % os.getpid()
-    subprocess.run(["g++", "-shared"] + (["-fsanitize=address"] if ASAN else []) + ["-o", tmp] + objs, check=True)
+    subprocess.run(["g++", "-shared"] + (["-fsanitize=address", "-fsanitize=alignment"] if ASAN else []) + ["-o", tmp] + objs, check=True)
     os.replace(tmp, LIB)
     return LIB
 

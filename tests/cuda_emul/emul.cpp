@@ -223,6 +223,8 @@ bool mbar_try_wait(void *bar, unsigned parity)
     return false;
 }
 
+void mbar_timeout() { g_cta->progress++; }
+
 void tma_load_3d(void *dst, const void *map_, int x, int y, int z, void *bar)
 {
     const CUtensorMap *map = (const CUtensorMap *)map_;
@@ -373,6 +375,8 @@ cudaError_t cudaMalloc(void **p, size_t bytes)
 cudaError_t cudaFree(void *p) { free(p); return cudaSuccess; }
 cudaError_t cudaMallocHost(void **p, size_t bytes) { return cudaMalloc(p, bytes); }
 cudaError_t cudaMallocAsync(void **p, size_t bytes, cudaStream_t) { return cudaMalloc(p, bytes); }
+cudaError_t cudaMemPoolCreate(cudaMemPool_t *pool, const cudaMemPoolProps *) { *pool = (cudaMemPool_t)0x1; return cudaSuccess; }
+cudaError_t cudaMallocFromPoolAsync(void **p, size_t bytes, cudaMemPool_t, cudaStream_t) { return cudaMalloc(p, bytes); }
 cudaError_t cudaFreeAsync(void *p, cudaStream_t) { free(p); return cudaSuccess; }     // launches are synchronous here
 cudaError_t cudaMemset(void *p, int v, size_t bytes) { memset(p, v, bytes); return cudaSuccess; }
 cudaError_t cudaMemsetAsync(void *p, int v, size_t bytes, cudaStream_t) { memset(p, v, bytes); return cudaSuccess; }

@@ -71,6 +71,11 @@ cudaError_t cudaMalloc(void **p, size_t bytes);
 cudaError_t cudaFree(void *p);
 cudaError_t cudaMallocHost(void **p, size_t bytes);
 cudaError_t cudaMallocAsync(void **p, size_t bytes, cudaStream_t s);
+enum { cudaMemAllocationTypePinned = 1, cudaMemHandleTypeNone = 0, cudaMemLocationTypeDevice = 1 };
+struct cudaMemLocation { int type, id; };
+struct cudaMemPoolProps { int allocType, handleTypes; cudaMemLocation location; };
+cudaError_t cudaMemPoolCreate(cudaMemPool_t *pool, const cudaMemPoolProps *props);
+cudaError_t cudaMallocFromPoolAsync(void **p, size_t bytes, cudaMemPool_t pool, cudaStream_t s);
 cudaError_t cudaFreeAsync(void *p, cudaStream_t s);
 cudaError_t cudaMemset(void *p, int v, size_t bytes);
 cudaError_t cudaMemsetAsync(void *p, int v, size_t bytes, cudaStream_t s);
@@ -106,6 +111,7 @@ void warp_gather(unsigned mask, unsigned long long v, unsigned long long out[32]
 void mbar_init(void *bar, unsigned count);
 void mbar_arrive_expect_tx(void *bar, unsigned bytes);
 bool mbar_try_wait(void *bar, unsigned parity);
+void mbar_timeout();      // the kernel's bounded wait gave up (counts as progress: the thread moves on)
 void tma_load_3d(void *dst, const void *map, int x, int y, int z, void *bar);
 void bulk_load(void *dst, const void *src, unsigned bytes, void *bar);
 }  // namespace emul

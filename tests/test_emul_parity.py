@@ -31,7 +31,7 @@ def _shift_noise(vol, s, noise, seed):
 @pytest.fixture(autouse=True)
 def _default_options():
     for name, v in (("force_rows", 0), ("force_generic", 0), ("disable_tma", 0), ("pair_blocks_per_cta", 0), ("tie_band", 1e-4),
-                    ("select_generic", 0), ("boxstat_generic", 0), ("pair_xoff_classes", 0)):
+                    ("select_generic", 0), ("boxstat_generic", 0), ("pair_xoff_classes", 0), ("debug_expect_tx_extra", 0)):
         _emul.set_option(name, v)
     yield
 
@@ -273,3 +273,21 @@ def test_emulated_warp_matches_the_oracle(dims, amp):
     assert np.max(np.abs(got.astype(np.float64) - want)) <= 8 * 2.0 ** -24 * 1000.0
     zero = np.zeros_like(field)
     assert np.array_equal(_emul.warp(img, zero), img)              # identity is exact
+
+
+def test_emulated_staging_timeout_is_an_error_code_not_a_fault():
+    """A mis-programmed staging barrier (here: 16 bytes more expected than the copies deliver) must end as
+    NRR_E_DEVICE with NaN results -- the kernels' bounded wait gives up, every thread of the CTA leaves in an
+    orderly way, nothing traps (a device trap is an Xid on a shared GPU box)."""
+    dims, block, window = (40, 36, 24), (5, 5, 5), (3, 3, 3)
+    vol = _smooth(dims, 77)
+    mov = _shift_noise(vol, (1, 0, -1), 10.0, 78)
+    sel = oracle.select(vol, block, block, 0.5)
+    assert _emul.match_info(dims, block, window)["kernel"] == 2 and _emul.match_info(dims, block, window)["tma"] == 1
+    good_d, good_n = _emul.match(vol, mov, sel["centres"], block, window)
+    _emul.set_option("debug_expect_tx_extra", 16)
+    with pytest.raises(RuntimeError, match="status -12"):
+        _emul.match(vol, mov, sel["centres"], block, window)
+    _emul.set_option("debug_expect_tx_extra", 0)
+    d, n = _emul.match(vol, mov, sel["centres"], block, window)      # the flag was cleared; the library still works
+    assert np.array_equal(d, good_d) and np.array_equal(n, good_n)
