@@ -237,8 +237,6 @@ NRR_BM_API int nrr_bm_pair_task_table(const int block[3], const int window[3], u
  *   "force_rows"    != 0: skip the pair kernel (one candidate row per thread instead)
  *   "disable_tma"   != 0: stage shared memory with plain loads instead of TMA
  *   "pair_blocks_per_cta"  > 0: blocks per CTA of the pair kernel (0 = the planner's choice)
- *   "pair_xoff_classes" != 0: the pair kernel's CTAs take blocks of one TMA alignment class and read the slack away in
- *                   register indices instead of shifting the staged rows (experimental, off by default)
  *   "boxstat_generic" / "select_generic" != 0: the runtime-shaped moving-statistics / selection kernels */
 NRR_BM_API int nrr_bm_set_option(const char *name, double value);
 

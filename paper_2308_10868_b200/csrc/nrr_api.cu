@@ -18,7 +18,6 @@ extern int g_force_generic;
 extern int g_disable_tma;
 extern int g_force_rows;
 extern int g_pair_g;
-extern int g_pair_xoff_classes;
 extern int g_debug_tx_extra;
 extern int g_boxstat_generic;
 extern int g_select_generic;
@@ -643,7 +642,6 @@ int nrr_bm_set_option(const char *name, double value)
     if (!strcmp(name, "select_generic")) { g_select_generic = value != 0.0; return NRR_OK; }
     if (!strcmp(name, "boxstat_generic")) { g_boxstat_generic = value != 0.0; return NRR_OK; }
     if (!strcmp(name, "force_rows")) { g_force_rows = value != 0.0; return NRR_OK; }
-    if (!strcmp(name, "pair_xoff_classes")) { g_pair_xoff_classes = value != 0.0; return NRR_OK; }
     if (!strcmp(name, "pair_blocks_per_cta")) { g_pair_g = (int)value; return NRR_OK; }
     if (!strcmp(name, "debug_expect_tx_extra")) { g_debug_tx_extra = (int)value & ~15; return NRR_OK; }
     return fail(NRR_E_ARG, "unknown option '%s'", name);

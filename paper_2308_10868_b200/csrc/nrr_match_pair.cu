@@ -50,7 +50,6 @@ namespace nrr {
 
 extern float g_tie_band;
 extern int g_disable_tma;
-int g_pair_xoff_classes = 0;   // experiment knob: CTAs of equal TMA alignment slack, no row shift (see PairArgs)
 int g_pair_g = 0;             // experiment knob: force the number of blocks per CTA (0 = planner's choice)
 int g_debug_tx_extra = 0;     // test hook: over-programs the staging barrier so that its wait must time out
 
@@ -160,10 +159,8 @@ template <int B, int R>
 __global__ void __launch_bounds__(kPrepWarps * 32)
 prep_kernel(const float *__restrict__ fixed, Int3 dims, const int *__restrict__ blocks, int n, int bz,
             const unsigned int *__restrict__ n_dev, float *__restrict__ records, int *__restrict__ out_disp,
-            float *__restrict__ out_ncc, unsigned int *err_flag, int *__restrict__ perm, unsigned int *cls_count,
-            int use_slack)
+            float *__restrict__ out_ncc, unsigned int *err_flag)
 {
-    const int n_cap = n;
     if (n_dev) n = min(n, (int)*n_dev);               // the launch was sized for an upper bound
     using C = PairCfg<B, R>;
     const int NVOX = B * B * bz;
@@ -217,10 +214,6 @@ prep_kernel(const float *__restrict__ fixed, Int3 dims, const int *__restrict__ 
         const int zr = row / B + 1, vy = row % B, vx = k >> 1, h = k & 1;
         pt[i] = vx < B ? f[((zr - h) * B + vy) * B + vx] : 0.f;
     }
-    if (lane == 0 && perm) {      // class mode: bucket the block by the alignment slack of its union (any order inside a class)
-        const int c = use_slack ? ((ox - R) & 3) : 0;
-        perm[(size_t)c * n_cap + atomicAdd(&cls_count[c], 1u)] = b;
-    }
     if (lane == 0) {
         hdr[0] = ssf == 0.0 ? 0.f : (float)(1.0 / sqrt(ssf));
         hdr[1] = 1.f;
@@ -242,14 +235,11 @@ __device__ __forceinline__ void load_row(float (&m)[NV * 4], const float *p)
 
 // Two candidate rows per thread: row A at union plane offset 0, row B one plane further.
 // urow = first moving row of A; rec = this block's record; ra/rb receive the raw numerators.
-// XOFF: the staged rows start XOFF floats left of the window union (the TMA alignment slack, left in place when
-// all blocks of a CTA share it): the moving voxel of candidate j and block column vx is m[j + vx + XOFF].
-template <int B, int R, int XOFF>
+template <int B, int R>
 __device__ __forceinline__ void pair_rows(const float *urow, const float *rec, int bz, float (&ra)[2 * R + 1], float (&rb)[2 * R + 1])
 {
     using C = PairCfg<B, R>;
-    constexpr int NVX = (C::UX + XOFF + 3) / 4;
-    static_assert(NVX * 4 <= C::PITCH, "row pitch must cover the slack");
+    constexpr int NVX = C::NV;
     constexpr int W = C::W, PITCH = C::PITCH, PLANE = C::UX * C::PITCH;
     u64 acc[W];
 #pragma unroll
@@ -263,7 +253,7 @@ __device__ __forceinline__ void pair_rows(const float *urow, const float *rec, i
 #pragma unroll
         for (int vx = 0; vx < B; ++vx)
 #pragma unroll
-            for (int j = 0; j < W; ++j) fma_lo(acc[j], f[vx], m[j + vx + XOFF]);
+            for (int j = 0; j < W; ++j) fma_lo(acc[j], f[vx], m[j + vx]);
     }
     // planes 1..bz-1: both rows, (f'[zr], f'[zr-1]) pairs
     const float *pt = rec + C::plain_floats(bz);
@@ -284,7 +274,7 @@ __device__ __forceinline__ void pair_rows(const float *urow, const float *rec, i
 #pragma unroll
             for (int vx = 0; vx < B; ++vx)
 #pragma unroll
-                for (int j = 0; j < W; ++j) fma2s(acc[j], m[j + vx + XOFF], f[vx]);
+                for (int j = 0; j < W; ++j) fma2s(acc[j], m[j + vx], f[vx]);
         }
     }
     // plane bz: row B only, fixed plane bz-1
@@ -299,7 +289,7 @@ __device__ __forceinline__ void pair_rows(const float *urow, const float *rec, i
 #pragma unroll
             for (int vx = 0; vx < B; ++vx)
 #pragma unroll
-                for (int j = 0; j < W; ++j) fma_hi(acc[j], f[vx], m[j + vx + XOFF]);
+                for (int j = 0; j < W; ++j) fma_hi(acc[j], f[vx], m[j + vx]);
         }
     }
 #pragma unroll
@@ -310,11 +300,11 @@ __device__ __forceinline__ void pair_rows(const float *urow, const float *rec, i
 }
 
 // One candidate row per thread (the odd last plane of candidates).
-template <int B, int R, int XOFF>
+template <int B, int R>
 __device__ __forceinline__ void single_row(const float *urow, const float *rec, int bz, float (&ra)[2 * R + 1])
 {
     using C = PairCfg<B, R>;
-    constexpr int NVX = (C::UX + XOFF + 3) / 4;
+    constexpr int NVX = C::NV;
     constexpr int W = C::W, PITCH = C::PITCH, PLANE = C::UX * C::PITCH;
 #pragma unroll
     for (int j = 0; j < W; ++j) ra[j] = 0.f;
@@ -330,7 +320,7 @@ __device__ __forceinline__ void single_row(const float *urow, const float *rec, 
 #pragma unroll
             for (int vx = 0; vx < B; ++vx)
 #pragma unroll
-                for (int j = 0; j < W; ++j) ra[j] = fmaf(f[vx], m[j + vx + XOFF], ra[j]);
+                for (int j = 0; j < W; ++j) ra[j] = fmaf(f[vx], m[j + vx], ra[j]);
         }
     }
 }
@@ -346,12 +336,6 @@ struct PairArgs {
     Int3 dims;
     int n, rz, bz, G, n_pair_warps;
     int use_tma;                   // 0: the unions are staged with plain loads (volumes TMA cannot address)
-    // class mode (option "pair_xoff_classes"): the prep kernel has bucketed the blocks by the alignment slack of their
-    // union, (ox - R) & 3; a CTA takes G blocks of ONE class, leaves the slack in place and reads it away in the
-    // register indices of a main loop compiled for it -- no row shift, one barrier less.
-    const int *perm;               // [4][n_cap] block indices per class, or NULL
-    const unsigned int *cls_count; // [4]
-    int n_cap;
     int union_stride;              // bytes between the unions of consecutive blocks of a CTA (multiple of 128)
     float tie_band;
     unsigned int *err_flag;        // sticky device flag (kErrStaging when the staged copies do not land)
@@ -372,28 +356,10 @@ match_pair_kernel(const __grid_constant__ CUtensorMap tm_moving, const PairArgs 
     PairCtrl *ctrl = (PairCtrl *)((unsigned char *)s_recs + (size_t)a.G * REC_FLOATS * 4);
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    int b0, gact, xcls = 0;
-    const int *blist = nullptr;                        // class mode: this CTA's block indices
-    if (a.perm) {
-        int first = 0, c = 0, cnt = 0;
-        for (; c < 4; ++c) {
-            cnt = (int)a.cls_count[c];
-            const int chunks = (cnt + a.G - 1) / a.G;
-            if ((int)blockIdx.x < first + chunks) break;
-            first += chunks;
-        }
-        if (c == 4) return;                            // uniform: the launch was sized for an upper bound
-        const int off = ((int)blockIdx.x - first) * a.G;
-        b0 = 0;
-        gact = min(a.G, cnt - off);
-        blist = a.perm + (size_t)c * a.n_cap + off;
-        xcls = a.use_tma ? c : 0;
-    } else {
-        const int n = a.n_dev ? min(a.n, (int)*a.n_dev) : a.n;
-        b0 = blockIdx.x * a.G;
-        if (b0 >= n) return;                           // uniform: the launch was sized for an upper bound
-        gact = min(a.G, n - b0);
-    }
+    const int n = a.n_dev ? min(a.n, (int)*a.n_dev) : a.n;
+    const int b0 = blockIdx.x * a.G;
+    if (b0 >= n) return;                               // uniform: the launch was sized for an upper bound
+    const int gact = min(a.G, n - b0);
     const int rz = a.rz, WZ = 2 * rz + 1, UZ = bz + 2 * rz;
     const Int3 dims = a.dims;
     const uint32_t union_bytes = (uint32_t)(sizeof(float) * UZ * UX * PITCH);
@@ -407,7 +373,7 @@ match_pair_kernel(const __grid_constant__ CUtensorMap tm_moving, const PairArgs 
         }
         int ox = 0, oy = 0, oz = 0, ok = 0, bi = 0;
         if (lane < gact) {
-            bi = blist ? blist[lane] : b0 + lane;
+            bi = b0 + lane;
             ox = a.blocks[3 * (size_t)bi + 0] - (B - 1) / 2;
             oy = a.blocks[3 * (size_t)bi + 1] - (B - 1) / 2;
             oz = a.blocks[3 * (size_t)bi + 2] - (bz - 1) / 2;
@@ -425,11 +391,7 @@ match_pair_kernel(const __grid_constant__ CUtensorMap tm_moving, const PairArgs 
             mbar_arrive_expect_tx(&ctrl->bar, (a.use_tma ? (uint32_t)__popc(okmask) * union_bytes : 0u) + (uint32_t)gact * REC_FLOATS * 4u + a.debug_tx_extra);
         __syncwarp();
         if (ok && a.use_tma) tma_load_3d(s_unions + (size_t)lane * a.union_stride, &tm_moving, (ox - R) & ~3, oy - R, oz - rz, &ctrl->bar);
-        if (blist) {       // the records of a class are scattered: one bulk copy per block
-            if (lane < gact) bulk_load(s_recs + (size_t)lane * REC_FLOATS, a.records + (size_t)bi * REC_FLOATS, (uint32_t)REC_FLOATS * 4u, &ctrl->bar);
-        } else if (lane == 0) {
-            bulk_load(s_recs, a.records + (size_t)b0 * REC_FLOATS, (uint32_t)gact * REC_FLOATS * 4u, &ctrl->bar);
-        }
+        if (lane == 0) bulk_load(s_recs, a.records + (size_t)b0 * REC_FLOATS, (uint32_t)gact * REC_FLOATS * 4u, &ctrl->bar);
     }
     // this lane's task
     const uint32_t task = a.task_tab[tid];
@@ -456,7 +418,7 @@ match_pair_kernel(const __grid_constant__ CUtensorMap tm_moving, const PairArgs 
     }
     if (!mbar_wait(&ctrl->bar, 0)) ctrl->stage_failed = 1;
     // ---- undo the TMA alignment slack: shift every staged row left by its block's 0..3 floats
-    if (a.use_tma && !blist) {
+    if (a.use_tma) {
         const int rows_per_block = UZ * UX;
         for (int r = tid; r < gact * rows_per_block; r += blockDim.x) {
             const int gg = r / rows_per_block, rr = r - gg * rows_per_block;
@@ -480,20 +442,9 @@ match_pair_kernel(const __grid_constant__ CUtensorMap tm_moving, const PairArgs 
     float ra[W], rb[W];
     const float *urow = (const float *)(s_unions + (size_t)g * a.union_stride) + (size_t)dzA * PLANE + dyi * PITCH;
     const float *rec = s_recs + (size_t)g * REC_FLOATS;
-    if (is_pair) {
-        if (active) {
-            if (xcls == 0) pair_rows<B, R, 0>(urow, rec, bz, ra, rb);
-            else if (xcls == 1) pair_rows<B, R, 1>(urow, rec, bz, ra, rb);
-            else if (xcls == 2) pair_rows<B, R, 2>(urow, rec, bz, ra, rb);
-            else pair_rows<B, R, 3>(urow, rec, bz, ra, rb);
-        }
-    } else {
-        if (active) {
-            if (xcls == 0) single_row<B, R, 0>(urow, rec, bz, ra);
-            else if (xcls == 1) single_row<B, R, 1>(urow, rec, bz, ra);
-            else if (xcls == 2) single_row<B, R, 2>(urow, rec, bz, ra);
-            else single_row<B, R, 3>(urow, rec, bz, ra);
-        }
+    if (active) {
+        if (is_pair) pair_rows<B, R>(urow, rec, bz, ra, rb);
+        else single_row<B, R>(urow, rec, bz, ra);
     }
 
     // ---- M4: NCC and the per-block arg-max
@@ -760,21 +711,13 @@ int launch_pair(const float *fixed, const float *moving, const float *inv_sd, In
     const uint32_t *tab = nullptr;
     int rc = task_table_device<B, R>(rz, g, stream, &tab);
     if (rc) return rc;
-    AsyncScratch rec_buf(stream), perm_buf(stream);
+    AsyncScratch rec_buf(stream);
     NRR_CUDA(rec_buf.alloc((size_t)n * C::rec_bytes(bz)));
     float *records = (float *)rec_buf.p;
-    int *perm = nullptr;
-    unsigned int *cls_count = nullptr;
-    if (g_pair_xoff_classes) {
-        NRR_CUDA(perm_buf.alloc(sizeof(int) * 4 * (size_t)n + 4 * sizeof(unsigned int)));
-        perm = (int *)perm_buf.p;
-        cls_count = (unsigned int *)(perm + 4 * (size_t)n);
-        NRR_CUDA(cudaMemsetAsync(cls_count, 0, 4 * sizeof(unsigned int), stream));
-    }
     auto prep = prep_kernel<B, R>;
     profile_begin(3, stream);
     NRR_LAUNCH(prep, (n + kPrepWarps - 1) / kPrepWarps, kPrepWarps * 32, 0, stream, fixed, dims, blocks, n, bz,
-               t_match_n_dev, records, out_disp, out_ncc, err_flag, perm, cls_count, use_tma);
+               t_match_n_dev, records, out_disp, out_ncc, err_flag);
     profile_end(3, stream);
     NRR_LAUNCH_CHECK("prep_kernel");
     auto kern = match_pair_kernel<B, R>;
@@ -790,11 +733,10 @@ int launch_pair(const float *fixed, const float *moving, const float *inv_sd, In
     a.fixed = fixed; a.moving = moving; a.inv_sd = inv_sd; a.records = records; a.blocks = blocks; a.task_tab = tab;
     a.out_disp = out_disp; a.out_ncc = out_ncc; a.dims = dims; a.n = n; a.rz = rz; a.bz = bz; a.G = g.G; a.n_dev = t_match_n_dev;
     a.use_tma = use_tma;
-    a.perm = perm; a.cls_count = cls_count; a.n_cap = n;
     a.n_pair_warps = g.n_pair_warps; a.union_stride = g.union_stride; a.tie_band = g_tie_band;
     a.err_flag = err_flag; a.debug_tx_extra = (unsigned int)g_debug_tx_extra;
     profile_begin(2, stream);
-    NRR_LAUNCH(kern, (n + g.G - 1) / g.G + (perm ? 3 : 0), g.threads, g.smem, stream, tm_m, a);
+    NRR_LAUNCH(kern, (n + g.G - 1) / g.G, g.threads, g.smem, stream, tm_m, a);
     profile_end(2, stream);
     NRR_LAUNCH_CHECK("match_pair_kernel");
     return NRR_OK;      // the scratch is released behind the kernels, in stream order

@@ -223,8 +223,6 @@ def main():
         case_match((36, 32, 28), (5, 5, 5), (7, 7, 1), expect_kernel=2)
         case_match((48, 44, 24), (7, 7, 3), (5, 5, 2), expect_kernel=2)
         case_match((40, 36, 24), (5, 5, 5), (3, 3, 3), {"pair_blocks_per_cta": 3}, expect_kernel=2)
-        case_match((40, 36, 24), (5, 5, 5), (3, 3, 3), {"pair_xoff_classes": 1}, expect_kernel=2)
-        case_match((48, 40, 30), (7, 7, 7), (5, 5, 3), {"pair_xoff_classes": 1}, expect_kernel=2)
         case_match((40, 36, 24), (5, 5, 5), (3, 3, 3), {"disable_tma": 1}, expect_kernel=2)
     case_match((40, 36, 24), (5, 5, 5), (3, 3, 3), {"force_rows": 1}, expect_kernel=1)
     if not quick:

@@ -31,7 +31,7 @@ def _shift_noise(vol, s, noise, seed):
 @pytest.fixture(autouse=True)
 def _default_options():
     for name, v in (("force_rows", 0), ("force_generic", 0), ("disable_tma", 0), ("pair_blocks_per_cta", 0), ("tie_band", 1e-4),
-                    ("select_generic", 0), ("boxstat_generic", 0), ("pair_xoff_classes", 0), ("debug_expect_tx_extra", 0)):
+                    ("select_generic", 0), ("boxstat_generic", 0), ("debug_expect_tx_extra", 0)):
         _emul.set_option(name, v)
     yield
 
@@ -126,13 +126,6 @@ def test_emulated_pair_kernel_matches_the_oracle(dims, b, r, rz, stride, g):
     disp2, ncc2 = _emul.match(fixed, moving, blocks, block, window)
     _emul.set_option("disable_tma", 0)
     assert np.array_equal(disp, disp2) and np.array_equal(ncc, ncc2)
-    for tma_off in (0, 1):                                 # CTAs of one alignment class, slack read away in registers
-        _emul.set_option("pair_xoff_classes", 1)
-        _emul.set_option("disable_tma", tma_off)
-        disp3, ncc3 = _emul.match(fixed, moving, blocks, block, window)
-        _emul.set_option("pair_xoff_classes", 0)
-        _emul.set_option("disable_tma", 0)
-        assert np.array_equal(disp, disp3) and np.array_equal(ncc, ncc3)
     _emul.set_option("force_rows", 1)                      # the one-row-per-thread kernel on the same input
     disp, ncc = _emul.match(fixed, moving, blocks, block, window)
     assert_match_parity(disp, ncc, om, "rows %s" % (dims,))
@@ -148,7 +141,7 @@ def test_emulated_degenerate_inputs():
     block, window = (5, 5, 5), (3, 3, 3)
     blocks = _grid_blocks(dims, block, (6, 6, 5))
     om = oracle.match(fixed, moving, blocks, block, window)
-    for opts in (dict(), dict(force_rows=1), dict(force_generic=1), dict(pair_xoff_classes=1)):
+    for opts in (dict(), dict(force_rows=1), dict(force_generic=1)):
         for k, v in opts.items():
             _emul.set_option(k, v)
         disp, ncc = _emul.match(fixed, moving, blocks, block, window)
@@ -202,7 +195,7 @@ def test_emulated_register_needs_no_host_side_count():
     ora_sel = oracle.select(fixed, block, stride, 0.5, mask)
     ora = oracle.match(fixed, moving, ora_sel["centres"], block, window)
     assert 0 < len(ora_sel["centres"]) < 0.2 * 8 * 7 * 6             # far fewer than the host-side bound
-    for opts in (dict(), dict(force_rows=1), dict(force_generic=1), dict(pair_xoff_classes=1)):
+    for opts in (dict(), dict(force_rows=1), dict(force_generic=1)):
         for k, v in opts.items():
             _emul.set_option(k, v)
         blocks, disp, ncc = _emul.register(fixed, moving, block, stride, window, 0.5, mask)
