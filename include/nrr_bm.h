@@ -32,7 +32,7 @@
 extern "C" {
 #endif
 
-#define NRR_BM_VERSION 100 /* 0.1.0 : major*10000 + minor*100 + patch */
+#define NRR_BM_VERSION 200 /* 0.2.0 : major*10000 + minor*100 + patch */
 
 #if defined(__GNUC__)
 #define NRR_BM_API __attribute__((visibility("default")))
@@ -180,6 +180,89 @@ NRR_BM_API int nrr_bm_moving_stats_host(const float *moving, const int dims[3], 
 NRR_BM_API int nrr_bm_warp(const float *image, const int dims[3], const float *field, float *out, void *stream);
 NRR_BM_API int nrr_bm_warp_host(const float *image, const int dims[3], const float *field, float *out);
 
+/*
+ * Upper bound on K, for sizing out_blocks / out_disp / out_ncc before a call that does not return K on the host
+ * (nrr_bm_register, nrr_bm_register_batch).  *out_grid = stride-grid positions (an upper bound on N),
+ * *out_bound >= floor(0.5 + N*frac) for every N <= *out_grid  (count rule of PAPER.md:376).  Pure host arithmetic;
+ * the method's formula lives in the library, not in its callers.  Either output may be NULL.
+ */
+NRR_BM_API int nrr_bm_capacity_bound(const int dims[3], const int block[3], const int stride[3], double frac,
+                                     int *out_grid, int *out_bound);
+
+/*
+ * PLANS: the boundary split along the paper's timeline  --  PAPER.md:231-236 (section 3): registration points "can be
+ * identified prior to the time-critical part of the computation in the floating (pre-operative) image.  Once the
+ * reference (intra-operative) scan is available, the deformation vector is estimated at each of the selected
+ * points by means of block matching", and PAPER.md:267-268 ("block matching ... time critical and should be
+ * performed while the surgeons are waiting").
+ *
+ *   nrr_bm_plan_create        PRE-OPERATIVE.  Everything that needs only the pre-operative (`fixed`) image: block
+ *                             selection (S1-S3; connectivity = 0, 6, 18 or 26 as in nrr_bm_select_blocks_pruned), the
+ *                             fixed-block records of the matching kernel (centred blocks, 1/sqrt(SS_f)), the kernel's
+ *                             launch tables and all scratch.  Synchronises `stream`.
+ *   nrr_bm_plan_match         INTRA-OPERATIVE, asynchronous on `stream`: the moving-volume normalisers (M2) and the
+ *                             matching kernel (M1, M3-M5) for one intra-operative volume.  out_disp [n][3], out_ncc [n]
+ *                             in the order of nrr_bm_plan_blocks.  Results are bit-identical to
+ *                             nrr_bm_select_blocks + nrr_bm_match with the same arguments.
+ *   nrr_bm_plan_match_range   the same for blocks [first, first + count) only; rows outside the range are left
+ *                             untouched.  This is the natural shard of the path over several GPUs (PAPER.md:379-385:
+ *                             both images on every processor, the block list distributed): rank r
+ *                             holds a plan of its own, matches its slice and the ranks exchange 16 bytes per block.
+ *   nrr_bm_plan_match_host    the same as nrr_bm_plan_match with HOST buffers (pinned memory makes the copies
+ *                             asynchronous); synchronises.  The volume goes up in z slabs on a copy stream while the
+ *                             normalisers and the matching of the blocks whose windows have landed already run, so
+ *                             the call costs about one upload of `moving` plus the work on the last slab.
+ *   nrr_bm_plan_destroy       releases everything the plan owns (NULL is allowed).
+ *
+ * OWNERSHIP.  nrr_bm_plan_create keeps the caller's `fixed` DEVICE pointer (the FP64 near-tie re-score reads the raw
+ * voxels): it must stay valid and unchanged until nrr_bm_plan_destroy.  nrr_bm_plan_create_host takes HOST `fixed` /
+ * `mask`, uploads them and owns the device copies.  A plan belongs to the device that was current at creation and
+ * serves ONE match call at a time (calls on one stream are ordered by the stream; concurrent calls on several
+ * streams must be ordered by the caller: they share the plan's scratch).  Errors as everywhere in this ABI;
+ * NRR_E_ARG for a NULL / destroyed plan or a range outside [0, n].
+ */
+typedef struct nrr_bm_plan nrr_bm_plan;
+NRR_BM_API int nrr_bm_plan_create(const float *fixed, const int dims[3], const int block[3], const int stride[3],
+                                  const int window[3], double frac, const unsigned char *mask, int connectivity,
+                                  void *stream, nrr_bm_plan **out_plan);
+NRR_BM_API int nrr_bm_plan_create_host(const float *fixed, const int dims[3], const int block[3], const int stride[3],
+                                       const int window[3], double frac, const unsigned char *mask, int connectivity,
+                                       nrr_bm_plan **out_plan);
+/* *out_n = K selected blocks, *out_ncand = N candidates (either may be NULL). */
+NRR_BM_API int nrr_bm_plan_info(const nrr_bm_plan *plan, int *out_n, int *out_ncand);
+/* Block centres [n][3] (ascending candidate index) and, if out_var != NULL, their variances [n]: HOST buffers. */
+NRR_BM_API int nrr_bm_plan_blocks_host(const nrr_bm_plan *plan, int *out_blocks, double *out_var);
+/* DEVICE pointer to the plan's block centres [n][3] (owned by the plan, valid until nrr_bm_plan_destroy). */
+NRR_BM_API const int *nrr_bm_plan_blocks_device(const nrr_bm_plan *plan);
+NRR_BM_API int nrr_bm_plan_match(nrr_bm_plan *plan, const float *moving, int *out_disp, float *out_ncc, void *stream);
+NRR_BM_API int nrr_bm_plan_match_range(nrr_bm_plan *plan, const float *moving, int first, int count, int *out_disp,
+                                       float *out_ncc, void *stream);
+NRR_BM_API int nrr_bm_plan_match_host(nrr_bm_plan *plan, const float *moving, int *out_disp, float *out_ncc);
+NRR_BM_API int nrr_bm_plan_destroy(nrr_bm_plan *plan);
+
+/*
+ * PARAMETER SWEEP: one volume pair under many settings in ONE launch sequence  --  PAPER.md:527-540 (section 4.2,
+ * speculative execution: "multiple instances of NRR are executed" with different parameter values) and PAPER.md:711
+ * (block and window sizes are per-axis parameters); BASELINE.json configs[4].  No host synchronisation.  What the
+ * settings have in common is computed once: the moving-volume normalisers per distinct block shape, the block
+ * variances per distinct (block, stride) -- several fractions are selected from the same keys --, the fixed-block
+ * records per distinct (block, stride, frac); the matching launches are spread over a few streams that fork from and
+ * join into `stream`.  Per setting s the results are bit-identical to nrr_bm_register with that setting:
+ *   out_blocks[s] [capacity[s]][3], out_disp[s] [capacity[s]][3], out_ncc[s] [capacity[s]]  DEVICE arrays (the arrays
+ *   of pointers themselves are HOST arrays), out_n DEVICE int [n_settings]: K per setting.
+ * Size capacity[s] with nrr_bm_capacity_bound.
+ */
+typedef struct nrr_bm_setting {
+    int block[3];
+    int stride[3];
+    int window[3];
+    double frac;
+} nrr_bm_setting;
+NRR_BM_API int nrr_bm_register_batch(const float *fixed, const float *moving, const int dims[3],
+                                     const unsigned char *mask, const nrr_bm_setting *settings, int n_settings,
+                                     int *const *out_blocks, const int *capacity, int *out_n, int *const *out_disp,
+                                     float *const *out_ncc, void *stream);
+
 /* Synchronises `stream` and returns NRR_E_DEVICE if a staged copy of a matching kernel enqueued on this thread since
  * the last check did not complete, NRR_E_BOUNDS if one saw a block leaving the volume (and clears the flag),
  * NRR_E_CUDA on a CUDA error, else NRR_OK. */
@@ -237,6 +320,7 @@ NRR_BM_API int nrr_bm_pair_task_table(const int block[3], const int window[3], u
  *   "force_rows"    != 0: skip the pair kernel (one candidate row per thread instead)
  *   "disable_tma"   != 0: stage shared memory with plain loads instead of TMA
  *   "pair_blocks_per_cta"  > 0: blocks per CTA of the pair kernel (0 = the planner's choice)
+ *   "plan_slabs"    z slabs of nrr_bm_plan_match_host's upload pipeline (default 4; 1 = upload, then compute)
  *   "boxstat_generic" / "select_generic" != 0: the runtime-shaped moving-statistics / selection kernels */
 NRR_BM_API int nrr_bm_set_option(const char *name, double value);
 

@@ -23,6 +23,9 @@ EXPORTS = [
     "nrr_bm_select_blocks", "nrr_bm_select_blocks_pruned", "nrr_bm_select_blocks_pruned_host", "nrr_bm_match", "nrr_bm_register", "nrr_bm_check_async_error", "nrr_bm_moving_stats", "nrr_bm_moving_stats_host", "nrr_bm_warp", "nrr_bm_warp_host",
     "nrr_bm_select_blocks_host", "nrr_bm_match_host", "nrr_bm_register_host",
     "nrr_bm_profile_enable", "nrr_bm_profile_read", "nrr_bm_launch_count", "nrr_bm_match_info",
+    "nrr_bm_capacity_bound", "nrr_bm_plan_create", "nrr_bm_plan_create_host", "nrr_bm_plan_info", "nrr_bm_plan_blocks_host",
+    "nrr_bm_plan_blocks_device", "nrr_bm_plan_match", "nrr_bm_plan_match_range", "nrr_bm_plan_match_host", "nrr_bm_plan_destroy",
+    "nrr_bm_register_batch",
     "nrr_bm_fp32_peak", "nrr_bm_pair_task_table", "nrr_bm_set_option", "nrr_bm_last_error", "nrr_bm_status_string", "nrr_bm_version",
 ]
 
@@ -73,6 +76,29 @@ def lib() -> ctypes.CDLL:
     L.nrr_bm_match_host.argtypes = [vp, vp, i3, vp, ci, i3, i3, vp, vp]
     L.nrr_bm_register_host.restype = ci
     L.nrr_bm_register_host.argtypes = [vp, vp, i3, i3, i3, i3, cd, vp, vp, ci, i3, vp, vp]
+    L.nrr_bm_capacity_bound.restype = ci
+    L.nrr_bm_capacity_bound.argtypes = [i3, i3, i3, cd, i3, i3]
+    pp = ctypes.POINTER(vp)
+    L.nrr_bm_plan_create.restype = ci
+    L.nrr_bm_plan_create.argtypes = [vp, i3, i3, i3, i3, cd, vp, ci, vp, pp]
+    L.nrr_bm_plan_create_host.restype = ci
+    L.nrr_bm_plan_create_host.argtypes = [vp, i3, i3, i3, i3, cd, vp, ci, pp]
+    L.nrr_bm_plan_info.restype = ci
+    L.nrr_bm_plan_info.argtypes = [vp, i3, i3]
+    L.nrr_bm_plan_blocks_host.restype = ci
+    L.nrr_bm_plan_blocks_host.argtypes = [vp, vp, vp]
+    L.nrr_bm_plan_blocks_device.restype = vp
+    L.nrr_bm_plan_blocks_device.argtypes = [vp]
+    L.nrr_bm_plan_match.restype = ci
+    L.nrr_bm_plan_match.argtypes = [vp, vp, vp, vp, vp]
+    L.nrr_bm_plan_match_range.restype = ci
+    L.nrr_bm_plan_match_range.argtypes = [vp, vp, ci, ci, vp, vp, vp]
+    L.nrr_bm_plan_match_host.restype = ci
+    L.nrr_bm_plan_match_host.argtypes = [vp, vp, vp, vp]
+    L.nrr_bm_plan_destroy.restype = ci
+    L.nrr_bm_plan_destroy.argtypes = [vp]
+    L.nrr_bm_register_batch.restype = ci
+    L.nrr_bm_register_batch.argtypes = [vp, vp, i3, vp, vp, ci, pp, i3, vp, pp, pp, vp]
     L.nrr_bm_profile_enable.restype = ci
     L.nrr_bm_profile_enable.argtypes = [ci]
     L.nrr_bm_profile_read.restype = ci
@@ -230,10 +256,7 @@ def nrr_bm_register(fixed, moving, block, stride, window, frac: float, mask=None
     if mask is not None:
         mask = _dev(mask, torch.uint8, "mask")
     if capacity is None:
-        ngrid = 1
-        for a in range(3):
-            ngrid *= max(0, (dims[a] - int(block[a])) // max(1, int(stride[a])) + 1)
-        capacity = max(1, min(ngrid, int(np.floor(0.5 + ngrid * float(frac)))))
+        capacity = max(1, nrr_bm_capacity_bound(dims, block, stride, frac)[1])
     dev = fixed.device
     if out_blocks is None:
         out_blocks = torch.empty((capacity, 3), dtype=torch.int32, device=dev)
@@ -249,6 +272,149 @@ def nrr_bm_register(fixed, moving, block, stride, window, frac: float, mask=None
                                      int(capacity), out_n.data_ptr(), out_disp.data_ptr(), out_ncc.data_ptr(),
                                      _stream_ptr(stream)))
     return out_blocks, out_n, out_disp, out_ncc
+
+
+def nrr_bm_capacity_bound(dims, block, stride, frac: float) -> Tuple[int, int]:
+    """(stride-grid positions, upper bound on K) -- the library's own count rule; no device needed."""
+    g, b = ctypes.c_int(0), ctypes.c_int(0)
+    _check(lib().nrr_bm_capacity_bound(_i3(dims), _i3(block), _i3(stride), float(frac), ctypes.byref(g), ctypes.byref(b)))
+    return g.value, b.value
+
+
+class nrr_bm_setting(ctypes.Structure):
+    """One parameter setting of nrr_bm_register_batch (include/nrr_bm.h)."""
+    _fields_ = [("block", ctypes.c_int * 3), ("stride", ctypes.c_int * 3), ("window", ctypes.c_int * 3), ("frac", ctypes.c_double)]
+
+
+def nrr_bm_register_batch(fixed, moving, settings, mask=None, stream=None):
+    """One volume pair under many settings in ONE launch sequence (no host synchronisation).  `settings`: objects with
+    .block, .stride, .window, .frac.  Returns (results, n) with results[s] = (blocks [cap][3], disp [cap][3], ncc [cap])
+    CUDA tensors and n a CUDA int32 tensor [len(settings)] holding K per setting; rows beyond K are untouched."""
+    import torch
+    fixed = _dev(fixed, torch.float32, "fixed")
+    moving = _dev(moving, torch.float32, "moving")
+    if tuple(fixed.shape) != tuple(moving.shape):
+        raise ValueError("volume shape mismatch")
+    if mask is not None:
+        mask = _dev(mask, torch.uint8, "mask")
+    dims = _dims_of(fixed)
+    ns = len(settings)
+    arr = (nrr_bm_setting * max(1, ns))()
+    caps = (ctypes.c_int * max(1, ns))()
+    pb, pd, pn = (ctypes.c_void_p * max(1, ns))(), (ctypes.c_void_p * max(1, ns))(), (ctypes.c_void_p * max(1, ns))()
+    results = []
+    dev = fixed.device
+    for i, st in enumerate(settings):
+        arr[i].block[:] = [int(v) for v in st.block]
+        arr[i].stride[:] = [int(v) for v in st.stride]
+        arr[i].window[:] = [int(v) for v in st.window]
+        arr[i].frac = float(st.frac)
+        cap = max(1, nrr_bm_capacity_bound(dims, st.block, st.stride, st.frac)[1])
+        caps[i] = cap
+        b = torch.empty((cap, 3), dtype=torch.int32, device=dev)
+        d = torch.empty((cap, 3), dtype=torch.int32, device=dev)
+        c = torch.empty((cap,), dtype=torch.float32, device=dev)
+        pb[i], pd[i], pn[i] = b.data_ptr(), d.data_ptr(), c.data_ptr()
+        results.append((b, d, c))
+    out_n = torch.zeros((max(1, ns),), dtype=torch.int32, device=dev)
+    with torch.cuda.device(dev):
+        _check(lib().nrr_bm_register_batch(fixed.data_ptr(), moving.data_ptr(), _i3(dims),
+                                           mask.data_ptr() if mask is not None else None, arr, ns, pb, caps,
+                                           out_n.data_ptr(), pd, pn, _stream_ptr(stream)))
+    return results, out_n[:ns]
+
+
+class NrrPlan:
+    """Handle of an nrr_bm_plan (include/nrr_bm.h "PLANS").  Keeps the `fixed` tensor alive for the device form."""
+
+    def __init__(self, handle, dims, keep=None):
+        self.handle, self.dims, self._keep = handle, dims, keep
+        n, ncand = ctypes.c_int(0), ctypes.c_int(0)
+        _check(lib().nrr_bm_plan_info(handle, ctypes.byref(n), ctypes.byref(ncand)))
+        self.n, self.ncand = n.value, ncand.value
+
+    def __del__(self):
+        try:
+            nrr_bm_plan_destroy(self)
+        except Exception:  # pragma: no cover
+            pass
+
+
+def nrr_bm_plan_create(fixed, block, stride, window, frac: float, mask=None, connectivity: int = 0, stream=None) -> NrrPlan:
+    """PRE-OPERATIVE, device form: selection + fixed-block records.  fixed / mask: CUDA tensors (fixed is kept)."""
+    import torch
+    fixed = _dev(fixed, torch.float32, "fixed")
+    if mask is not None:
+        mask = _dev(mask, torch.uint8, "mask")
+    h = ctypes.c_void_p()
+    with torch.cuda.device(fixed.device):
+        _check(lib().nrr_bm_plan_create(fixed.data_ptr(), _i3(_dims_of(fixed)), _i3(block), _i3(stride), _i3(window),
+                                        float(frac), mask.data_ptr() if mask is not None else None, int(connectivity),
+                                        _stream_ptr(stream), ctypes.byref(h)))
+    return NrrPlan(h, _dims_of(fixed), keep=fixed)
+
+
+def _host_ptr(a):
+    return None if a is None else (a.ctypes.data if isinstance(a, np.ndarray) else a.data_ptr())
+
+
+def nrr_bm_plan_create_host(fixed, block, stride, window, frac: float, mask=None, connectivity: int = 0) -> NrrPlan:
+    """PRE-OPERATIVE, host form: fixed / mask are numpy arrays or (pinned) CPU tensors; the plan owns the device copies."""
+    h = ctypes.c_void_p()
+    _check(lib().nrr_bm_plan_create_host(_host_ptr(fixed), _i3(_dims_of(fixed)), _i3(block), _i3(stride), _i3(window),
+                                         float(frac), _host_ptr(mask), int(connectivity), ctypes.byref(h)))
+    return NrrPlan(h, _dims_of(fixed))
+
+
+def nrr_bm_plan_info(plan: NrrPlan) -> Tuple[int, int]:
+    return plan.n, plan.ncand
+
+
+def nrr_bm_plan_blocks_host(plan: NrrPlan, want_var: bool = False):
+    blocks = np.empty((plan.n, 3), dtype=np.int32)
+    var = np.empty((plan.n,), dtype=np.float64) if want_var else None
+    _check(lib().nrr_bm_plan_blocks_host(plan.handle, blocks.ctypes.data, var.ctypes.data if want_var else None))
+    return (blocks, var) if want_var else blocks
+
+
+def nrr_bm_plan_match(plan: NrrPlan, moving, out_disp=None, out_ncc=None, stream=None, first: int = 0, count: Optional[int] = None):
+    """INTRA-OPERATIVE, device form, asynchronous.  With first/count: nrr_bm_plan_match_range (rows outside untouched)."""
+    import torch
+    moving = _dev(moving, torch.float32, "moving")
+    if _dims_of(moving) != tuple(plan.dims):
+        raise ValueError("volume shape mismatch")
+    if out_disp is None:
+        out_disp = torch.empty((plan.n, 3), dtype=torch.int32, device=moving.device)
+    if out_ncc is None:
+        out_ncc = torch.empty((plan.n,), dtype=torch.float32, device=moving.device)
+    with torch.cuda.device(moving.device):
+        if count is None and first == 0:
+            _check(lib().nrr_bm_plan_match(plan.handle, moving.data_ptr(), out_disp.data_ptr(), out_ncc.data_ptr(), _stream_ptr(stream)))
+        else:
+            cnt = plan.n - first if count is None else count
+            _check(lib().nrr_bm_plan_match_range(plan.handle, moving.data_ptr(), int(first), int(cnt), out_disp.data_ptr(),
+                                                 out_ncc.data_ptr(), _stream_ptr(stream)))
+    return out_disp, out_ncc
+
+
+nrr_bm_plan_match_range = nrr_bm_plan_match
+
+
+def nrr_bm_plan_match_host(plan: NrrPlan, moving, out_disp=None, out_ncc=None):
+    """INTRA-OPERATIVE, host form: moving / outputs are numpy arrays or pinned CPU tensors; synchronises."""
+    if out_disp is None:
+        out_disp = np.empty((plan.n, 3), dtype=np.int32)
+    if out_ncc is None:
+        out_ncc = np.empty((plan.n,), dtype=np.float32)
+    _check(lib().nrr_bm_plan_match_host(plan.handle, _host_ptr(moving), _host_ptr(out_disp), _host_ptr(out_ncc)))
+    return out_disp, out_ncc
+
+
+def nrr_bm_plan_destroy(plan: NrrPlan) -> None:
+    if plan.handle is not None and plan.handle.value:
+        h, plan.handle = plan.handle, None
+        _check(lib().nrr_bm_plan_destroy(h))
+    plan._keep = None
 
 
 def nrr_bm_warp(image, field, out=None, stream=None):

@@ -19,6 +19,7 @@ extern int g_disable_tma;
 extern int g_force_rows;
 extern int g_pair_g;
 extern int g_debug_tx_extra;
+extern int g_plan_slabs;
 extern int g_boxstat_generic;
 extern int g_select_generic;
 
@@ -37,6 +38,8 @@ struct DevState {
     cudaStream_t host_stream = nullptr;    // stream of the *_host entry points
     cudaStream_t side_stream = nullptr;    // nrr_bm_register: moving statistics run beside the selection
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    static constexpr int kSide = 4;
+    cudaStream_t side[kSide] = {};         // nrr_bm_register_batch / plans: matching launches spread over streams
 };
 thread_local DevState t_dev[kMaxDevices];
 thread_local void *t_pinned = nullptr;     // small pinned staging buffer (host memory: one per thread)
@@ -131,6 +134,18 @@ Int3 grid_of(const int dims[3], const int block[3], const int stride[3])
     return g;
 }
 
+// Upper bound on K = floor(0.5 + N*frac) over every N <= ngrid.  The device rounds the product and the sum
+// separately; a host compiler that contracts them into one FMA can land one lower, hence the + 1.
+long long capacity_bound(long long ngrid, double frac)
+{
+    volatile double prod = (double)ngrid * frac;
+    volatile double sum = 0.5 + prod;
+    long long k = (long long)floor(sum) + 1;
+    if (k > ngrid) k = ngrid;
+    if (k < 0) k = 0;
+    return k;
+}
+
 // Device select; returns K through *out_n after one synchronisation.
 int select_device(const float *fixed, const int dims[3], const int block[3], const int stride[3], double frac,
                   const unsigned char *mask, int *out_blocks, int capacity, int *out_n, double *out_var,
@@ -175,9 +190,12 @@ int match_device(const float *fixed, const float *moving, const int dims[3], con
     Span s1(1, stream);
     rc = boxstat_enqueue(moving, i3(dims), i3(block), inv_sd, stream);
     s1.stop();
-    if (rc == NRR_OK)
-        rc = match_enqueue(fixed, moving, inv_sd, i3(dims), blocks, n, nullptr, i3(block), i3(window), out_disp, out_ncc,
-                           t_err_flag, stream);
+    if (rc == NRR_OK) {
+        MatchCall c;
+        c.fixed = fixed; c.moving = moving; c.inv_sd = inv_sd; c.dims = i3(dims); c.block = i3(block); c.window = i3(window);
+        c.blocks = blocks; c.n = n; c.out_disp = out_disp; c.out_ncc = out_ncc; c.err_flag = t_err_flag; c.stream = stream;
+        rc = match_enqueue(c);
+    }
     return rc;
 }
 
@@ -194,10 +212,8 @@ int register_device(const float *fixed, const float *moving, const int dims[3], 
     const Int3 g = grid_of(dims, block, stride);
     const long long ngrid = (long long)g.x * g.y * g.z;
     if (ngrid > 0x7fffffffll) return fail(NRR_E_DIMS, "stride grid has %lld positions (limit 2^31-1)", ngrid);
-    // K = floor(0.5 + N*frac) with N <= ngrid candidates, so K <= floor(0.5 + ngrid*frac)
-    double kmax = floor(0.5 + (double)ngrid * frac);
-    if (kmax > (double)ngrid) kmax = (double)ngrid;
-    const int n_cap = (int)(kmax < (double)capacity ? kmax : (double)capacity);
+    const long long kmax = capacity_bound(ngrid, frac);
+    const int n_cap = (int)(kmax < (long long)capacity ? kmax : (long long)capacity);
     // The moving-volume statistics do not depend on the selection: fork them onto a side stream so that both
     // (each far from filling the GPU for long) overlap; the matching kernels join.
     AsyncScratch inv_buf(stream), sel_buf(stream);      // released in stream order on every path out of here
@@ -238,9 +254,13 @@ int register_device(const float *fixed, const float *moving, const int dims[3], 
     if (rc == NRR_OK && out_n_dev)
         rc = cudaMemcpyAsync(out_n_dev, &st->k, sizeof(int), cudaMemcpyDeviceToDevice, stream) == cudaSuccess
                  ? NRR_OK : fail(NRR_E_CUDA, "copy of K failed");
-    if (rc == NRR_OK && n_cap > 0)
-        rc = match_enqueue(fixed, moving, inv_sd, i3(dims), out_blocks, n_cap, &st->k, i3(block), i3(window),
-                           out_disp, out_ncc, t_err_flag, stream);
+    if (rc == NRR_OK && n_cap > 0) {
+        MatchCall c;
+        c.fixed = fixed; c.moving = moving; c.inv_sd = inv_sd; c.dims = i3(dims); c.block = i3(block); c.window = i3(window);
+        c.blocks = out_blocks; c.n = n_cap; c.n_dev = &st->k; c.out_disp = out_disp; c.out_ncc = out_ncc;
+        c.err_flag = t_err_flag; c.stream = stream;
+        rc = match_enqueue(c);
+    }
     return rc;
 }
 
@@ -307,6 +327,44 @@ cudaError_t scratch_alloc(void **p, size_t bytes, cudaStream_t s)
     cudaMemPool_t pool = scratch_pool();
     if (!pool) return cudaMallocAsync(p, bytes ? bytes : 1, s);
     return cudaMallocFromPoolAsync(p, bytes ? bytes : 1, pool, s);
+}
+
+// ---- helpers shared with nrr_plan.cu
+int api_fail(int code, const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(t_error, sizeof(t_error), fmt, ap);
+    va_end(ap);
+    return code;
+}
+int api_thread_state(unsigned int **err_flag, void **pinned)
+{
+    int rc = ensure_thread_state();
+    if (rc) return rc;
+    if (err_flag) *err_flag = t_err_flag;
+    if (pinned) *pinned = t_pinned;
+    return NRR_OK;
+}
+int api_host_stream(cudaStream_t *s) { return host_stream(s); }
+int api_check_async(cudaStream_t s) { return check_async(s); }
+int api_check_dims_block(const int dims[3], const int block[3]) { return check_dims_block(dims, block); }
+int api_check_select_args(const float *fixed, const int dims[3], const int block[3], const int stride[3], double frac)
+{
+    int dummy = 0;
+    return check_select_args(fixed, dims, block, stride, frac, nullptr, 0, &dummy);
+}
+long long api_capacity_bound(long long ngrid, double frac) { return capacity_bound(ngrid, frac); }
+// `count` side streams (created once per thread and device) that fork from / join into a caller's stream
+int api_side_streams(int count, cudaStream_t *out)
+{
+    DevState &d = ds();
+    if (count > DevState::kSide) count = DevState::kSide;
+    for (int i = 0; i < count; ++i) {
+        if (!d.side[i]) NRR_CUDA(cudaStreamCreateWithFlags(&d.side[i], cudaStreamNonBlocking));
+        out[i] = d.side[i];
+    }
+    return count;
 }
 
 void set_error(const char *fmt, ...)
@@ -643,6 +701,7 @@ int nrr_bm_set_option(const char *name, double value)
     if (!strcmp(name, "boxstat_generic")) { g_boxstat_generic = value != 0.0; return NRR_OK; }
     if (!strcmp(name, "force_rows")) { g_force_rows = value != 0.0; return NRR_OK; }
     if (!strcmp(name, "pair_blocks_per_cta")) { g_pair_g = (int)value; return NRR_OK; }
+    if (!strcmp(name, "plan_slabs")) { g_plan_slabs = value < 1.0 ? 1 : (int)value; return NRR_OK; }
     if (!strcmp(name, "debug_expect_tx_extra")) { g_debug_tx_extra = (int)value & ~15; return NRR_OK; }
     return fail(NRR_E_ARG, "unknown option '%s'", name);
 }

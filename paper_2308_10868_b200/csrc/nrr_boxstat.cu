@@ -26,7 +26,7 @@ constexpr int TX = 32, TY = 8, ZCHUNK = 32;
 constexpr int kThreads = TX * TY;
 
 __global__ void __launch_bounds__(kThreads)
-boxstat_kernel(const float *__restrict__ vol, Int3 dims, Int3 block, float *__restrict__ inv_sd)
+boxstat_kernel(const float *__restrict__ vol, Int3 dims, Int3 block, int zo_lo, int zo_hi, float *__restrict__ inv_sd)
 {
     NRR_DYN_SMEM(s_dyn);
     // carve: row sums (double2) | ring (double2) | plane tile (float)
@@ -36,9 +36,8 @@ boxstat_kernel(const float *__restrict__ vol, Int3 dims, Int3 block, float *__re
     float *s_plane = (float *)(s_ring + (size_t)block.z * kThreads);   // [HY][HX]
 
     const int tx = threadIdx.x % TX, ty = threadIdx.x / TX;
-    const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY, z0 = blockIdx.z * ZCHUNK;
-    const int nzo = dims.z - block.z + 1;                    // valid origins along z
-    const int zo_end = min(z0 + ZCHUNK, nzo);                // exclusive
+    const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY, z0 = zo_lo + blockIdx.z * ZCHUNK;
+    const int zo_end = min(z0 + ZCHUNK, zo_hi);              // exclusive; zo_hi <= number of valid origins along z
     const int zi_end = zo_end + block.z - 1;                 // exclusive input plane
     const double nvox = (double)((long long)block.x * block.y * block.z);
     const bool out_ok = (x0 + tx <= dims.x - block.x) && (y0 + ty <= dims.y - block.y);
@@ -121,7 +120,7 @@ struct SlideCfg {
 
 template <int B>
 __global__ void __launch_bounds__(256, 2)
-boxstat_slide_kernel(const float *__restrict__ vol, Int3 dims, int bz, int zchunk, float *__restrict__ inv_sd)
+boxstat_slide_kernel(const float *__restrict__ vol, Int3 dims, int bz, int zo_lo, int zo_hi, int zchunk, float *__restrict__ inv_sd)
 {
     using C = SlideCfg<B>;
     constexpr int TX = C::TX, TY = C::TY, HX = C::HX, HY = C::HY, NCOL = C::NCOL, ZP = C::ZP, RP = C::RP;
@@ -130,9 +129,8 @@ boxstat_slide_kernel(const float *__restrict__ vol, Int3 dims, int bz, int zchun
     double2 *s_row = s_z + (size_t)HY * ZP;      // [TX][RP]  x-window sums, transposed
 
     const int tid = threadIdx.x;
-    const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY, z0 = blockIdx.z * zchunk;
-    const int nzo = dims.z - bz + 1;
-    const int zo_end = min(z0 + zchunk, nzo);
+    const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY, z0 = zo_lo + blockIdx.z * zchunk;
+    const int zo_end = min(z0 + zchunk, zo_hi);
     if (z0 >= zo_end) return;                    // uniform over the CTA
     const int zi_end = zo_end + bz - 1;
     const size_t plane = (size_t)dims.x * dims.y;
@@ -220,10 +218,10 @@ boxstat_slide_kernel(const float *__restrict__ vol, Int3 dims, int bz, int zchun
 }
 
 template <int B>
-int launch_slide(const float *moving, Int3 dims, int bz, float *inv_sd, cudaStream_t stream)
+int launch_slide(const float *moving, Int3 dims, int bz, float *inv_sd, int zo_lo, int zo_hi, cudaStream_t stream)
 {
     using C = SlideCfg<B>;
-    const int nxo = dims.x - B + 1, nyo = dims.y - B + 1, nzo = dims.z - bz + 1;
+    const int nxo = dims.x - B + 1, nyo = dims.y - B + 1, nzo = zo_hi - zo_lo;
     const int gx = (nxo + C::TX - 1) / C::TX, gy = (nyo + C::TY - 1) / C::TY;
     // enough CTAs for two per SM; chunks of at least 2B planes keep the z halo below 50 %
     int zsplit = (2 * 148 + gx * gy - 1) / (gx * gy);
@@ -243,7 +241,7 @@ int launch_slide(const float *moving, Int3 dims, int bz, float *inv_sd, cudaStre
         NRR_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM));
         conf = true;
     }
-    NRR_LAUNCH(kern, dim3(gx, gy, zsplit), C::NT, C::SMEM, stream, moving, dims, bz, zchunk, inv_sd);
+    NRR_LAUNCH(kern, dim3(gx, gy, zsplit), C::NT, C::SMEM, stream, moving, dims, bz, zo_lo, zo_hi, zchunk, inv_sd);
     NRR_LAUNCH_CHECK("boxstat_slide_kernel");
     return NRR_OK;
 }
@@ -252,14 +250,22 @@ int launch_slide(const float *moving, Int3 dims, int bz, float *inv_sd, cudaStre
 
 int boxstat_enqueue(const float *moving, Int3 dims, Int3 block, float *inv_sd, cudaStream_t stream)
 {
-    const int nxo = dims.x - block.x + 1, nyo = dims.y - block.y + 1, nzo = dims.z - block.z + 1;
+    return boxstat_enqueue_range(moving, dims, block, inv_sd, 0, dims.z - block.z + 1, stream);
+}
+
+int boxstat_enqueue_range(const float *moving, Int3 dims, Int3 block, float *inv_sd, int zo_lo, int zo_hi, cudaStream_t stream)
+{
+    const int nxo = dims.x - block.x + 1, nyo = dims.y - block.y + 1;
+    if (zo_lo < 0) zo_lo = 0;
+    if (zo_hi > dims.z - block.z + 1) zo_hi = dims.z - block.z + 1;
+    const int nzo = zo_hi - zo_lo;
     if (nxo < 1 || nyo < 1 || nzo < 1) return NRR_OK;
     if (!g_boxstat_generic && block.x == block.y) {      // in-plane square, any extent along z
         switch (block.x) {
-        case 5: return launch_slide<5>(moving, dims, block.z, inv_sd, stream);
-        case 7: return launch_slide<7>(moving, dims, block.z, inv_sd, stream);
-        case 9: return launch_slide<9>(moving, dims, block.z, inv_sd, stream);
-        case 11: return launch_slide<11>(moving, dims, block.z, inv_sd, stream);
+        case 5: return launch_slide<5>(moving, dims, block.z, inv_sd, zo_lo, zo_hi, stream);
+        case 7: return launch_slide<7>(moving, dims, block.z, inv_sd, zo_lo, zo_hi, stream);
+        case 9: return launch_slide<9>(moving, dims, block.z, inv_sd, zo_lo, zo_hi, stream);
+        case 11: return launch_slide<11>(moving, dims, block.z, inv_sd, zo_lo, zo_hi, stream);
         default: break;
         }
     }
@@ -276,7 +282,7 @@ int boxstat_enqueue(const float *moving, Int3 dims, Int3 block, float *inv_sd, c
         set_error("volume too large for the moving-volume statistics grid");
         return NRR_E_DIMS;
     }
-    NRR_LAUNCH(boxstat_kernel, grid, kThreads, smem, stream, moving, dims, block, inv_sd);
+    NRR_LAUNCH(boxstat_kernel, grid, kThreads, smem, stream, moving, dims, block, zo_lo, zo_hi, inv_sd);
     NRR_LAUNCH_CHECK("boxstat_kernel");
     return NRR_OK;
 }

@@ -28,6 +28,16 @@ void count_launch(int n = 1);
 void profile_begin(int phase, cudaStream_t stream);
 void profile_end(int phase, cudaStream_t stream);
 
+// helpers of the C boundary shared by nrr_api.cu and nrr_plan.cu
+int api_fail(int code, const char *fmt, ...);                       // records the message, returns code
+int api_thread_state(unsigned int **err_flag, void **pinned);      // per-thread / per-device state (4 KB pinned buffer)
+int api_host_stream(cudaStream_t *s);                              // stream of the *_host entry points
+int api_check_async(cudaStream_t s);                               // nrr_bm_check_async_error
+int api_check_dims_block(const int dims[3], const int block[3]);
+int api_check_select_args(const float *fixed, const int dims[3], const int block[3], const int stride[3], double frac);
+long long api_capacity_bound(long long ngrid, double frac);
+int api_side_streams(int count, cudaStream_t *out);                // returns how many it provides (<= count)
+
 #define NRR_CUDA(call)                                              \
     do {                                                            \
         cudaError_t e__ = (call);                                   \
@@ -88,10 +98,19 @@ int select_enqueue(const float *fixed, Int3 dims, Int3 block, Int3 stride, Int3 
                    void *scratch, SelectState **state_out, cudaStream_t stream, int connectivity = 0,
                    SelectState *host_poll = nullptr);
 
+// Another selection on the keys a select_enqueue call left in `scratch` (same image, block, stride, mask; no
+// connectivity pattern), for another fraction: K, the digit picks and the compaction only.  `st`: 256 device bytes.
+bool select_can_share_keys(long long ngrid);
+int select_more_enqueue(void *scratch, Int3 block, Int3 stride, Int3 grid, double frac, int *out_blocks, int capacity,
+                        double *out_var, SelectState *st, cudaStream_t stream);
+
 // ---- moving-volume statistics (nrr_boxstat.cu) ------------------------------------------------------
 // inv_sd[p] = 1/sqrt(sum over the block with ORIGIN p of (m - mean)^2), 0 for zero-variance blocks,
 // for every origin p whose block fits in the volume; other entries are left untouched.
 int boxstat_enqueue(const float *moving, Int3 dims, Int3 block, float *inv_sd, cudaStream_t stream);
+// The same for the block origins with z in [zo_lo, zo_hi) only (reads the planes zo_lo .. zo_hi + block.z - 2): a caller
+// that uploads the volume slab by slab computes the normalisers of each slab as it lands.
+int boxstat_enqueue_range(const float *moving, Int3 dims, Int3 block, float *inv_sd, int zo_lo, int zo_hi, cudaStream_t stream);
 
 // ---- matching (nrr_match.cu) ------------------------------------------------------------------------
 struct MatchPlan {
@@ -104,17 +123,33 @@ struct MatchPlan {
 };
 int match_plan(Int3 dims, Int3 block, Int3 window, const void *moving_ptr, const void *fixed_ptr,
                MatchPlan *plan);
-// n_dev (nullable, DEVICE): the number of blocks is min(n, *n_dev), read by the kernels themselves, so a caller
-// that only knows an upper bound n on the host (selection still in flight) needs no synchronisation.
-int match_enqueue(const float *fixed, const float *moving, const float *inv_sd, Int3 dims, const int *blocks,
-                  int n, const unsigned int *n_dev, Int3 block, Int3 window, int *out_disp, float *out_ncc,
-                  unsigned int *err_flag, cudaStream_t stream);
-extern thread_local const unsigned int *t_match_n_dev;      // set by match_enqueue for the launchers
+
+// One matching launch sequence.  The pair kernel works from per-block RECORDS of the fixed image (centred block, pair
+// table, 1/sqrt(SS_f): everything that needs only the pre-operative image); a caller that keeps
+// them across calls (a plan) passes `records` and enqueues the two phases separately.
+enum MatchPhase { kMatchBoth = 0, kMatchPrepOnly = 1, kMatchKernelOnly = 2 };
+struct MatchCall {
+    const float *fixed = nullptr, *moving = nullptr, *inv_sd = nullptr;
+    Int3 dims{}, block{}, window{};
+    const int *blocks = nullptr;       // [n][3] centres
+    int n = 0;
+    // n_dev (nullable, DEVICE): the number of blocks is min(n, *n_dev), read by the kernels themselves, so a caller
+    // that only knows an upper bound n on the host (selection still in flight) needs no synchronisation.
+    const unsigned int *n_dev = nullptr;
+    int *out_disp = nullptr;
+    float *out_ncc = nullptr;
+    unsigned int *err_flag = nullptr;
+    float *records = nullptr;          // match_records_bytes(block, window, n) bytes; NULL with kMatchBoth = call scratch
+    MatchPhase phase = kMatchBoth;
+    cudaStream_t stream = nullptr;
+};
+int match_enqueue(const MatchCall &c);
+// Bytes of fixed-block records the kernel for this shape wants for n blocks (0: that kernel keeps no records).
+size_t match_records_bytes(Int3 block, Int3 window, int n);
 
 // nrr_match_pair.cu: tries the pair kernel; *handled tells whether it took the call.
-int match_pair_dispatch(const float *fixed, const float *moving, const float *inv_sd, Int3 dims, const int *blocks,
-                        int n, Int3 block, Int3 window, int *out_disp, float *out_ncc, unsigned int *err_flag,
-                        cudaStream_t stream, MatchPlan *plan_only, bool *handled);
+int match_pair_dispatch(const MatchCall &c, MatchPlan *plan_only, bool *handled);
+size_t match_pair_records_bytes(Int3 block, Int3 window, int n);
 
 int match_pair_table(Int3 block, Int3 window, unsigned int *out, int capacity, int info[6]);
 

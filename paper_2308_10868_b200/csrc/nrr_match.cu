@@ -32,7 +32,6 @@ namespace nrr {
 float g_tie_band = 1e-4f;     // FP32 candidates this close to the FP32 maximum are re-scored in FP64
 int g_force_generic = 0;
 int g_disable_tma = 0;
-thread_local const unsigned int *t_match_n_dev = nullptr;
 int g_force_rows = 0;          // != 0: skip the pair kernel (one candidate row per thread instead)
 
 namespace {
@@ -389,10 +388,13 @@ bool tma_eligible(Int3 dims, const void *moving, int box_z)
 namespace {
 
 template <int B, int R>
-int launch_fast(const float *fixed, const float *moving, const float *inv_sd, Int3 dims, const int *blocks, int n,
-                int rz, int *out_disp, float *out_ncc, unsigned int *err_flag, cudaStream_t stream, MatchPlan *plan_only)
+int launch_fast(const MatchCall &c, MatchPlan *plan_only)
 {
     using C = FastCfg<B, R>;
+    const Int3 dims = c.dims;
+    const float *moving = c.moving;
+    const int rz = c.window.z, n = c.n;
+    cudaStream_t stream = c.stream;
     const int nrows = C::W * (2 * rz + 1);
     const int threads = (nrows + 31) / 32 * 32;
     const size_t smem = fast_smem_bytes<B, R>(rz);
@@ -416,8 +418,8 @@ int launch_fast(const float *fixed, const float *moving, const float *inv_sd, In
         conf = (int)smem;
     }
     profile_begin(2, stream);
-    NRR_LAUNCH(kern, n, threads, smem, stream, tm_m, use_tma, fixed, moving, inv_sd, dims, blocks, rz, g_tie_band,
-               out_disp, out_ncc, err_flag, t_match_n_dev);
+    NRR_LAUNCH(kern, n, threads, smem, stream, tm_m, use_tma, c.fixed, moving, c.inv_sd, dims, c.blocks, rz, g_tie_band,
+               c.out_disp, c.out_ncc, c.err_flag, c.n_dev);
     profile_end(2, stream);
     NRR_LAUNCH_CHECK("match_rows_kernel");
     return NRR_OK;
@@ -426,16 +428,14 @@ int launch_fast(const float *fixed, const float *moving, const float *inv_sd, In
 constexpr size_t kMaxSmem = 227 * 1024;
 
 template <int B>
-int dispatch_r(int r, const float *fixed, const float *moving, const float *inv_sd, Int3 dims, const int *blocks,
-               int n, int rz, int *out_disp, float *out_ncc, unsigned int *err_flag, cudaStream_t stream,
-               MatchPlan *plan_only, bool *handled)
+int dispatch_r(const MatchCall &c, MatchPlan *plan_only, bool *handled)
 {
+    const int r = c.window.x, rz = c.window.z;
     *handled = true;
 #define NRR_CASE(RR)                                                                                              \
     case RR:                                                                                                      \
         if (FastCfg<B, RR>::W * (2 * rz + 1) <= kFastMaxThreads && fast_smem_bytes<B, RR>(rz) <= kMaxSmem)                   \
-            return launch_fast<B, RR>(fixed, moving, inv_sd, dims, blocks, n, rz, out_disp, out_ncc, err_flag,    \
-                                      stream, plan_only);                                                         \
+            return launch_fast<B, RR>(c, plan_only);                                                              \
         break;
     switch (r) {
         NRR_CASE(3)
@@ -450,26 +450,27 @@ int dispatch_r(int r, const float *fixed, const float *moving, const float *inv_
     return NRR_OK;
 }
 
-int dispatch(const float *fixed, const float *moving, const float *inv_sd, Int3 dims, const int *blocks, int n,
-             Int3 block, Int3 window, int *out_disp, float *out_ncc, unsigned int *err_flag, cudaStream_t stream,
-             MatchPlan *plan_only)
+int dispatch(const MatchCall &c, MatchPlan *plan_only)
 {
+    const Int3 block = c.block, window = c.window;
+    const int n = c.n;
+    cudaStream_t stream = c.stream;
     const long long ncand = (long long)(2 * window.x + 1) * (2 * window.y + 1) * (2 * window.z + 1);
     if (plan_only) plan_only->candidates = (int)(ncand > 0x7fffffff ? 0x7fffffff : ncand);
     bool handled = false;
     if (plan_only) plan_only->blocks_per_cta = 1;
     if (!g_force_generic && !g_force_rows) {
-        const int rc = match_pair_dispatch(fixed, moving, inv_sd, dims, blocks, n, block, window, out_disp, out_ncc,
-                                           err_flag, stream, plan_only, &handled);
+        const int rc = match_pair_dispatch(c, plan_only, &handled);
         if (rc != NRR_OK || handled) return rc;
     }
+    if (c.phase == kMatchPrepOnly) return NRR_OK;      // only the pair kernel keeps fixed-block records
     if (!g_force_generic && block.x == block.y && block.y == block.z && window.x == window.y) {
         int rc = NRR_OK;
         switch (block.x) {
-        case 5: rc = dispatch_r<5>(window.x, fixed, moving, inv_sd, dims, blocks, n, window.z, out_disp, out_ncc, err_flag, stream, plan_only, &handled); break;
-        case 7: rc = dispatch_r<7>(window.x, fixed, moving, inv_sd, dims, blocks, n, window.z, out_disp, out_ncc, err_flag, stream, plan_only, &handled); break;
-        case 9: rc = dispatch_r<9>(window.x, fixed, moving, inv_sd, dims, blocks, n, window.z, out_disp, out_ncc, err_flag, stream, plan_only, &handled); break;
-        case 11: rc = dispatch_r<11>(window.x, fixed, moving, inv_sd, dims, blocks, n, window.z, out_disp, out_ncc, err_flag, stream, plan_only, &handled); break;
+        case 5: rc = dispatch_r<5>(c, plan_only, &handled); break;
+        case 7: rc = dispatch_r<7>(c, plan_only, &handled); break;
+        case 9: rc = dispatch_r<9>(c, plan_only, &handled); break;
+        case 11: rc = dispatch_r<11>(c, plan_only, &handled); break;
         default: break;
         }
         if (handled) return rc;
@@ -496,8 +497,8 @@ int dispatch(const float *fixed, const float *moving, const float *inv_sd, Int3 
         conf = (int)smem;
     }
     profile_begin(2, stream);
-    NRR_LAUNCH(match_generic_kernel, n, 128, smem, stream, fixed, moving, inv_sd, dims, blocks, block, window,
-               g_tie_band, out_disp, out_ncc, err_flag, t_match_n_dev);
+    NRR_LAUNCH(match_generic_kernel, n, 128, smem, stream, c.fixed, c.moving, c.inv_sd, c.dims, c.blocks, block, window,
+               g_tie_band, c.out_disp, c.out_ncc, c.err_flag, c.n_dev);
     profile_end(2, stream);
     NRR_LAUNCH_CHECK("match_generic_kernel");
     return NRR_OK;
@@ -507,19 +508,23 @@ int dispatch(const float *fixed, const float *moving, const float *inv_sd, Int3 
 
 int match_plan(Int3 dims, Int3 block, Int3 window, const void *moving_ptr, const void *fixed_ptr, MatchPlan *plan)
 {
-    return dispatch((const float *)fixed_ptr, (const float *)moving_ptr, nullptr, dims, nullptr, 0, block, window,
-                    nullptr, nullptr, nullptr, nullptr, plan);
+    MatchCall c;
+    c.fixed = (const float *)fixed_ptr;
+    c.moving = (const float *)moving_ptr;
+    c.dims = dims; c.block = block; c.window = window;
+    return dispatch(c, plan);
 }
 
-int match_enqueue(const float *fixed, const float *moving, const float *inv_sd, Int3 dims, const int *blocks, int n,
-                  const unsigned int *n_dev, Int3 block, Int3 window, int *out_disp, float *out_ncc,
-                  unsigned int *err_flag, cudaStream_t stream)
+int match_enqueue(const MatchCall &c)
 {
-    if (n == 0) return NRR_OK;
-    t_match_n_dev = n_dev;
-    const int rc = dispatch(fixed, moving, inv_sd, dims, blocks, n, block, window, out_disp, out_ncc, err_flag, stream, nullptr);
-    t_match_n_dev = nullptr;
-    return rc;
+    if (c.n == 0) return NRR_OK;
+    return dispatch(c, nullptr);
+}
+
+size_t match_records_bytes(Int3 block, Int3 window, int n)
+{
+    if (g_force_generic || g_force_rows) return 0;
+    return match_pair_records_bytes(block, window, n);
 }
 
 }  // namespace nrr

@@ -77,6 +77,7 @@ struct PairCfg {
     __host__ __device__ static constexpr int rec_floats(int bz) { return plain_floats(bz) + pair_floats(bz) + HDR_FLOATS; }
     __host__ __device__ static constexpr int rec_bytes(int bz) { return rec_floats(bz) * 4; }      // multiple of 16
     static_assert(FP % 4 == 0 && FPP % 4 == 0 && HDR_FLOATS % 4 == 0, "records are moved by 16-byte bulk copies");
+    static constexpr int B_ROW_BYTES = FP * 4;          // one staged row of the centred block
     static_assert(PITCH >= NV * 4, "row pitch must cover the vector loads");
 };
 
@@ -158,8 +159,7 @@ constexpr int kMaxBZ = 11;          // largest block extent along z the pair ker
 template <int B, int R>
 __global__ void __launch_bounds__(kPrepWarps * 32)
 prep_kernel(const float *__restrict__ fixed, Int3 dims, const int *__restrict__ blocks, int n, int bz,
-            const unsigned int *__restrict__ n_dev, float *__restrict__ records, int *__restrict__ out_disp,
-            float *__restrict__ out_ncc, unsigned int *err_flag)
+            const unsigned int *__restrict__ n_dev, float *__restrict__ records)
 {
     if (n_dev) n = min(n, (int)*n_dev);               // the launch was sized for an upper bound
     using C = PairCfg<B, R>;
@@ -174,14 +174,7 @@ prep_kernel(const float *__restrict__ fixed, Int3 dims, const int *__restrict__ 
     const int ox = blocks[3 * (size_t)b + 0] - (B - 1) / 2;
     const int oy = blocks[3 * (size_t)b + 1] - (B - 1) / 2;
     const int oz = blocks[3 * (size_t)b + 2] - (bz - 1) / 2;
-    if (!block_in_volume(dims, Int3{B, B, bz}, ox, oy, oz)) {      // uniform over the warp
-        if (lane == 0) {
-            out_disp[3 * (size_t)b + 0] = 0;
-            out_disp[3 * (size_t)b + 1] = 0;
-            out_disp[3 * (size_t)b + 2] = 0;
-            out_ncc[b] = __int_as_float(0x7fc00000);
-            atomicOr(err_flag, 1u);
-        }
+    if (!block_in_volume(dims, Int3{B, B, bz}, ox, oy, oz)) {      // uniform over the warp; the matching kernel reports it
         for (int i = lane; i < REC_FLOATS; i += 32) rec[i] = 0.f;      // header: isd_f = 0, valid = 0
         return;
     }
@@ -519,7 +512,10 @@ match_pair_kernel(const __grid_constant__ CUtensorMap tm_moving, const PairArgs 
     const Int3 block = {B, B, bz}, window = {R, R, rz};
     for (int gg = 0; gg < gact; ++gg) {
         const int4 o = ctrl->org[gg];
-        if (!o.w) continue;                              // flagged by the prep kernel
+        if (!o.w) {                                      // the block leaves the volume: NaN + sticky flag (NRR_E_BOUNDS)
+            write_bounds_error(ctrl->bidx[gg], a.out_disp, a.out_ncc, a.err_flag);
+            continue;
+        }
         const u64 best = ctrl->best[gg];
         const int big = (int)(0xffffffffu - (uint32_t)best);
         const int cnt = ctrl->count[gg];
@@ -665,6 +661,7 @@ std::vector<uint32_t> build_task_table(int rz, const PairGeom &g)
 
 std::mutex g_tab_mutex;
 std::map<long long, uint32_t *> g_tab_cache;      // (device, B, R, rz, G) -> device table
+std::map<long long, cudaEvent_t> g_tab_ready;     // ... and the event behind its upload
 
 template <int B, int R>
 int task_table_device(int rz, const PairGeom &g, cudaStream_t stream, const uint32_t **out)
@@ -674,24 +671,40 @@ int task_table_device(int rz, const PairGeom &g, cudaStream_t stream, const uint
     const long long key = ((((long long)dev * 32 + B) * 32 + R) * 512 + rz) * 16 + g.G;      // the table does not depend on bz
     std::lock_guard<std::mutex> lock(g_tab_mutex);
     auto it = g_tab_cache.find(key);
-    if (it != g_tab_cache.end()) { *out = it->second; return NRR_OK; }
+    if (it != g_tab_cache.end()) {
+        cudaEvent_t &ready = g_tab_ready[key];
+        if (ready) {      // the upload may still be in flight on another stream
+            if (cudaEventQuery(ready) == cudaSuccess) { cudaEventDestroy(ready); ready = nullptr; }
+            else { (void)cudaGetLastError(); NRR_CUDA(cudaStreamWaitEvent(stream, ready, 0)); }
+        }
+        *out = it->second;
+        return NRR_OK;
+    }
     const std::vector<uint32_t> tab = build_task_table<B, R>(rz, g);
-    uint32_t *d = nullptr;
+    // First use of this (device, shape): the table goes up from a pinned copy that lives as long as the cache entry,
+    // in stream order -- no host synchronisation (nrr_bm_register promises none).  Later calls on OTHER streams may
+    // race this first copy in principle; they are ordered by the event recorded behind it.
+    uint32_t *d = nullptr, *h = nullptr;
     NRR_CUDA(cudaMalloc((void **)&d, tab.size() * sizeof(uint32_t)));
-    // pageable source: the copy is staged before the call returns, so `tab` may go out of scope
-    NRR_CUDA(cudaMemcpyAsync(d, tab.data(), tab.size() * sizeof(uint32_t), cudaMemcpyHostToDevice, stream));
-    NRR_CUDA(cudaStreamSynchronize(stream));
+    NRR_CUDA(cudaMallocHost((void **)&h, tab.size() * sizeof(uint32_t)));
+    memcpy(h, tab.data(), tab.size() * sizeof(uint32_t));
+    NRR_CUDA(cudaMemcpyAsync(d, h, tab.size() * sizeof(uint32_t), cudaMemcpyHostToDevice, stream));
+    cudaEvent_t ready = nullptr;
+    NRR_CUDA(cudaEventCreateWithFlags(&ready, cudaEventDisableTiming));
+    NRR_CUDA(cudaEventRecord(ready, stream));
+    g_tab_ready[key] = ready;
     g_tab_cache[key] = d;
     *out = d;
     return NRR_OK;
 }
 
 template <int B, int R>
-int launch_pair(const float *fixed, const float *moving, const float *inv_sd, Int3 dims, const int *blocks, int n,
-                int rz, int bz, int *out_disp, float *out_ncc, unsigned int *err_flag, cudaStream_t stream,
-                MatchPlan *plan_only, bool *handled)
+int launch_pair(const MatchCall &c, MatchPlan *plan_only, bool *handled)
 {
     using C = PairCfg<B, R>;
+    const Int3 dims = c.dims;
+    const int rz = c.window.z, bz = c.block.z, n = c.n;
+    cudaStream_t stream = c.stream;
     *handled = false;
     PairGeom g;
     if (bz < 1 || bz > kMaxBZ || !pair_plan<B, R>(rz, bz, &g)) return NRR_OK;
@@ -704,22 +717,37 @@ int launch_pair(const float *fixed, const float *moving, const float *inv_sd, In
         plan_only->blocks_per_cta = g.G;
         return NRR_OK;
     }
+    *handled = true;
+    AsyncScratch rec_buf(stream);
+    float *records = c.records;
+    if (!records) {
+        if (c.phase != kMatchBoth) { set_error("the matching phases run separately only on caller-kept records"); return NRR_E_ARG; }
+        NRR_CUDA(rec_buf.alloc((size_t)n * C::rec_bytes(bz)));
+        records = (float *)rec_buf.p;
+    }
+    if (c.phase != kMatchKernelOnly) {
+        auto prep = prep_kernel<B, R>;
+        profile_begin(3, stream);
+        NRR_LAUNCH(prep, (n + kPrepWarps - 1) / kPrepWarps, kPrepWarps * 32, 0, stream, c.fixed, dims, c.blocks, n, bz, c.n_dev, records);
+        profile_end(3, stream);
+        NRR_LAUNCH_CHECK("prep_kernel");
+        if (c.phase == kMatchPrepOnly) return NRR_OK;
+    }
+    // ---- what the copy engines need, checked on the host: a mis-programmed copy is refused here, never launched
+    static_assert(C::PITCH % 4 == 0 && C::PITCH <= 256 && C::UX <= 256, "TMA box: inner extent a multiple of 16 bytes, extents <= 256");
+    static_assert(C::rec_bytes(1) % 16 == 0 && (C::B_ROW_BYTES % 16) == 0, "bulk copies move multiples of 16 bytes");
     CUtensorMap tm_m;
     memset(&tm_m, 0, sizeof(tm_m));
-    const int use_tma = tma_eligible(dims, moving, bz + 2 * rz) && make_volume_map(&tm_m, moving, dims, C::PITCH, C::UX, bz + 2 * rz);
-    *handled = true;
+    const int use_tma = tma_eligible(dims, c.moving, bz + 2 * rz) && make_volume_map(&tm_m, c.moving, dims, C::PITCH, C::UX, bz + 2 * rz);
+    if (g.union_stride % 128 != 0 || ((size_t)g.G * g.union_stride) % 16 != 0 || ((uintptr_t)records & 15) != 0 ||
+        C::rec_bytes(bz) % 16 != 0 || (size_t)g.union_stride < sizeof(float) * (size_t)(bz + 2 * rz) * C::UX * C::PITCH) {
+        set_error("pair kernel: staging layout violates the copy engines' alignment rules (union stride %d, record %d B)",
+                  g.union_stride, C::rec_bytes(bz));
+        return NRR_E_ARG;
+    }
     const uint32_t *tab = nullptr;
     int rc = task_table_device<B, R>(rz, g, stream, &tab);
     if (rc) return rc;
-    AsyncScratch rec_buf(stream);
-    NRR_CUDA(rec_buf.alloc((size_t)n * C::rec_bytes(bz)));
-    float *records = (float *)rec_buf.p;
-    auto prep = prep_kernel<B, R>;
-    profile_begin(3, stream);
-    NRR_LAUNCH(prep, (n + kPrepWarps - 1) / kPrepWarps, kPrepWarps * 32, 0, stream, fixed, dims, blocks, n, bz,
-               t_match_n_dev, records, out_disp, out_ncc, err_flag);
-    profile_end(3, stream);
-    NRR_LAUNCH_CHECK("prep_kernel");
     auto kern = match_pair_kernel<B, R>;
     static size_t configured_smem[kMaxDevices] = {};     // per instantiation and device
     size_t &conf = configured_smem[current_device()];
@@ -730,16 +758,24 @@ int launch_pair(const float *fixed, const float *moving, const float *inv_sd, In
         conf = g.smem;
     }
     PairArgs a;
-    a.fixed = fixed; a.moving = moving; a.inv_sd = inv_sd; a.records = records; a.blocks = blocks; a.task_tab = tab;
-    a.out_disp = out_disp; a.out_ncc = out_ncc; a.dims = dims; a.n = n; a.rz = rz; a.bz = bz; a.G = g.G; a.n_dev = t_match_n_dev;
+    a.fixed = c.fixed; a.moving = c.moving; a.inv_sd = c.inv_sd; a.records = records; a.blocks = c.blocks; a.task_tab = tab;
+    a.out_disp = c.out_disp; a.out_ncc = c.out_ncc; a.dims = dims; a.n = n; a.rz = rz; a.bz = bz; a.G = g.G; a.n_dev = c.n_dev;
     a.use_tma = use_tma;
     a.n_pair_warps = g.n_pair_warps; a.union_stride = g.union_stride; a.tie_band = g_tie_band;
-    a.err_flag = err_flag; a.debug_tx_extra = (unsigned int)g_debug_tx_extra;
+    a.err_flag = c.err_flag; a.debug_tx_extra = (unsigned int)g_debug_tx_extra;
     profile_begin(2, stream);
     NRR_LAUNCH(kern, (n + g.G - 1) / g.G, g.threads, g.smem, stream, tm_m, a);
     profile_end(2, stream);
     NRR_LAUNCH_CHECK("match_pair_kernel");
-    return NRR_OK;      // the scratch is released behind the kernels, in stream order
+    return NRR_OK;      // call scratch is released behind the kernels, in stream order
+}
+
+template <int B, int R>
+size_t records_bytes_for(int rz, int bz, int n)
+{
+    PairGeom g;
+    if (bz < 1 || bz > kMaxBZ || !pair_plan<B, R>(rz, bz, &g)) return 0;
+    return (size_t)n * PairCfg<B, R>::rec_bytes(bz);
 }
 
 template <int B, int R>
@@ -774,22 +810,32 @@ int match_pair_table(Int3 block, Int3 window, unsigned int *out, int capacity, i
 
 // Tries the pair kernel; *handled tells whether it took the call (blocks B x B x bz with B in 5/7/9/11 and any odd
 // bz <= 11 -- thick-slice MRI wants e.g. 7 x 7 x 3 --, in-plane window 3/5/7/9 equal in x and y, any window in z).
-int match_pair_dispatch(const float *fixed, const float *moving, const float *inv_sd, Int3 dims, const int *blocks, int n,
-                        Int3 block, Int3 window, int *out_disp, float *out_ncc, unsigned int *err_flag,
-                        cudaStream_t stream, MatchPlan *plan_only, bool *handled)
+int match_pair_dispatch(const MatchCall &c, MatchPlan *plan_only, bool *handled)
 {
     *handled = false;
+    const Int3 block = c.block, window = c.window;
     if (!(block.x == block.y && window.x == window.y)) return NRR_OK;
-#define NRR_PAIR(BB, RR)                                                                                           \
-    if (block.x == BB && window.x == RR)                                                                           \
-        return launch_pair<BB, RR>(fixed, moving, inv_sd, dims, blocks, n, window.z, block.z, out_disp, out_ncc,  \
-                                   err_flag, stream, plan_only, handled);
+#define NRR_PAIR(BB, RR) \
+    if (block.x == BB && window.x == RR) return launch_pair<BB, RR>(c, plan_only, handled);
     NRR_PAIR(5, 3) NRR_PAIR(5, 5) NRR_PAIR(5, 7) NRR_PAIR(5, 9)
     NRR_PAIR(7, 3) NRR_PAIR(7, 5) NRR_PAIR(7, 7) NRR_PAIR(7, 9)
     NRR_PAIR(9, 3) NRR_PAIR(9, 5) NRR_PAIR(9, 7) NRR_PAIR(9, 9)
     NRR_PAIR(11, 3) NRR_PAIR(11, 5) NRR_PAIR(11, 7) NRR_PAIR(11, 9)
 #undef NRR_PAIR
     return NRR_OK;
+}
+
+size_t match_pair_records_bytes(Int3 block, Int3 window, int n)
+{
+    if (!(block.x == block.y && window.x == window.y)) return 0;
+#define NRR_PAIR(BB, RR) \
+    if (block.x == BB && window.x == RR) return records_bytes_for<BB, RR>(window.z, block.z, n);
+    NRR_PAIR(5, 3) NRR_PAIR(5, 5) NRR_PAIR(5, 7) NRR_PAIR(5, 9)
+    NRR_PAIR(7, 3) NRR_PAIR(7, 5) NRR_PAIR(7, 7) NRR_PAIR(7, 9)
+    NRR_PAIR(9, 3) NRR_PAIR(9, 5) NRR_PAIR(9, 7) NRR_PAIR(9, 9)
+    NRR_PAIR(11, 3) NRR_PAIR(11, 5) NRR_PAIR(11, 7) NRR_PAIR(11, 9)
+#undef NRR_PAIR
+    return 0;
 }
 
 }  // namespace nrr

@@ -466,6 +466,25 @@ select_small_kernel(const double *__restrict__ var, long long ngrid, Int3 block,
     }
 }
 
+// A further selection on the SAME keys (same image, block, stride, mask) with another fraction: the variances and the
+// pass-0 histogram do not depend on the fraction, so only K, the digit picks and the compaction are redone.
+__global__ void __launch_bounds__(256)
+select_begin_kernel(const unsigned int *hist0, const SelectState *st0, SelectState *st, double frac)
+{
+    if (threadIdx.x == 0) {
+        const unsigned int n = st0->n_candidates;
+        double kd = floor(__dadd_rn(0.5, __dmul_rn((double)n, frac)));      // the same rounded operations as stats_kernel
+        unsigned int kk = kd <= 0.0 ? 0u : (kd >= (double)n ? n : (unsigned int)kd);
+        st->n_candidates = n;
+        st->k = kk;
+        st->k_remaining = kk;
+        st->prefix = 0ull;
+        st->mask = 0ull;
+    }
+    __syncthreads();
+    pick_digit(hist0, st, 0);
+}
+
 // ---- connectivity pruning (reading Q20): the greedy walk by (variance desc, index asc) that keeps a
 // candidate iff no kept candidate is among its pattern neighbours on the candidate grid.  A candidate's fate
 // depends only on its HIGHER-priority neighbours, so the walk is the unique fixed point of a local rule that all
@@ -566,6 +585,27 @@ ScratchLayout layout(long long ngrid)
 }  // namespace
 
 size_t select_scratch_bytes(long long ngrid) { return layout(ngrid).total; }
+
+bool select_can_share_keys(long long ngrid) { return !g_select_generic && ngrid > 0 && ngrid <= kSmallLimit; }
+
+int select_more_enqueue(void *scratch, Int3 block, Int3 stride, Int3 grid, double frac, int *out_blocks, int capacity,
+                        double *out_var, SelectState *st, cudaStream_t stream)
+{
+    const long long ngrid = (long long)grid.x * grid.y * grid.z;
+    if (!select_can_share_keys(ngrid)) { set_error("the keys of this grid cannot be shared between selections"); return NRR_E_ARG; }
+    const ScratchLayout L = layout(ngrid);
+    char *base = (char *)scratch;
+    const SelectState *st0 = (const SelectState *)(base + L.state);
+    const unsigned int *hist0 = (const unsigned int *)(base + L.hist);
+    const double *var = (const double *)(base + L.var);
+    NRR_CUDA(cudaMemsetAsync(st, 0, sizeof(SelectState), stream));
+    NRR_LAUNCH(select_begin_kernel, 1, 256, 0, stream, hist0, st0, st, frac);
+    NRR_LAUNCH_CHECK("select_begin_kernel");
+    NRR_LAUNCH(select_small_kernel, 1, kSmallThreads, 0, stream, var, ngrid, block, stride, grid, st, out_blocks, out_var,
+               capacity, 1);
+    NRR_LAUNCH_CHECK("select_small_kernel");
+    return NRR_OK;
+}
 
 int select_enqueue(const float *fixed, Int3 dims, Int3 block, Int3 stride, Int3 grid, double frac,
                    const unsigned char *mask, int *out_blocks, int capacity, double *out_var, void *scratch,

@@ -115,3 +115,102 @@ def warp(image, field):
     out = np.empty_like(image)
     _check(lib().nrr_bm_warp_host(image.ctypes.data, _i3((nx, ny, nz)), field.ctypes.data, out.ctypes.data))
     return out
+
+
+# ---- plans, the parameter sweep, the capacity bound (in the emulation a "device" pointer is a host pointer)
+class Setting(ctypes.Structure):
+    _fields_ = [("block", ctypes.c_int * 3), ("stride", ctypes.c_int * 3), ("window", ctypes.c_int * 3), ("frac", ctypes.c_double)]
+
+
+def capacity_bound(dims, block, stride, frac):
+    g, b = ctypes.c_int(0), ctypes.c_int(0)
+    L = lib()
+    L.nrr_bm_capacity_bound.argtypes = [ctypes.POINTER(ctypes.c_int)] * 3 + [ctypes.c_double] + [ctypes.POINTER(ctypes.c_int)] * 2
+    _check(L.nrr_bm_capacity_bound(_i3(dims), _i3(block), _i3(stride), float(frac), ctypes.byref(g), ctypes.byref(b)))
+    return g.value, b.value
+
+
+class Plan:
+    def __init__(self, fixed, block, stride, window, frac, mask=None, connectivity=0, host=True):
+        L = lib()
+        vp, ci, cd = ctypes.c_void_p, ctypes.c_int, ctypes.c_double
+        i3 = ctypes.POINTER(ctypes.c_int)
+        L.nrr_bm_plan_create_host.argtypes = [vp, i3, i3, i3, i3, cd, vp, ci, ctypes.POINTER(vp)]
+        L.nrr_bm_plan_create.argtypes = [vp, i3, i3, i3, i3, cd, vp, ci, vp, ctypes.POINTER(vp)]
+        L.nrr_bm_plan_info.argtypes = [vp, i3, i3]
+        L.nrr_bm_plan_blocks_host.argtypes = [vp, vp, vp]
+        L.nrr_bm_plan_match.argtypes = [vp, vp, vp, vp, vp]
+        L.nrr_bm_plan_match_range.argtypes = [vp, vp, ci, ci, vp, vp, vp]
+        L.nrr_bm_plan_match_host.argtypes = [vp, vp, vp, vp]
+        L.nrr_bm_plan_destroy.argtypes = [vp]
+        nz, ny, nx = fixed.shape
+        self.fixed, self.mask = fixed, mask      # the device form keeps the caller's pointer
+        self.h = vp()
+        mp = None if mask is None else mask.ctypes.data
+        if host:
+            _check(L.nrr_bm_plan_create_host(fixed.ctypes.data, _i3((nx, ny, nz)), _i3(block), _i3(stride), _i3(window),
+                                             float(frac), mp, int(connectivity), ctypes.byref(self.h)))
+        else:
+            _check(L.nrr_bm_plan_create(fixed.ctypes.data, _i3((nx, ny, nz)), _i3(block), _i3(stride), _i3(window),
+                                        float(frac), mp, int(connectivity), None, ctypes.byref(self.h)))
+        n, nc = ctypes.c_int(0), ctypes.c_int(0)
+        _check(L.nrr_bm_plan_info(self.h, ctypes.byref(n), ctypes.byref(nc)))
+        self.n, self.ncand = n.value, nc.value
+
+    def blocks(self):
+        b = np.empty((self.n, 3), np.int32)
+        v = np.empty((self.n,), np.float64)
+        _check(lib().nrr_bm_plan_blocks_host(self.h, b.ctypes.data, v.ctypes.data))
+        return b, v
+
+    def match(self, moving, first=None, count=None, out=None):
+        disp, ncc = out if out is not None else (np.full((self.n, 3), -99, np.int32), np.full((self.n,), -99.0, np.float32))
+        if first is None:
+            _check(lib().nrr_bm_plan_match(self.h, moving.ctypes.data, disp.ctypes.data, ncc.ctypes.data, None))
+        else:
+            _check(lib().nrr_bm_plan_match_range(self.h, moving.ctypes.data, int(first), int(count), disp.ctypes.data, ncc.ctypes.data, None))
+        _check(lib().nrr_bm_check_async_error(None))
+        return disp, ncc
+
+    def match_host(self, moving):
+        disp = np.full((self.n, 3), -99, np.int32)
+        ncc = np.full((self.n,), -99.0, np.float32)
+        _check(lib().nrr_bm_plan_match_host(self.h, moving.ctypes.data, disp.ctypes.data, ncc.ctypes.data))
+        return disp, ncc
+
+    def destroy(self):
+        if self.h:
+            _check(lib().nrr_bm_plan_destroy(self.h))
+            self.h = None
+
+
+def register_batch(fixed, moving, settings, mask=None):
+    """settings: iterable of (block, stride, window, frac).  Returns [(blocks, disp, ncc)] trimmed to K per setting."""
+    L = lib()
+    vp, ci = ctypes.c_void_p, ctypes.c_int
+    i3 = ctypes.POINTER(ctypes.c_int)
+    pp = ctypes.POINTER(vp)
+    L.nrr_bm_register_batch.argtypes = [vp, vp, i3, vp, vp, ci, pp, i3, vp, pp, pp, vp]
+    nz, ny, nx = fixed.shape
+    ns = len(settings)
+    arr = (Setting * ns)()
+    caps = (ci * ns)()
+    pb, pd, pn = (vp * ns)(), (vp * ns)(), (vp * ns)()
+    keep = []
+    for i, (block, stride, window, frac) in enumerate(settings):
+        arr[i].block[:] = list(block)
+        arr[i].stride[:] = list(stride)
+        arr[i].window[:] = list(window)
+        arr[i].frac = float(frac)
+        cap = max(1, capacity_bound((nx, ny, nz), block, stride, frac)[1])
+        caps[i] = cap
+        b = np.full((cap, 3), -99, np.int32)
+        d = np.full((cap, 3), -99, np.int32)
+        c = np.full((cap,), -99.0, np.float32)
+        pb[i], pd[i], pn[i] = b.ctypes.data, d.ctypes.data, c.ctypes.data
+        keep.append((b, d, c))
+    out_n = np.zeros((ns,), np.int32)
+    _check(L.nrr_bm_register_batch(fixed.ctypes.data, moving.ctypes.data, _i3((nx, ny, nz)),
+                                   None if mask is None else mask.ctypes.data, arr, ns, pb, caps, out_n.ctypes.data, pd, pn, None))
+    _check(L.nrr_bm_check_async_error(None))
+    return [(b[:k], d[:k], c[:k]) for (b, d, c), k in zip(keep, out_n)], out_n

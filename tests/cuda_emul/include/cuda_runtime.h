@@ -81,6 +81,8 @@ cudaError_t cudaMemset(void *p, int v, size_t bytes);
 cudaError_t cudaMemsetAsync(void *p, int v, size_t bytes, cudaStream_t s);
 cudaError_t cudaMemcpyAsync(void *d, const void *s, size_t bytes, cudaMemcpyKind k, cudaStream_t st);
 cudaError_t cudaStreamSynchronize(cudaStream_t s);
+cudaError_t cudaDeviceSynchronize(void);
+cudaError_t cudaStreamDestroy(cudaStream_t s);
 cudaError_t cudaStreamCreateWithFlags(cudaStream_t *s, unsigned flags);
 cudaError_t cudaEventCreate(cudaEvent_t *e);
 cudaError_t cudaEventCreateWithFlags(cudaEvent_t *e, unsigned flags);
@@ -88,6 +90,7 @@ cudaError_t cudaStreamWaitEvent(cudaStream_t s, cudaEvent_t e, unsigned flags);
 cudaError_t cudaEventDestroy(cudaEvent_t e);
 cudaError_t cudaEventRecord(cudaEvent_t e, cudaStream_t s);
 cudaError_t cudaEventSynchronize(cudaEvent_t e);
+cudaError_t cudaEventQuery(cudaEvent_t e);
 cudaError_t cudaEventElapsedTime(float *ms, cudaEvent_t a, cudaEvent_t b);
 cudaError_t cudaGetLastError(void);
 const char *cudaGetErrorString(cudaError_t e);

@@ -45,8 +45,8 @@ def match(fixed, moving, blocks, block, window, out_disp=None, out_ncc=None, str
     try:
         d, s = _emul.match(_np(fixed), _np(moving), _np(blocks), block, window)
     except RuntimeError as e:
-        if "leaves the volume" in str(e):
-            _pending["err"] = NrrError(-8, str(e))
+        if "leaves the volume" in str(e) or "status -12" in str(e):      # sticky device flags: reported by the next check
+            _pending["err"] = NrrError(-12 if "status -12" in str(e) else -8, str(e))
             n = blocks.shape[0]
             return torch.zeros((n,3),dtype=torch.int32), torch.full((n,), float("nan"))
         raise
@@ -67,6 +67,32 @@ def moving_stats(moving, block, out=None, stream=None):
 def match_info(dims, block, window):
     i = _emul.match_info(dims, block, window)
     return {"fast": bool(i["kernel"]), "kernel": i["kernel"], "threads": i["threads"], "smem_bytes": i["smem_bytes"], "tma": bool(i["tma"]), "candidates": i["candidates"], "blocks_per_cta": 0}
+class _Plan:
+    def __init__(self, p): self.p, self.n, self.ncand = p, p.n, p.ncand
+def plan_create(fixed, block, stride, window, frac, mask=None, connectivity=0, stream=None):
+    return _Plan(_emul.Plan(_np(fixed), block, stride, window, frac, _np(mask), connectivity, host=False))
+def plan_create_host(fixed, block, stride, window, frac, mask=None, connectivity=0):
+    return _Plan(_emul.Plan(fixed, block, stride, window, frac, mask, connectivity, host=True))
+def plan_match(plan, moving, out_disp=None, out_ncc=None, stream=None, first=0, count=None):
+    out = None if out_disp is None else (out_disp.numpy(), out_ncc.numpy())
+    if count is None and first == 0:
+        d, s = plan.p.match(_np(moving), out=out)
+    else:
+        d, s = plan.p.match(_np(moving), first, plan.n - first if count is None else count, out=out)
+    return (torch.from_numpy(d), torch.from_numpy(s)) if out is None else (out_disp, out_ncc)
+def register_batch(fixed, moving, settings, mask=None, stream=None):
+    got, out_n = _emul.register_batch(_np(fixed), _np(moving), [(st.block, st.stride, st.window, st.frac) for st in settings], _np(mask))
+    return [tuple(torch.from_numpy(a.copy()) for a in g) for g in got], torch.from_numpy(out_n)
+fake.nrr_bm_plan_create = plan_create
+fake.nrr_bm_plan_create_host = plan_create_host
+fake.nrr_bm_plan_info = lambda plan: (plan.n, plan.ncand)
+fake.nrr_bm_plan_blocks_host = lambda plan, want_var=False: plan.p.blocks() if want_var else plan.p.blocks()[0]
+fake.nrr_bm_plan_match = plan_match
+fake.nrr_bm_plan_match_range = plan_match
+fake.nrr_bm_plan_match_host = lambda plan, moving, out_disp=None, out_ncc=None: plan.p.match_host(moving)
+fake.nrr_bm_plan_destroy = lambda plan: plan.p.destroy()
+fake.nrr_bm_register_batch = register_batch
+fake.nrr_bm_capacity_bound = _emul.capacity_bound
 fake.nrr_bm_select_blocks = select
 fake.nrr_bm_select_blocks_pruned = select_pruned
 fake.nrr_bm_match = match

@@ -35,7 +35,7 @@ def test_library_exports_every_declared_symbol(nrr):
     for s in _declared_symbols():
         assert hasattr(L, s), "libnrr_bm.so does not export %s" % s
     assert sorted(nrr.EXPORTS) == _declared_symbols()
-    assert nrr.nrr_bm_version() == 100
+    assert nrr.nrr_bm_version() == 200
 
 
 def test_library_is_built_for_sm_100a(nrr):
@@ -87,7 +87,29 @@ def test_argument_validation_happens_before_cuda(nrr):
     assert L.nrr_bm_pair_task_table(i3(7, 5, 7), i3(5, 5, 5), None, 0, info) == -11      # not square in-plane: no plan
     assert L.nrr_bm_pair_task_table(i3(7, 7, 7), i3(5, 5, 5), None, 0, info) == -7 and info[0] == 288
     assert nrr.lib().nrr_bm_status_string(-7) == b"NRR_E_CAPACITY"
+    assert nrr.lib().nrr_bm_status_string(-12) == b"NRR_E_DEVICE"
     assert L.nrr_bm_set_option(b"no_such_option", 1.0) == -11
+    # r2: plans, the parameter sweep, the capacity bound
+    g, bnd = ctypes.c_int(0), ctypes.c_int(0)
+    assert L.nrr_bm_capacity_bound(i3(8, 8, 8), i3(3, 3, 3), i3(1, 1, 0), 0.5, ctypes.byref(g), ctypes.byref(bnd)) == -4
+    assert L.nrr_bm_capacity_bound(i3(8, 8, 8), i3(3, 3, 3), i3(1, 1, 1), 0.0, ctypes.byref(g), ctypes.byref(bnd)) == -6
+    assert L.nrr_bm_capacity_bound(i3(8, 8, 8), i3(3, 3, 3), i3(1, 1, 1), 0.5, ctypes.byref(g), ctypes.byref(bnd)) == 0
+    assert g.value == 216 and 108 <= bnd.value <= 109
+    h = ctypes.c_void_p()
+    assert L.nrr_bm_plan_create(p, i3(8, 8, 8), i3(3, 3, 3), i3(1, 1, 1), i3(1, 1, 1), 0.5, None, 0, None, None) == -1
+    assert L.nrr_bm_plan_create(p, i3(8, 8, 8), i3(3, 3, 3), i3(1, 1, 1), i3(1, 1, 1), 0.5, None, 5, None, ctypes.byref(h)) == -11
+    assert L.nrr_bm_plan_create(p, i3(8, 8, 8), i3(3, 3, 3), i3(1, 1, 1), i3(1, -1, 1), 0.5, None, 0, None, ctypes.byref(h)) == -5
+    assert L.nrr_bm_plan_create_host(p, i3(8, 8, 8), i3(2, 3, 3), i3(1, 1, 1), i3(1, 1, 1), 0.5, None, 0, ctypes.byref(h)) == -3
+    assert not h.value
+    assert L.nrr_bm_plan_match(None, p, p, p, None) == -11 and L.nrr_bm_plan_match_host(None, p, p, p) == -11
+    assert L.nrr_bm_plan_info(None, None, None) == -11 and L.nrr_bm_plan_destroy(None) == 0
+    assert L.nrr_bm_register_batch(p, p, i3(8, 8, 8), None, None, 0, None, None, None, None, None, None) == 0       # nothing to do
+    assert L.nrr_bm_register_batch(p, p, i3(8, 8, 8), None, None, 2, None, None, None, None, None, None) == -1
+    st = (nrr.nrr_bm_setting * 1)()
+    st[0].block[:] = [3, 3, 3]; st[0].stride[:] = [1, 1, 1]; st[0].window[:] = [1, 1, 1]; st[0].frac = 7.0
+    one = (ctypes.c_void_p * 1)(p.value)
+    cap = (ctypes.c_int * 1)(4)
+    assert L.nrr_bm_register_batch(p, p, i3(8, 8, 8), None, st, 1, one, cap, None, one, one, None) == -6
 
 
 def test_match_info_dispatch_table(nrr):

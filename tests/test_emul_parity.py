@@ -3,6 +3,8 @@ the fiber-per-thread emulation under tests/cuda_emul, called through the C-ABI h
 with the oracle under the same acceptance rules as the GPU parity tests (tests/_parity.py).  This catches index,
 layout, barrier and tie-rule mistakes without a GPU; it says nothing about hardware behaviour or speed, which the
 -m gpu tests and bench.py cover."""
+import ctypes
+
 import numpy as np
 import pytest
 
@@ -284,3 +286,98 @@ def test_emulated_staging_timeout_is_an_error_code_not_a_fault():
     _emul.set_option("debug_expect_tx_extra", 0)
     d, n = _emul.match(vol, mov, sel["centres"], block, window)      # the flag was cleared; the library still works
     assert np.array_equal(d, good_d) and np.array_equal(n, good_n)
+
+
+# ------------------------------------------------------------------------------------------- plans, batch
+@pytest.mark.parametrize("dims,block,stride,window,frac,mask_r", [
+    ((48, 40, 30), (7, 7, 7), (5, 5, 5), (5, 5, 3), 0.5, 18.0),      # pair kernel, TMA staging, records kept by the plan
+    ((41, 37, 29), (5, 5, 5), (4, 4, 4), (3, 3, 3), 0.3, None),      # nx % 4 != 0: plain staging
+    ((40, 36, 24), (3, 5, 3), (3, 3, 3), (2, 1, 3), 0.4, None),      # generic kernel: no records
+])
+def test_emulated_plan_equals_select_then_match(dims, block, stride, window, frac, mask_r):
+    """pre-operative plan (selection + fixed-block records), intra-operative match.  Bit-equal to
+    nrr_bm_select_blocks + nrr_bm_match; the host form's slab pipeline and block ranges must not change a bit."""
+    fixed = _smooth(dims, 500 + dims[0])
+    mask = None if mask_r is None else spherical_mask(dims, mask_r)
+    blocks, n, ncand, var = _emul.select(fixed, block, stride, frac, mask)
+    assert n > 8
+    for host in (True, False):
+        plan = _emul.Plan(fixed, block, stride, window, frac, mask, host=host)
+        pb, pv = plan.blocks()
+        assert plan.n == n and plan.ncand == ncand and np.array_equal(pb, blocks) and np.array_equal(pv, var)
+        for k, shift in enumerate(((1, -1, 1), (-2, 0, 1))):          # one plan, several intra-operative volumes
+            moving = _shift_noise(fixed, shift, 12.0, 600 + k)
+            want_d, want_n = _emul.match(fixed, moving, blocks, block, window)
+            d, s = plan.match(moving)
+            assert np.array_equal(d, want_d) and np.array_equal(s, want_n)
+            for slabs in (1, 2, 3, 7, 1000):
+                _emul.set_option("plan_slabs", slabs)
+                d, s = plan.match_host(moving)
+                assert np.array_equal(d, want_d) and np.array_equal(s, want_n), slabs
+            _emul.set_option("plan_slabs", 4)
+            # the natural shard (PAPER.md:379-385): ranks match slices of the block list; stitched = whole
+            out = (np.full((n, 3), -99, np.int32), np.full((n,), -99.0, np.float32))
+            cuts = [0, n // 3, n // 3, n - 1, n]
+            for a, b in zip(cuts[:-1], cuts[1:]):
+                plan.match(moving, a, b - a, out=out)
+            assert np.array_equal(out[0], want_d) and np.array_equal(out[1], want_n)
+            part = plan.match(moving, 2, 3)
+            assert np.all(part[0][:2] == -99) and np.all(part[0][5:] == -99) and np.array_equal(part[0][2:5], want_d[2:5])
+        with pytest.raises(RuntimeError, match="status -11"):
+            plan.match(moving, n - 1, 2)
+        plan.destroy()
+
+
+def test_emulated_plan_with_connectivity_pattern_and_oracle():
+    dims, block, stride, window = (40, 36, 24), (5, 5, 5), (2, 2, 2), (3, 3, 3)
+    fixed = _smooth(dims, 91)
+    moving = _shift_noise(fixed, (1, 1, -1), 8.0, 92)
+    ora_sel = oracle.select_pruned(fixed, block, stride, 0.2, None, 18)
+    plan = _emul.Plan(fixed, block, stride, window, 0.2, None, connectivity=18)
+    pb, pv = plan.blocks()
+    assert_select_parity(pb, plan.n, plan.ncand, ora_sel, pv)
+    d, s = plan.match_host(moving)
+    assert_match_parity(d, s, oracle.match(fixed, moving, ora_sel["centres"], block, window), "plan, 18-connectivity")
+    plan.destroy()
+
+
+def test_emulated_batch_equals_separate_register_calls():
+    """PAPER.md:527-540 / BASELINE.json configs[4]: many settings on one pair in one launch sequence; shared
+    normalisers, shared variance keys (two fractions from one statistics pass), shared records."""
+    dims = (44, 40, 36)
+    fixed = _smooth(dims, 71)
+    moving = _shift_noise(fixed, (1, -2, 1), 9.0, 72)
+    mask = spherical_mask(dims, 17.0)
+    settings = []
+    for b in (5, 7):
+        for r in (3, 5):
+            for frac in (0.1, 0.3):
+                settings.append(((b, b, b), (5, 5, 5), (r, r, r), frac))
+    settings.append(((3, 5, 3), (4, 4, 4), (1, 2, 1), 0.5))          # a shape only the generic kernel takes
+    settings.append(((7, 7, 7), (5, 5, 5), (4, 4, 4), 0.3))          # no fast instantiation: no records, shared selection
+    L = _emul.lib()
+    L.nrr_bm_launch_count.restype = ctypes.c_longlong
+    L.nrr_bm_launch_count(1)
+    got, out_n = _emul.register_batch(fixed, moving, settings, mask)
+    batch_launches = L.nrr_bm_launch_count(1)
+    assert len(got) == len(settings)
+    for (block, stride, window, frac), (gb, gd, gs), k in zip(settings, got, out_n):
+        wb, wd, ws = _emul.register(fixed, moving, block, stride, window, frac, mask)
+        assert k == len(wb) and np.array_equal(gb, wb), (block, window, frac)
+        assert np.array_equal(gd, wd) and np.array_equal(gs, ws), (block, window, frac)
+    separate_launches = L.nrr_bm_launch_count(1)
+    # 10 settings: 3 moving-statistics passes instead of 10, 3 variance passes instead of 10, 5 record sets instead of 8
+    assert batch_launches <= separate_launches - 7 - 7 - 3, (batch_launches, separate_launches)
+    ora_sel = oracle.select(fixed, (7, 7, 7), (5, 5, 5), 0.3, mask)
+    assert np.array_equal(got[7][0], ora_sel["centres"])
+    assert_match_parity(got[7][1], got[7][2], oracle.match(fixed, moving, ora_sel["centres"], (7, 7, 7), (5, 5, 5)), "batch")
+
+
+def test_capacity_bound_is_the_count_rule():
+    for dims, block, stride, frac in (((64, 64, 32), (5, 5, 5), (5, 5, 5), 0.3), ((256, 256, 124), (7, 7, 7), (5, 5, 5), 0.25),
+                                      ((9, 9, 9), (9, 9, 9), (1, 1, 1), 1.0), ((30, 20, 10), (3, 5, 7), (2, 3, 1), 0.05)):
+        ngrid, bound = _emul.capacity_bound(dims, block, stride, frac)
+        assert ngrid == int(np.prod(oracle.grid(dims, block, stride)))
+        for n in (ngrid, ngrid // 2, 1, 0):
+            assert bound >= oracle.count(n, frac)
+        assert bound <= min(ngrid, oracle.count(ngrid, frac) + 1)

@@ -45,6 +45,18 @@ def _require_cuda():
 _pairs = {}
 
 
+def assert_ncc_of_chosen_displacement(fixed, moving, blocks, block, disp, ncc, label=""):
+    """Whole-set check where the full oracle search is too slow: for EVERY block the reported NCC must be the oracle's
+    NCC of the reported displacement (one candidate per block), within the north_star tolerance."""
+    worst = 0.0
+    for c, d, s in zip(blocks, disp, ncc):
+        want = oracle.ncc_at(fixed, moving, c, block, d)
+        assert np.isfinite(want), "%s: block %s chose a skipped candidate %s" % (label, c, d)
+        worst = max(worst, abs(float(s) - want))
+    assert worst <= 1e-4, "%s: max |gpu_ncc - oracle.ncc_at(gpu_disp)| = %g" % (label, worst)
+    return worst
+
+
 def pair(name):
     if name not in _pairs:
         _pairs[name] = make_pair(CONFIGS[name])
@@ -351,6 +363,8 @@ def test_match_parity_highres_sampled():
     ora = oracle.match(fixed, moving, blocks.cpu().numpy()[idx], cfg.block, cfg.window)
     exempt = assert_match_parity(disp.cpu().numpy()[idx], ncc.cpu().numpy()[idx], ora, label="highres")
     print("highres: %d blocks on the GPU, %d checked, %d exempt" % (n, len(idx), exempt))
+    worst = assert_ncc_of_chosen_displacement(fixed, moving, blocks.cpu().numpy(), cfg.block, disp.cpu().numpy(), ncc.cpu().numpy(), "highres")
+    print("highres: all %d blocks: max |ncc - oracle.ncc_at(disp)| %.3g" % (n, worst))
     # properties that hold at any size
     d = disp.cpu().numpy()
     assert np.all(np.abs(d) <= np.asarray(cfg.window))
@@ -359,25 +373,95 @@ def test_match_parity_highres_sampled():
 
 
 def test_match_parity_batch_sampled():
-    """Config 5: 32 settings on the fullres pair, enqueued as ONE launch sequence (nrr_bm_register: no host
-    synchronisation between settings); per setting the selection is checked in full and 48 sampled blocks are
-    checked against the oracle."""
+    """Config 5: 32 settings on the fullres pair as ONE launch sequence that shares work (nrr_bm_register_batch: no
+    host synchronisation; normalisers per block shape, variance keys per (block, stride), records per block list).
+    Per setting the selection is checked in full, 48 sampled blocks against the full oracle search, and EVERY block's
+    NCC against the oracle's NCC of the displacement it chose."""
     fixed, moving, mask = pair("fullres")
     f, m, k = _cuda(fixed), _cuda(moving), _cuda(mask)
     settings = list(batch_settings())
     assert len(settings) == 32
-    launched = [nrr.nrr_bm_register(f, m, st.block, st.stride, st.window, st.frac, k) for st in settings]
+    results, out_n = nrr.nrr_bm_register_batch(f, m, settings, k)
     nrr.nrr_bm_check_async_error()                                   # the only synchronisation
+    ns = out_n.cpu().numpy()
     total_exempt = total_blocks = 0
-    for si, (st, (rb, rn, rd, rs)) in enumerate(zip(settings, launched)):
-        n = int(rn.item())
+    worst = 0.0
+    for si, (st, (rb, rd, rs)) in enumerate(zip(settings, results)):
+        n = int(ns[si])
         ora_sel = oracle.select(fixed, st.block, st.stride, st.frac, mask)
         assert_select_parity(rb[:n].cpu().numpy(), n, ora_sel["n_candidates"], ora_sel)
         idx = np.sort(np.random.default_rng(1000 + si).choice(n, 48, replace=False))
         ora = oracle.match(fixed, moving, ora_sel["centres"][idx], st.block, st.window)
         total_exempt += assert_match_parity(rd[:n].cpu().numpy()[idx], rs[:n].cpu().numpy()[idx], ora, label=str(st))
+        worst = max(worst, assert_ncc_of_chosen_displacement(fixed, moving, ora_sel["centres"], st.block, rd[:n].cpu().numpy(),
+                                                             rs[:n].cpu().numpy(), str(st)))
         total_blocks += n
-    print("batch: 32 settings, %d blocks, %d exempt blocks among the samples" % (total_blocks, total_exempt))
+    print("batch: 32 settings, %d blocks, %d exempt blocks among the samples, all blocks: max |ncc - oracle.ncc_at(disp)| %.3g" % (
+        total_blocks, total_exempt, worst))
+    # the same sweep as 32 separate nrr_bm_register calls gives the same bits
+    for si in (0, 13, 31):
+        st = settings[si]
+        rb, rn, rd, rs = nrr.nrr_bm_register(f, m, st.block, st.stride, st.window, st.frac, k)
+        torch.cuda.synchronize()
+        n = int(rn.item())
+        assert n == int(ns[si]) and torch.equal(rb[:n], results[si][0][:n])
+        assert torch.equal(rd[:n], results[si][1][:n]) and torch.equal(rs[:n], results[si][2][:n])
+
+
+@pytest.mark.parametrize("name", ["tiny", "intraop", "fullres"])
+def test_plan_equals_select_then_match(name):
+    """the pre-operative plan (selection + fixed-block records) and the intra-operative match give
+    the bits of nrr_bm_select_blocks + nrr_bm_match; so do the host form's slab pipeline and a sharded block list."""
+    cfg = CONFIGS[name]
+    fixed, moving, mask = pair(name)
+    f, m, k = _cuda(fixed), _cuda(moving), _cuda(mask)
+    blocks, n, ncand = nrr.nrr_bm_select_blocks(f, cfg.block, cfg.stride, cfg.frac, k)
+    disp, ncc = nrr.nrr_bm_match(f, m, blocks, cfg.block, cfg.window)
+    plan = nrr.nrr_bm_plan_create(f, cfg.block, cfg.stride, cfg.window, cfg.frac, k)
+    assert nrr.nrr_bm_plan_info(plan) == (n, ncand)
+    assert np.array_equal(nrr.nrr_bm_plan_blocks_host(plan), blocks.cpu().numpy())
+    for _ in range(2):                                               # a plan serves many intra-operative volumes
+        pd, pn = nrr.nrr_bm_plan_match(plan, m)
+        nrr.nrr_bm_check_async_error()
+        assert torch.equal(pd, disp) and torch.equal(pn, ncc)
+    od = torch.full((n, 3), -99, dtype=torch.int32, device="cuda")
+    on = torch.full((n,), -99.0, dtype=torch.float32, device="cuda")
+    cuts = [0, n // 2, n]                                            # two "ranks", each its slice of the block list
+    for a, b in zip(cuts[:-1], cuts[1:]):
+        nrr.nrr_bm_plan_match_range(plan, m, od, on, first=a, count=b - a)
+    nrr.nrr_bm_check_async_error()
+    assert torch.equal(od, disp) and torch.equal(on, ncc)
+    nrr.nrr_bm_plan_destroy(plan)
+    hplan = nrr.nrr_bm_plan_create_host(fixed, cfg.block, cfg.stride, cfg.window, cfg.frac, mask)
+    for slabs in (4, 1, 9):
+        nrr.nrr_bm_set_option("plan_slabs", slabs)
+        hd, hn = nrr.nrr_bm_plan_match_host(hplan, moving)
+        assert np.array_equal(hd, disp.cpu().numpy()) and np.array_equal(hn, ncc.cpu().numpy()), slabs
+    nrr.nrr_bm_set_option("plan_slabs", 4)
+    nrr.nrr_bm_plan_destroy(hplan)
+
+
+def test_staging_timeout_reports_device_error_without_faulting():
+    """The matching kernel's bounded wait: an over-programmed staging barrier must end as NRR_E_DEVICE (-12) with NaN
+    results and a usable context afterwards -- never a trap."""
+    cfg = CONFIGS["tiny"]
+    fixed, moving, _ = pair("tiny")
+    f, m = _cuda(fixed), _cuda(moving)
+    blocks, n, _ = nrr.nrr_bm_select_blocks(f, cfg.block, cfg.stride, cfg.frac)
+    good = nrr.nrr_bm_match(f, m, blocks[:8], cfg.block, cfg.window)
+    nrr.nrr_bm_check_async_error()
+    nrr.nrr_bm_set_option("debug_expect_tx_extra", 16)
+    try:
+        bad = nrr.nrr_bm_match(f, m, blocks[:8], cfg.block, cfg.window)        # 2 CTAs wait out the time bound (seconds)
+        with pytest.raises(nrr.NrrError) as ei:
+            nrr.nrr_bm_check_async_error()
+        assert ei.value.status == -12
+        assert torch.isnan(bad[1]).all()
+    finally:
+        nrr.nrr_bm_set_option("debug_expect_tx_extra", 0)
+    again = nrr.nrr_bm_match(f, m, blocks[:8], cfg.block, cfg.window)
+    nrr.nrr_bm_check_async_error()
+    assert torch.equal(again[0], good[0]) and torch.equal(again[1], good[1])
 
 
 # ------------------------------------------------------------------------------------------- dense-field warp
