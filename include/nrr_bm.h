@@ -296,14 +296,20 @@ NRR_BM_API int nrr_bm_register_host(const float *fixed, const float *moving, con
  *      info[0] = 2 pair kernel (two candidate rows per thread) / 1 one-row-per-thread kernel / 0 generic kernel,
  *      info[1] = threads per CTA, info[2] = dynamic shared memory bytes, info[3] = 1 if TMA staging is used,
  *      info[4] = candidates per block, info[5] = blocks per CTA.
- *  nrr_bm_fp32_peak: runs an FFMA-only microbenchmark on `stream`'s device and returns the measured
- *      dense FP32 rate in TFLOP/s (the denominator context for the matching kernel's roofline).
+ *  nrr_bm_fp32_peak: runs register-only FFMA / FFMA2 microbenchmarks on `stream`'s device and returns the best
+ *      measured dense FP32 rate in TFLOP/s (the denominator context for the matching kernel's roofline).
  */
 NRR_BM_API int nrr_bm_profile_enable(int on);
 NRR_BM_API int nrr_bm_profile_read(double ms[4], int calls[4]);
 NRR_BM_API long long nrr_bm_launch_count(int reset);
 NRR_BM_API int nrr_bm_match_info(const int dims[3], const int block[3], const int window[3], int info[6]);
 NRR_BM_API int nrr_bm_fp32_peak(double *out_tflops, void *stream);
+/*  nrr_bm_fp32_microbench: the FP32 microbenchmarks behind the matching kernel's design, TFLOP/s:
+ *      out[0] FFMA register chain, out[1] FFMA register tile, out[2] FFMA2 (fma.rn.f32x2) packed x packed,
+ *      out[3] FFMA2 scalar-broadcast x packed  (nrr_bm_fp32_peak = the best of these four);
+ *      USEFUL TFLOP/s of three main-loop bodies on synthetic shared-memory data shaped like the 7^3 / +-5 search:
+ *      out[4] one candidate row per thread with FFMA, out[5] two rows with FFMA, out[6] two rows with FFMA2. */
+NRR_BM_API int nrr_bm_fp32_microbench(double out_tflops[7], void *stream);
 /*  nrr_bm_pair_task_table: the host-built lane -> task table of the pair matching kernel for a cubic block and a
  *      window (wx == wy), one word per thread of a CTA: bit 31 = lane has a task, bit 30 = one-row warp,
  *      bits 16..23 = block of the CTA's group, bits 8..15 = dy index, bits 0..7 = pair index p (rows dz = 2p, 2p+1;

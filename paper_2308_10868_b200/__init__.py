@@ -5,7 +5,7 @@ Python binding.  Same names as the C entry points.
 """
 from .binding import (  # noqa: F401
     EXPORTS, LIB_PATH, NrrError, lib,
-    nrr_bm_check_async_error, nrr_bm_fp32_peak, nrr_bm_launch_count, nrr_bm_match, nrr_bm_register, nrr_bm_moving_stats, nrr_bm_match_host,
+    nrr_bm_check_async_error, nrr_bm_fp32_peak, nrr_bm_fp32_microbench, nrr_bm_launch_count, nrr_bm_match, nrr_bm_register, nrr_bm_moving_stats, nrr_bm_match_host,
     nrr_bm_match_info, nrr_bm_pair_task_table, nrr_bm_profile_enable, nrr_bm_profile_read, nrr_bm_register_host, nrr_bm_select_blocks,
     nrr_bm_select_blocks_pruned,
     nrr_bm_select_blocks_host, nrr_bm_set_option, nrr_bm_version, nrr_bm_warp,

@@ -26,7 +26,7 @@ EXPORTS = [
     "nrr_bm_capacity_bound", "nrr_bm_plan_create", "nrr_bm_plan_create_host", "nrr_bm_plan_info", "nrr_bm_plan_blocks_host",
     "nrr_bm_plan_blocks_device", "nrr_bm_plan_match", "nrr_bm_plan_match_range", "nrr_bm_plan_match_host", "nrr_bm_plan_destroy",
     "nrr_bm_register_batch",
-    "nrr_bm_fp32_peak", "nrr_bm_pair_task_table", "nrr_bm_set_option", "nrr_bm_last_error", "nrr_bm_status_string", "nrr_bm_version",
+    "nrr_bm_fp32_peak", "nrr_bm_fp32_microbench", "nrr_bm_pair_task_table", "nrr_bm_set_option", "nrr_bm_last_error", "nrr_bm_status_string", "nrr_bm_version",
 ]
 
 
@@ -111,6 +111,8 @@ def lib() -> ctypes.CDLL:
     L.nrr_bm_pair_task_table.argtypes = [i3, i3, vp, ci, ctypes.POINTER(ci)]
     L.nrr_bm_fp32_peak.restype = ci
     L.nrr_bm_fp32_peak.argtypes = [ctypes.POINTER(cd), vp]
+    L.nrr_bm_fp32_microbench.restype = ci
+    L.nrr_bm_fp32_microbench.argtypes = [ctypes.POINTER(cd), vp]
     L.nrr_bm_set_option.restype = ci
     L.nrr_bm_set_option.argtypes = [ctypes.c_char_p, cd]
     L.nrr_bm_last_error.restype = ctypes.c_char_p
@@ -543,6 +545,14 @@ def nrr_bm_fp32_peak(stream=None) -> float:
     out = ctypes.c_double(0.0)
     _check(lib().nrr_bm_fp32_peak(ctypes.byref(out), _stream_ptr(stream)))
     return out.value
+
+
+def nrr_bm_fp32_microbench(stream=None):
+    """TFLOP/s of the FP32 microbenchmarks (include/nrr_bm.h): register-only FFMA / FFMA2 and three main-loop bodies."""
+    out = (ctypes.c_double * 7)()
+    _check(lib().nrr_bm_fp32_microbench(out, _stream_ptr(stream)))
+    names = ("ffma_chain", "ffma_tile", "ffma2_packed", "ffma2_scalar", "loop_1row_ffma_useful", "loop_2row_ffma_useful", "loop_2row_ffma2_useful")
+    return dict(zip(names, [float(v) for v in out]))
 
 
 def nrr_bm_set_option(name: str, value: float) -> None:

@@ -691,6 +691,12 @@ int nrr_bm_fp32_peak(double *out_tflops, void *stream)
     return fp32_peak_measure(out_tflops, (cudaStream_t)stream);
 }
 
+int nrr_bm_fp32_microbench(double out_tflops[7], void *stream)
+{
+    if (!out_tflops) return fail(NRR_E_NULL, "out_tflops is NULL");
+    return fp32_microbench(out_tflops, (cudaStream_t)stream);
+}
+
 int nrr_bm_set_option(const char *name, double value)
 {
     if (!name) return fail(NRR_E_NULL, "name is NULL");

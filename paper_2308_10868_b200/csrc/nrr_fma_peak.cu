@@ -1,10 +1,16 @@
-// nrr_fma_peak.cu -- FFMA-only microbenchmark: the measured dense-FP32 rate of this GPU, reported next to
-// the matching kernel's achieved rate (MEASURED_PEAKS.json carries no FP32 figure).
-//
-// Two register-only loop bodies are timed and the faster one is reported:
-//   chain : 16 independent accumulators, acc = fma(acc, x, y)
-//   tile  : the register-tile shape of the matching kernel, acc[j] += f[v] * m[j+v] (16 x 4)
-// 148 x 8 CTAs of 256 threads, enough iterations for ~1 ms; CUDA events on the caller's stream.
+// nrr_fma_peak.cu -- FP32 microbenchmarks: the measured dense-FP32 rate of this GPU, reported next to the matching
+// kernel's achieved rate (MEASURED_PEAKS.json carries no FP32 figure), and the loop-body experiments
+// behind the design of match_pair_kernel.  Register-only bodies (148 x 8 CTAs of 256 threads):
+//   [0] FFMA chain      : 16 independent accumulators, acc = fma(acc, x, y)
+//   [1] FFMA tile       : the register-tile shape of the matching kernel, acc[j] += f[v] * m[j+v] (16 x 4)
+//   [2] FFMA2 pair-pair : fma.rn.f32x2 with two packed operands
+//   [3] FFMA2 scalar    : fma.rn.f32x2, one operand a broadcast scalar (what match_pair_kernel issues)
+// Loop bodies over synthetic shared-memory data shaped like the 7^3 / +-5 search (148 x 7 x 4 CTAs of 128 threads, 121
+// of them with a task; USEFUL flops, counting those 121 lanes only):
+//   [4] one candidate row per thread, FFMA        (r1b's match_rows_kernel)
+//   [5] two candidate rows per thread, FFMA
+//   [6] two candidate rows per thread, FFMA2      (match_pair_kernel)
+// CUDA events on the caller's stream, best of the repetitions after warm-up.
 #include "nrr_internal.cuh"
 
 namespace nrr {
@@ -12,6 +18,15 @@ namespace nrr {
 namespace {
 
 constexpr int kIters = 4096;
+typedef unsigned long long u64;
+
+__device__ __forceinline__ void mb_fma2s(u64 &d, float a, u64 b)
+{
+    u64 aa;
+    asm("mov.b64 %0, {%1, %1};" : "=l"(aa) : "f"(a));
+    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(d) : "l"(aa), "l"(b));
+}
+__device__ __forceinline__ void mb_fma2p(u64 &d, u64 a, u64 b) { asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(d) : "l"(a), "l"(b)); }
 
 __global__ void __launch_bounds__(256) ffma_chain_kernel(float *out, float x, float y)
 {
@@ -53,41 +68,213 @@ __global__ void __launch_bounds__(256) ffma_tile_kernel(float *out, const float 
     if (s == 123.456f) out[0] = s;
 }
 
+// 8 packed accumulators x 4: 64 lane-FMAs per v-iteration pair, the same flops per iteration as the FFMA tile
+__global__ void __launch_bounds__(256) ffma2_pp_kernel(float *out, const float *in)
+{
+    u64 acc[8], m[11], f[4];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) acc[i] = 0;
+#pragma unroll
+    for (int i = 0; i < 11; ++i) m[i] = ((const u64 *)in)[(threadIdx.x + i) & 31];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) f[i] = ((const u64 *)in)[32 + i];
+#pragma unroll 1
+    for (int it = 0; it < kIters; ++it) {
+#pragma unroll
+        for (int v = 0; v < 4; ++v)
+#pragma unroll
+            for (int j = 0; j < 8; ++j) mb_fma2p(acc[j], f[v], m[j + v]);
+    }
+    u64 s = 0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) s ^= acc[i];
+    if (s == 0x123456789ull) ((u64 *)out)[0] = s;
+}
+
+// 16 packed accumulators x 4 with a scalar-broadcast operand: twice the flops of the FFMA tile per iteration
+__global__ void __launch_bounds__(256) ffma2_sp_kernel(float *out, const float *in)
+{
+    u64 acc[16], f[4];
+    float m[19];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) acc[i] = 0;
+#pragma unroll
+    for (int i = 0; i < 19; ++i) m[i] = in[(threadIdx.x + i) & 63];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) f[i] = ((const u64 *)in)[32 + i];
+#pragma unroll 1
+    for (int it = 0; it < kIters; ++it) {
+#pragma unroll
+        for (int v = 0; v < 4; ++v)
+#pragma unroll
+            for (int j = 0; j < 16; ++j) mb_fma2s(acc[j], m[j + v], f[v]);
+    }
+    u64 s = 0;
+#pragma unroll
+    for (int i = 0; i < 16; ++i) s ^= acc[i];
+    if (s == 0x123456789ull) ((u64 *)out)[0] = s;
+}
+
+// Main-loop bodies on synthetic shared data: union 17 x 19 rows x 20 floats (pitch 4 * odd), 121 candidate rows of 11.
+constexpr int kLoopUnion = 17 * 19 * 20, kLoopSmemFloats = kLoopUnion + 1024;
+
+template <int MODE>
+__global__ void __launch_bounds__(128) loop_body_kernel(float *out, const float *in, int reps)
+{
+    extern __shared__ __align__(16) float mb_sm[];
+    float *s_u = mb_sm, *s_f = mb_sm + kLoopUnion;
+    for (int i = threadIdx.x; i < kLoopSmemFloats; i += blockDim.x) mb_sm[i] = in[i & 1023];
+    __syncthreads();
+    const int t = threadIdx.x < 121 ? threadIdx.x : 120;
+    const float *urow = s_u + ((t / 11) * 19 + (t % 11)) * 20;
+    if (MODE == 0) {
+        float acc[11];
+#pragma unroll
+        for (int j = 0; j < 11; ++j) acc[j] = 0.f;
+#pragma unroll 1
+        for (int rep = 0; rep < reps; ++rep)
+#pragma unroll 1
+            for (int vz = 0; vz < 7; ++vz) {
+                const float *up = urow + vz * 19 * 20, *fp = s_f + vz * 7 * 8;
+#pragma unroll
+                for (int vy = 0; vy < 7; ++vy) {
+                    float m[20], f[8];
+#pragma unroll
+                    for (int q = 0; q < 5; ++q) { const float4 v = *(const float4 *)(up + vy * 20 + 4 * q); m[4 * q] = v.x; m[4 * q + 1] = v.y; m[4 * q + 2] = v.z; m[4 * q + 3] = v.w; }
+#pragma unroll
+                    for (int q = 0; q < 2; ++q) { const float4 v = *(const float4 *)(fp + vy * 8 + 4 * q); f[4 * q] = v.x; f[4 * q + 1] = v.y; f[4 * q + 2] = v.z; f[4 * q + 3] = v.w; }
+#pragma unroll
+                    for (int vx = 0; vx < 7; ++vx)
+#pragma unroll
+                        for (int j = 0; j < 11; ++j) acc[j] = fmaf(f[vx], m[j + vx], acc[j]);
+                }
+            }
+        float s = 0.f;
+#pragma unroll
+        for (int j = 0; j < 11; ++j) s += acc[j];
+        if (s == 123.456f) out[0] = s;
+    } else if (MODE == 1) {
+        float a[11], b[11];
+#pragma unroll
+        for (int j = 0; j < 11; ++j) { a[j] = 0.f; b[j] = 0.f; }
+#pragma unroll 1
+        for (int rep = 0; rep < reps; ++rep)
+#pragma unroll 1
+            for (int vz = 0; vz < 7; ++vz) {
+                const float *up = urow + vz * 19 * 20, *fp = s_f + vz * 7 * 16;
+#pragma unroll
+                for (int vy = 0; vy < 7; ++vy) {
+                    float m[20], f[16];
+#pragma unroll
+                    for (int q = 0; q < 5; ++q) { const float4 v = *(const float4 *)(up + vy * 20 + 4 * q); m[4 * q] = v.x; m[4 * q + 1] = v.y; m[4 * q + 2] = v.z; m[4 * q + 3] = v.w; }
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) { const float4 v = *(const float4 *)(fp + vy * 16 + 4 * q); f[4 * q] = v.x; f[4 * q + 1] = v.y; f[4 * q + 2] = v.z; f[4 * q + 3] = v.w; }
+#pragma unroll
+                    for (int vx = 0; vx < 7; ++vx)
+#pragma unroll
+                        for (int j = 0; j < 11; ++j) { a[j] = fmaf(f[2 * vx], m[j + vx], a[j]); b[j] = fmaf(f[2 * vx + 1], m[j + vx], b[j]); }
+                }
+            }
+        float s = 0.f;
+#pragma unroll
+        for (int j = 0; j < 11; ++j) s += a[j] + b[j];
+        if (s == 123.456f) out[0] = s;
+    } else {
+        u64 acc[11];
+#pragma unroll
+        for (int j = 0; j < 11; ++j) acc[j] = 0;
+#pragma unroll 1
+        for (int rep = 0; rep < reps; ++rep)
+#pragma unroll 1
+            for (int vz = 0; vz < 7; ++vz) {
+                const float *up = urow + vz * 19 * 20, *fp = s_f + vz * 7 * 16;
+#pragma unroll
+                for (int vy = 0; vy < 7; ++vy) {
+                    float m[20];
+                    u64 f[8];
+#pragma unroll
+                    for (int q = 0; q < 5; ++q) { const float4 v = *(const float4 *)(up + vy * 20 + 4 * q); m[4 * q] = v.x; m[4 * q + 1] = v.y; m[4 * q + 2] = v.z; m[4 * q + 3] = v.w; }
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) { const ulonglong2 v = *(const ulonglong2 *)(fp + vy * 16 + 4 * q); f[2 * q] = v.x; f[2 * q + 1] = v.y; }
+#pragma unroll
+                    for (int vx = 0; vx < 7; ++vx)
+#pragma unroll
+                        for (int j = 0; j < 11; ++j) mb_fma2s(acc[j], m[j + vx], f[vx]);
+                }
+            }
+        u64 s = 0;
+#pragma unroll
+        for (int j = 0; j < 11; ++j) s ^= acc[j];
+        if (s == 0x123456789ull) ((u64 *)out)[0] = s;
+    }
+}
+
+template <class Launch>
+int time_best(Launch launch, cudaStream_t stream, cudaEvent_t e0, cudaEvent_t e1, float *best_ms)
+{
+    float best = 1e30f;
+    for (int rep = 0; rep < 6; ++rep) {     // the first repetitions warm the clocks up
+        NRR_CUDA(cudaEventRecord(e0, stream));
+        launch();
+        NRR_LAUNCH_CHECK("fp32 microbenchmark");
+        NRR_CUDA(cudaEventRecord(e1, stream));
+        NRR_CUDA(cudaEventSynchronize(e1));
+        float ms = 0.f;
+        NRR_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+        if (rep >= 2 && ms < best) best = ms;
+    }
+    *best_ms = best;
+    return NRR_OK;
+}
+
 }  // namespace
 
-int fp32_peak_measure(double *out_tflops, cudaStream_t stream)
+// out[0..6] as listed at the top of this file, TFLOP/s.
+int fp32_microbench(double out[7], cudaStream_t stream)
 {
     int dev = 0, sms = 0;
     NRR_CUDA(cudaGetDevice(&dev));
     NRR_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     float *buf = nullptr;
-    NRR_CUDA(cudaMallocAsync((void **)&buf, 128 * sizeof(float), stream));
-    NRR_CUDA(cudaMemsetAsync(buf, 0, 128 * sizeof(float), stream));
+    NRR_CUDA(cudaMalloc((void **)&buf, 4096 * sizeof(float)));
+    NRR_CUDA(cudaMemsetAsync(buf, 0, 4096 * sizeof(float), stream));
     cudaEvent_t e0, e1;
     NRR_CUDA(cudaEventCreate(&e0));
     NRR_CUDA(cudaEventCreate(&e1));
     const int ctas = sms * 8, threads = 256;
     const double flops = 2.0 * 64.0 * kIters * (double)ctas * threads;
-    double best = 0.0;
-    for (int variant = 0; variant < 2; ++variant) {
-        for (int rep = 0; rep < 6; ++rep) {     // first reps warm the clocks up
-            NRR_CUDA(cudaEventRecord(e0, stream));
-            if (variant == 0)
-                ffma_chain_kernel<<<ctas, threads, 0, stream>>>(buf, 1.0000001f, 1e-9f);
-            else
-                ffma_tile_kernel<<<ctas, threads, 0, stream>>>(buf, buf);
-            NRR_LAUNCH_CHECK("ffma microbenchmark");
-            NRR_CUDA(cudaEventRecord(e1, stream));
-            NRR_CUDA(cudaEventSynchronize(e1));
-            float ms = 0.f;
-            NRR_CUDA(cudaEventElapsedTime(&ms, e0, e1));
-            const double tf = flops / ((double)ms * 1e-3) * 1e-12;
-            if (rep >= 2 && tf > best) best = tf;
-        }
+    int rc = NRR_OK;
+    float ms = 0.f;
+    if (!rc && !(rc = time_best([&] { ffma_chain_kernel<<<ctas, threads, 0, stream>>>(buf, 1.0000001f, 1e-9f); }, stream, e0, e1, &ms))) out[0] = flops / ms * 1e-9;
+    if (!rc && !(rc = time_best([&] { ffma_tile_kernel<<<ctas, threads, 0, stream>>>(buf, buf); }, stream, e0, e1, &ms))) out[1] = flops / ms * 1e-9;
+    if (!rc && !(rc = time_best([&] { ffma2_pp_kernel<<<ctas, threads, 0, stream>>>(buf, buf); }, stream, e0, e1, &ms))) out[2] = flops / ms * 1e-9;
+    if (!rc && !(rc = time_best([&] { ffma2_sp_kernel<<<ctas, threads, 0, stream>>>(buf, buf); }, stream, e0, e1, &ms))) out[3] = 2.0 * flops / ms * 1e-9;
+    const int smem = kLoopSmemFloats * (int)sizeof(float), reps = 8, grid = sms * 7 * 4;
+    const double useful = 2.0 * 121 * 11 * 343 * (double)reps * grid;
+    if (!rc) {
+        cudaError_t e = cudaFuncSetAttribute(loop_body_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(loop_body_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(loop_body_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e != cudaSuccess) rc = cuda_fail(e, "cudaFuncSetAttribute(loop_body_kernel)");
     }
+    if (!rc && !(rc = time_best([&] { loop_body_kernel<0><<<grid, 128, smem, stream>>>(buf, buf, reps); }, stream, e0, e1, &ms))) out[4] = useful / ms * 1e-9;
+    if (!rc && !(rc = time_best([&] { loop_body_kernel<1><<<grid, 128, smem, stream>>>(buf, buf, reps); }, stream, e0, e1, &ms))) out[5] = 2.0 * useful / ms * 1e-9;
+    if (!rc && !(rc = time_best([&] { loop_body_kernel<2><<<grid, 128, smem, stream>>>(buf, buf, reps); }, stream, e0, e1, &ms))) out[6] = 2.0 * useful / ms * 1e-9;
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
-    NRR_CUDA(cudaFreeAsync(buf, stream));
+    cudaStreamSynchronize(stream);
+    cudaFree(buf);
+    return rc;
+}
+
+// The best register-only rate (FFMA or FFMA2): the measured FP32 peak quoted beside the derived one.
+int fp32_peak_measure(double *out_tflops, cudaStream_t stream)
+{
+    double v[7] = {0, 0, 0, 0, 0, 0, 0};
+    const int rc = fp32_microbench(v, stream);
+    if (rc) return rc;
+    double best = 0.0;
+    for (int i = 0; i < 4; ++i) if (v[i] > best) best = v[i];
     *out_tflops = best;
     return NRR_OK;
 }

@@ -158,5 +158,6 @@ int warp_enqueue(const float *image, Int3 dims, const float *field, float *out, 
 
 // ---- FFMA microbenchmark (nrr_fma_peak.cu) ----------------------------------------------------------
 int fp32_peak_measure(double *out_tflops, cudaStream_t stream);
+int fp32_microbench(double out[7], cudaStream_t stream);
 
 }  // namespace nrr

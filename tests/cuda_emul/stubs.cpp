@@ -9,4 +9,10 @@ int fp32_peak_measure(double *out_tflops, cudaStream_t)      // the FFMA microbe
     set_error("the FFMA microbenchmark does not exist in the emulated build");
     return NRR_E_CUDA;
 }
+int fp32_microbench(double out[7], cudaStream_t)
+{
+    for (int i = 0; i < 7; ++i) out[i] = 0.0;
+    set_error("the FP32 microbenchmarks do not exist in the emulated build");
+    return NRR_E_CUDA;
+}
 }  // namespace nrr

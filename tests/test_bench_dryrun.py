@@ -49,6 +49,32 @@ class _EmulNrr:
         out_ncc[:k] = torch.from_numpy(s)
         return out_blocks[:k], out_disp[:k], out_ncc[:k]
 
+    def nrr_bm_capacity_bound(self, dims, block, stride, frac):
+        return _emul.capacity_bound(dims, block, stride, frac)
+
+    def nrr_bm_plan_create_host(self, fixed, block, stride, window, frac, mask=None):
+        return _emul.Plan(fixed.numpy(), block, stride, window, frac, None if mask is None else mask.numpy(), host=True)
+
+    def nrr_bm_plan_create(self, fixed, block, stride, window, frac, mask=None):
+        return _emul.Plan(fixed.numpy(), block, stride, window, frac, None if mask is None else mask.numpy(), host=False)
+
+    def nrr_bm_plan_match_host(self, plan, moving, out_disp, out_ncc):
+        d, s = plan.match_host(moving.numpy())
+        out_disp[:] = torch.from_numpy(d)
+        out_ncc[:] = torch.from_numpy(s)
+        return out_disp, out_ncc
+
+    def nrr_bm_plan_match_range(self, plan, moving, out_disp, out_ncc, first=0, count=None):
+        plan.match(moving.numpy(), first, plan.n - first if count is None else count, out=(out_disp.numpy(), out_ncc.numpy()))
+        self.launches += 2
+        return out_disp, out_ncc
+
+    def nrr_bm_plan_blocks_host(self, plan):
+        return plan.blocks()[0]
+
+    def nrr_bm_plan_destroy(self, plan):
+        plan.destroy()
+
     def nrr_bm_check_async_error(self):
         pass
 
@@ -100,8 +126,15 @@ def test_bench_main_runs_end_to_end_on_the_emulated_library():
                    backend_factory=_Backend)
     line = json.loads(out.getvalue().strip().splitlines()[-1])
     for key in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
-                "vs_baseline", "dtype", "data", "config", "roofline", "cpu_baseline", "e2e", "gpu_launches", "clocks"):
+                "vs_baseline", "dtype", "data", "config", "roofline", "cpu_baseline", "e2e", "gpu_launches", "clocks",
+                "parity", "ms_per_volume_pair", "phase_ms"):
         assert key in line, key
+    par = line["parity"]      # the tiny config against the oracle, outside the timed region
+    assert par["ok"] and par["selection_equal"] and par["disp_mismatch_outside_band"] == 0 and par["blocks_checked"] == 259
+    assert par["max_abs_dncc"] <= 1e-4 and par["exempt_ties"] >= 0
+    assert set(line["ms_per_volume_pair"]) >= {"select", "match", "sum"}
+    assert line["e2e"]["plan"]["h2d_bytes_per_step"] == 64 * 64 * 32 * 4 and line["e2e"]["plan"]["value"] > 0
+    assert "traffic" in line["roofline"] and "traffic_source" in line["roofline"]
     assert line["metric"] == "blocks_per_sec" and line["unit"] == "blocks/s" and line["steps"] == 2
     assert line["config"]["workload"] == "tiny" and line["config"]["blocks_per_pair"] == 259
     rf = line["roofline"]
@@ -112,3 +145,22 @@ def test_bench_main_runs_end_to_end_on_the_emulated_library():
     e2e = line["e2e"]
     assert e2e["h2d_bytes_per_step"] == 2 * 64 * 64 * 32 * 4 and e2e["d2h_bytes_per_step"] == 259 * 28 + 4
     assert line["gpu_launches"] == 10 and line["value"] > 0 and e2e["value"] > 0
+
+
+def test_reference_arm_times_the_whole_oracle_step_and_agrees_with_cpu_baseline():
+    """the reference arm must not under-report the oracle.  On a workload whose whole step fits,
+    every reference step IS the whole oracle step; its value and the cpu_baseline leg's value describe the same
+    program on the same box and agree (loosely here: two short timings on a shared CPU)."""
+    out = io.StringIO()
+    with redirect_stdout(out):
+        bench.main(["--impl", "reference", "--workload", "tiny", "--steps", "3", "--warmup", "1"])
+    ref = json.loads(out.getvalue().strip().splitlines()[-1])
+    assert ref["impl"] == "reference" and ref["cpu_baseline"]["kind"] == "oracle" and ref["e2e"]["h2d_bytes_per_step"] == 0
+    assert "whole oracle step" in ref["cpu_baseline"]["sample"] and ref["cpu_baseline"]["value"] == ref["value"]
+    out = io.StringIO()
+    with redirect_stdout(out):
+        bench.main(["--workload", "tiny", "--steps", "1", "--warmup", "3", "--e2e-steps", "1", "--no-parity"], backend_factory=_Backend)
+    cb = json.loads(out.getvalue().strip().splitlines()[-1])["cpu_baseline"]
+    assert cb["cores"] >= 1 and cb["threads_1_value"] > 0 and cb["matching_scaling_1_to_all_threads"] > 0
+    assert "whole step" in cb["sample"]
+    assert 0.25 < cb["value"] / ref["value"] < 4.0

@@ -50,3 +50,49 @@ def test_two_ranks_shard_pairs_and_reduce(tmp_path):
     assert r[0]["t_max"] == r[1]["t_max"] == 15.0                # MAX over ranks
     assert r[0]["n_all"] == r[1]["n_all"] == r[0]["n"] + r[1]["n"]      # SUM over ranks
     assert r[0]["n"] > 0 and r[1]["n"] > 0
+
+
+def _shard_worker(rank, world, port, outdir):
+    """--shard blocks (both images on every processor, the block list distributed): each rank builds
+    the same plan, matches its slice of the canonical block list, and one all-gather of 16 B/block completes it."""
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    sys.path.insert(0, ROOT)
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    import dataclasses
+    import torch
+    import torch.distributed as dist
+    import bench
+    import _emul
+    from nrr_inputs import CONFIGS, make_pair
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    cfg = dataclasses.replace(CONFIGS["tiny"], dims=(40, 32, 24))          # the SAME pair on every rank
+    fixed, moving, mask = make_pair(cfg)
+    plan = _emul.Plan(fixed, cfg.block, cfg.stride, cfg.window, cfg.frac, mask, host=False)
+    n = plan.n
+    first, count = bench.shard_range(n, rank, world)
+    o_disp = torch.full((n, 3), -99, dtype=torch.int32)
+    o_ncc = torch.full((n,), -99.0, dtype=torch.float32)
+    plan.match(moving, first, count, out=(o_disp.numpy(), o_ncc.numpy()))
+    cmax = max(bench.shard_range(n, r, world)[1] for r in range(world))
+    send = torch.zeros((cmax, 4), dtype=torch.int32)
+    recv = torch.zeros((world, cmax, 4), dtype=torch.int32)
+    bench.exchange_block_results(dist, o_disp, o_ncc, n, rank, world, send, recv)
+    whole_d, whole_s = plan.match(moving)                                   # what one rank alone computes
+    np.save(os.path.join(outdir, "disp%d.npy" % rank), o_disp.numpy())
+    with open(os.path.join(outdir, "shard%d.json" % rank), "w") as f:
+        json.dump({"n": n, "first": first, "count": count,
+                   "equal": bool(np.array_equal(o_disp.numpy(), whole_d) and np.array_equal(o_ncc.numpy(), whole_s))}, f)
+    plan.destroy()
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_two_ranks_shard_one_block_list_and_gather(tmp_path):
+    import torch.multiprocessing as mp
+    port = _free_port()
+    mp.spawn(_shard_worker, args=(2, port, str(tmp_path)), nprocs=2, join=True)
+    r = [json.load(open(tmp_path / ("shard%d.json" % k))) for k in range(2)]
+    assert r[0]["n"] == r[1]["n"] > 4
+    assert r[0]["first"] == 0 and r[0]["count"] == r[1]["first"] and r[1]["first"] + r[1]["count"] == r[0]["n"]
+    assert r[0]["equal"] and r[1]["equal"]                       # gathered result == single-rank result, bit for bit
+    assert np.array_equal(np.load(tmp_path / "disp0.npy"), np.load(tmp_path / "disp1.npy"))
