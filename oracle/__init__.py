@@ -17,7 +17,9 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "nrr_oracle.c")
 _BUILD = os.path.join(_HERE, "build")
-_SO = os.path.join(_BUILD, "libnrr_oracle.so")
+# NRR_ORACLE_SANITIZE=1 (tests/test_oracle_sanitized.py): the same source under AddressSanitizer + UBSan
+_SANITIZE = os.environ.get("NRR_ORACLE_SANITIZE", "0") == "1"
+_SO = os.path.join(_BUILD, "libnrr_oracle_san.so" if _SANITIZE else "libnrr_oracle.so")
 _lib = None
 
 
@@ -28,6 +30,8 @@ def build(force: bool = False) -> str:
         tmp = _SO + ".tmp.%d" % os.getpid()
         cmd = ["gcc", "-O2", "-std=c99", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared",
                "-Wall", "-Wextra", "-o", tmp, _SRC, "-lm"]
+        if _SANITIZE:
+            cmd[1:2] = ["-O1", "-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=all", "-fno-omit-frame-pointer"]
         subprocess.run(cmd, check=True)
         os.replace(tmp, _SO)
     return _SO

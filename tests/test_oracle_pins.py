@@ -58,9 +58,10 @@ def test_ncc_golden(golden):
 
 
 def test_ncc_equals_numpy_corrcoef():
+    """SPEC.md:681 acceptance #1: 10^4 random block pairs against an independently coded correlation."""
     r = _rng(2)
     for n in (3, 125, 343, 729, 1331):
-        for _ in range(20):
+        for _ in range(2000):
             a = r.uniform(0, 1000, size=n).astype(np.float32)
             b = (0.3 * a + r.normal(0, 200, size=n)).astype(np.float32)
             ref = float(np.corrcoef(a.astype(np.float64), b.astype(np.float64))[0, 1])
@@ -120,8 +121,12 @@ def _bruteforce_select(vol, block, stride, frac, mask):
         var.append(np.var(vol[oz:oz + bz, oy:oy + by, ox:ox + bx].astype(np.float64)))
     var = np.asarray(var)
     k = int(math.floor(0.5 + len(cents) * frac))
-    order = np.lexsort((np.arange(len(cents)), -var))[:k]
+    full = np.lexsort((np.arange(len(cents)), -var))
+    order = full[:k]
     keep = np.sort(order)
+    # K / K+1 variance margin: how far the last kept candidate is from the first one left out
+    margin = float("nan") if k == 0 else (float("inf") if k == len(cents) else float(var[full[k - 1]] - var[full[k]]))
+    _bruteforce_select.margin = margin
     return np.asarray(cents, dtype=np.int32)[keep], var[keep], len(cents)
 
 
@@ -143,6 +148,11 @@ def test_select_matches_numpy_bruteforce(block, stride, frac, use_mask):
     assert res["n_candidates"] == n
     assert res["centres"].tolist() == cents.tolist()
     np.testing.assert_allclose(res["var"], var, rtol=1e-12)
+    want_margin = _bruteforce_select.margin           # out_margin of nrr_oracle_select, against numpy
+    if math.isinf(want_margin):
+        assert math.isinf(res["margin"]) and res["margin"] > 0
+    else:
+        assert res["margin"] >= 0 and res["margin"] == pytest.approx(want_margin, rel=1e-9, abs=1e-9)
     lin = (res["centres"][:, 2].astype(np.int64) * dims[1] + res["centres"][:, 1]) * dims[0] + res["centres"][:, 0]
     assert np.all(np.diff(lin) > 0)             # canonical ascending order (Q8)
 
@@ -352,7 +362,10 @@ def test_tiny_config_exact_recovery_with_noise():
 
 # ------------------------------------------------------------------------- selection with a connectivity pattern
 def _pruned_bruteforce(vol, block, stride, frac, mask, connectivity):
-    """Independent restatement (numpy + python sets) of reading Q20: greedy by (variance desc, index asc)."""
+    """Independent restatement (numpy + python sets) of reading Q20: greedy by (variance desc, index asc).
+    The per-candidate variance is taken from oracle.variance ON PURPOSE: that function is pinned on its own
+    (closed forms, numpy.var) and using its bits keeps exact variance ties exact, so that this pin tests the walk
+    (priority order, neighbourhood, stopping rule, output order) and nothing else."""
     nz, ny, nx = vol.shape
     g = [(n - b) // s + 1 for n, b, s in zip((nx, ny, nz), block, stride)]
     reach = {0: 0, 6: 1, 18: 2, 26: 3}[connectivity]
