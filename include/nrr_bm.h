@@ -55,6 +55,8 @@ typedef enum nrr_status {
     NRR_E_SMEM = -9,     /* block / window too large for the kernels' shared-memory or index limits */
     NRR_E_CUDA = -10,    /* a CUDA runtime call failed (message in nrr_bm_last_error) */
     NRR_E_ARG = -11,     /* other invalid argument (n < 0, capacity < 0, ...) */
+    NRR_E_NOCONV = -13,  /* nrr_bm_fem_solve: conjugate gradients did not reach the tolerance within max_cg iterations
+                            (out_u holds the last iterate) */
     NRR_E_DEVICE = -12   /* a staged copy of a matching kernel did not complete within its time bound; the blocks
                             of that CTA get out_disp = (0,0,0), out_ncc = NaN.  Reported like NRR_E_BOUNDS (sticky
                             device flag); the kernel leaves in an orderly way and never faults the GPU */
@@ -262,6 +264,52 @@ NRR_BM_API int nrr_bm_register_batch(const float *fixed, const float *moving, co
                                      const unsigned char *mask, const nrr_bm_setting *settings, int n_settings,
                                      int *const *out_blocks, const int *capacity, int *out_n, int *const *out_disp,
                                      float *const *out_ncc, void *stream);
+
+/*
+ * BIOMECHANICAL REGULARISATION of the sparse displacement field (the step that consumes out_disp / out_ncc)  --
+ * PAPER.md:252-265 (section 3): "Estimation of brain deformation is based on the finite element analysis (FEA) using a
+ * linear elastic model ... We then iteratively seek such a position of the mesh vertices U that balances the mechanical
+ * forces of the modeled tissue that resist deformation, with the external forces that correspond to the displacements D
+ * estimated by block matching:
+ *        F_i <= K U_i ,      U_{i+1} <= [K + H^T S H]^-1 [H^T S D + F_i]
+ * K is the mechanical stiffness matrix, H is the interpolation matrix from the mesh vertices to the block matching
+ * displacements, S is the matrix that captures the confidence in the block matching results"; "Both
+ * block matching and iterative estimation of displacements are time critical".
+ *
+ * Readings (Q22-Q25; the paper gives none of these).  MESH: the paper's mesher is out of scope; the model is a
+ * regular grid of nodes, `spacing` voxels apart, covering the volume (nodes per axis = max(2, ceil((n-1)/spacing) + 1),
+ * node index (k*nny + j)*nnx + i at position (i*hx, j*hy, k*hz) voxels), every cell cut into the six Kuhn tetrahedra
+ * around its main diagonal, constant-strain elements.  MATERIAL: isotropic, Young's modulus `young` >= 0 and Poisson's
+ * ratio `poisson` in (-1, 0.5) are inputs (the paper prints no constants).  S = weight * diag(max(NCC, 0)), one value per
+ * block for its three axes; blocks with NCC <= 0 or NaN have no influence.  Displacements, positions and U in voxels.
+ *
+ *   nrr_bm_fem_create       builds the model (mesh geometry, the element stiffness table, all vectors) on the current device
+ *   nrr_bm_fem_solve        U_0 = 0, then n_iter >= 1 iterations of the scheme above; each linear system is solved by
+ *                           Jacobi-preconditioned conjugate gradients in FP64 to |r| <= tol * |b|, at most max_cg
+ *                           iterations per system (NRR_E_NOCONV otherwise, with the last iterate in out_u).
+ *                           blocks / disp int32 [n][3], ncc fp32 [n] as written by nrr_bm_select_blocks / nrr_bm_match
+ *                           (DEVICE); out_u DEVICE double [n_nodes][3]; *out_cg_iters (HOST, nullable) = CG iterations
+ *                           over all systems.  Synchronises `stream` (it polls the convergence flag every 16
+ *                           iterations).  FP64 atomics accumulate H^T S H and H^T S D: bits can differ between runs in
+ *                           the last places; against the oracle's direct solve |U - U_oracle| <= 1e-6 * max(1, max|U|)
+ *                           for tol <= 1e-10.
+ *   nrr_bm_fem_dense_field  "dense deformation field that defines transformation for each point in the image space"
+ *                           (PAPER.md:225-229): out_field fp32 [3][nz][ny][nx] (component-major, what nrr_bm_warp
+ *                           takes) = U interpolated at every voxel by the barycentric weights of its tetrahedron.
+ *                           Asynchronous on `stream`.
+ *   *_host                  the same with HOST buffers; synchronise.
+ *   nrr_bm_fem_destroy      releases the model (NULL is allowed).
+ */
+typedef struct nrr_bm_fem nrr_bm_fem;
+NRR_BM_API int nrr_bm_fem_create(const int dims[3], const int spacing[3], double young, double poisson, nrr_bm_fem **out_fem);
+NRR_BM_API int nrr_bm_fem_info(const nrr_bm_fem *fem, int nodes[3], int *n_nodes);
+NRR_BM_API int nrr_bm_fem_solve(nrr_bm_fem *fem, const int *blocks, const int *disp, const float *ncc, int n, double weight,
+                                int n_iter, double tol, int max_cg, double *out_u, int *out_cg_iters, void *stream);
+NRR_BM_API int nrr_bm_fem_solve_host(nrr_bm_fem *fem, const int *blocks, const int *disp, const float *ncc, int n,
+                                     double weight, int n_iter, double tol, int max_cg, double *out_u, int *out_cg_iters);
+NRR_BM_API int nrr_bm_fem_dense_field(const nrr_bm_fem *fem, const double *u, float *out_field, void *stream);
+NRR_BM_API int nrr_bm_fem_dense_field_host(const nrr_bm_fem *fem, const double *u, float *out_field);
+NRR_BM_API int nrr_bm_fem_destroy(nrr_bm_fem *fem);
 
 /* Synchronises `stream` and returns NRR_E_DEVICE if a staged copy of a matching kernel enqueued on this thread since
  * the last check did not complete, NRR_E_BOUNDS if one saw a block leaving the volume (and clears the flag),

@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libnrr_bm.so")
 
 NRR_OK = 0
 NRR_E_NULL, NRR_E_DIMS, NRR_E_BLOCK, NRR_E_STRIDE, NRR_E_WINDOW, NRR_E_FRAC = -1, -2, -3, -4, -5, -6
-NRR_E_CAPACITY, NRR_E_BOUNDS, NRR_E_SMEM, NRR_E_CUDA, NRR_E_ARG, NRR_E_DEVICE = -7, -8, -9, -10, -11, -12
+NRR_E_CAPACITY, NRR_E_BOUNDS, NRR_E_SMEM, NRR_E_CUDA, NRR_E_ARG, NRR_E_DEVICE, NRR_E_NOCONV = -7, -8, -9, -10, -11, -12, -13
 
 EXPORTS = [
     "nrr_bm_select_blocks", "nrr_bm_select_blocks_pruned", "nrr_bm_select_blocks_pruned_host", "nrr_bm_match", "nrr_bm_register", "nrr_bm_check_async_error", "nrr_bm_moving_stats", "nrr_bm_moving_stats_host", "nrr_bm_warp", "nrr_bm_warp_host",
@@ -26,6 +26,8 @@ EXPORTS = [
     "nrr_bm_capacity_bound", "nrr_bm_plan_create", "nrr_bm_plan_create_host", "nrr_bm_plan_info", "nrr_bm_plan_blocks_host",
     "nrr_bm_plan_blocks_device", "nrr_bm_plan_match", "nrr_bm_plan_match_range", "nrr_bm_plan_match_host", "nrr_bm_plan_destroy",
     "nrr_bm_register_batch",
+    "nrr_bm_fem_create", "nrr_bm_fem_info", "nrr_bm_fem_solve", "nrr_bm_fem_solve_host", "nrr_bm_fem_dense_field",
+    "nrr_bm_fem_dense_field_host", "nrr_bm_fem_destroy",
     "nrr_bm_fp32_peak", "nrr_bm_fp32_microbench", "nrr_bm_pair_task_table", "nrr_bm_set_option", "nrr_bm_last_error", "nrr_bm_status_string", "nrr_bm_version",
 ]
 
@@ -99,6 +101,20 @@ def lib() -> ctypes.CDLL:
     L.nrr_bm_plan_destroy.argtypes = [vp]
     L.nrr_bm_register_batch.restype = ci
     L.nrr_bm_register_batch.argtypes = [vp, vp, i3, vp, vp, ci, pp, i3, vp, pp, pp, vp]
+    L.nrr_bm_fem_create.restype = ci
+    L.nrr_bm_fem_create.argtypes = [i3, i3, cd, cd, pp]
+    L.nrr_bm_fem_info.restype = ci
+    L.nrr_bm_fem_info.argtypes = [vp, i3, i3]
+    L.nrr_bm_fem_solve.restype = ci
+    L.nrr_bm_fem_solve.argtypes = [vp, vp, vp, vp, ci, cd, ci, cd, ci, vp, i3, vp]
+    L.nrr_bm_fem_solve_host.restype = ci
+    L.nrr_bm_fem_solve_host.argtypes = [vp, vp, vp, vp, ci, cd, ci, cd, ci, vp, i3]
+    L.nrr_bm_fem_dense_field.restype = ci
+    L.nrr_bm_fem_dense_field.argtypes = [vp, vp, vp, vp]
+    L.nrr_bm_fem_dense_field_host.restype = ci
+    L.nrr_bm_fem_dense_field_host.argtypes = [vp, vp, vp]
+    L.nrr_bm_fem_destroy.restype = ci
+    L.nrr_bm_fem_destroy.argtypes = [vp]
     L.nrr_bm_profile_enable.restype = ci
     L.nrr_bm_profile_enable.argtypes = [ci]
     L.nrr_bm_profile_read.restype = ci
@@ -417,6 +433,82 @@ def nrr_bm_plan_destroy(plan: NrrPlan) -> None:
         h, plan.handle = plan.handle, None
         _check(lib().nrr_bm_plan_destroy(h))
     plan._keep = None
+
+
+class NrrFem:
+    """Handle of an nrr_bm_fem model (include/nrr_bm.h "BIOMECHANICAL REGULARISATION")."""
+
+    def __init__(self, handle, dims):
+        self.handle, self.dims = handle, tuple(int(v) for v in dims)
+        nodes = (ctypes.c_int * 3)()
+        n = ctypes.c_int(0)
+        _check(lib().nrr_bm_fem_info(handle, nodes, ctypes.byref(n)))
+        self.nodes, self.n_nodes = (nodes[0], nodes[1], nodes[2]), n.value
+
+    def __del__(self):
+        try:
+            nrr_bm_fem_destroy(self)
+        except Exception:  # pragma: no cover
+            pass
+
+
+def nrr_bm_fem_create(dims, spacing, young: float, poisson: float) -> NrrFem:
+    h = ctypes.c_void_p()
+    _check(lib().nrr_bm_fem_create(_i3(dims), _i3(spacing), float(young), float(poisson), ctypes.byref(h)))
+    return NrrFem(h, dims)
+
+
+def nrr_bm_fem_solve(fem: NrrFem, blocks, disp, ncc, weight: float = 1.0, n_iter: int = 1, tol: float = 1e-10,
+                     max_cg: int = 2000, out_u=None, stream=None):
+    """Device form: blocks/disp int32 CUDA [n][3], ncc fp32 CUDA [n].  Returns (U float64 CUDA [n_nodes][3], CG iterations)."""
+    import torch
+    blocks = _dev(blocks, torch.int32, "blocks")
+    disp = _dev(disp, torch.int32, "disp")
+    ncc = _dev(ncc, torch.float32, "ncc")
+    n = int(blocks.shape[0])
+    if out_u is None:
+        out_u = torch.empty((fem.n_nodes, 3), dtype=torch.float64, device=blocks.device)
+    iters = ctypes.c_int(0)
+    with torch.cuda.device(blocks.device):
+        _check(lib().nrr_bm_fem_solve(fem.handle, blocks.data_ptr(), disp.data_ptr(), ncc.data_ptr(), n, float(weight),
+                                      int(n_iter), float(tol), int(max_cg), out_u.data_ptr(), ctypes.byref(iters), _stream_ptr(stream)))
+    return out_u, iters.value
+
+
+def nrr_bm_fem_solve_host(fem: NrrFem, blocks: np.ndarray, disp: np.ndarray, ncc: np.ndarray, weight: float = 1.0,
+                          n_iter: int = 1, tol: float = 1e-10, max_cg: int = 2000):
+    blocks, disp, ncc = _np(blocks, np.int32, "blocks"), _np(disp, np.int32, "disp"), _np(ncc, np.float32, "ncc")
+    out_u = np.empty((fem.n_nodes, 3), dtype=np.float64)
+    iters = ctypes.c_int(0)
+    _check(lib().nrr_bm_fem_solve_host(fem.handle, blocks.ctypes.data, disp.ctypes.data, ncc.ctypes.data, int(blocks.shape[0]),
+                                       float(weight), int(n_iter), float(tol), int(max_cg), out_u.ctypes.data, ctypes.byref(iters)))
+    return out_u, iters.value
+
+
+def nrr_bm_fem_dense_field(fem: NrrFem, u, out_field=None, stream=None):
+    """Device form, asynchronous: u float64 CUDA [n_nodes][3] -> field fp32 CUDA [3][nz][ny][nx] (what nrr_bm_warp takes)."""
+    import torch
+    u = _dev(u, torch.float64, "u")
+    nx, ny, nz = fem.dims
+    if out_field is None:
+        out_field = torch.empty((3, nz, ny, nx), dtype=torch.float32, device=u.device)
+    with torch.cuda.device(u.device):
+        _check(lib().nrr_bm_fem_dense_field(fem.handle, u.data_ptr(), out_field.data_ptr(), _stream_ptr(stream)))
+    return out_field
+
+
+def nrr_bm_fem_dense_field_host(fem: NrrFem, u: np.ndarray) -> np.ndarray:
+    u = _np(u, np.float64, "u")
+    nx, ny, nz = fem.dims
+    out = np.empty((3, nz, ny, nx), dtype=np.float32)
+    _check(lib().nrr_bm_fem_dense_field_host(fem.handle, u.ctypes.data, out.ctypes.data))
+    return out
+
+
+def nrr_bm_fem_destroy(fem: NrrFem) -> None:
+    if fem.handle is not None and fem.handle.value:
+        h, fem.handle = fem.handle, None
+        _check(lib().nrr_bm_fem_destroy(h))
 
 
 def nrr_bm_warp(image, field, out=None, stream=None):

@@ -8,7 +8,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-SOURCES = ["nrr_api.cu", "nrr_select.cu", "nrr_boxstat.cu", "nrr_match.cu", "nrr_match_pair.cu", "nrr_plan.cu", "nrr_warp.cu", "nrr_fma_peak.cu"]
+SOURCES = ["nrr_api.cu", "nrr_select.cu", "nrr_boxstat.cu", "nrr_match.cu", "nrr_match_pair.cu", "nrr_plan.cu", "nrr_fem.cu", "nrr_warp.cu", "nrr_fma_peak.cu"]
 HEADERS = ["nrr_internal.cuh", "nrr_match_common.cuh", os.path.join("..", "..", "include", "nrr_bm.h")]
 LIB = os.path.join(HERE, "libnrr_bm.so")
 

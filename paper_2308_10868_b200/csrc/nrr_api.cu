@@ -730,6 +730,7 @@ const char *nrr_bm_status_string(int status)
     case NRR_E_CUDA: return "NRR_E_CUDA";
     case NRR_E_ARG: return "NRR_E_ARG";
     case NRR_E_DEVICE: return "NRR_E_DEVICE";
+    case NRR_E_NOCONV: return "NRR_E_NOCONV";
     default: return "NRR_E_UNKNOWN";
     }
 }

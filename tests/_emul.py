@@ -214,3 +214,48 @@ def register_batch(fixed, moving, settings, mask=None):
                                    None if mask is None else mask.ctypes.data, arr, ns, pb, caps, out_n.ctypes.data, pd, pn, None))
     _check(L.nrr_bm_check_async_error(None))
     return [(b[:k], d[:k], c[:k]) for (b, d, c), k in zip(keep, out_n)], out_n
+
+
+# ---- biomechanical regularisation (nrr_fem.cu)
+class Fem:
+    def __init__(self, dims, spacing, young, poisson):
+        L = lib()
+        vp, ci, cd = ctypes.c_void_p, ctypes.c_int, ctypes.c_double
+        i3 = ctypes.POINTER(ctypes.c_int)
+        L.nrr_bm_fem_create.argtypes = [i3, i3, cd, cd, ctypes.POINTER(vp)]
+        L.nrr_bm_fem_info.argtypes = [vp, i3, i3]
+        L.nrr_bm_fem_solve_host.argtypes = [vp, vp, vp, vp, ci, cd, ci, cd, ci, vp, i3]
+        L.nrr_bm_fem_solve.argtypes = [vp, vp, vp, vp, ci, cd, ci, cd, ci, vp, i3, vp]
+        L.nrr_bm_fem_dense_field_host.argtypes = [vp, vp, vp]
+        L.nrr_bm_fem_destroy.argtypes = [vp]
+        self.dims = tuple(dims)
+        self.h = vp()
+        _check(L.nrr_bm_fem_create(_i3(dims), _i3(spacing), float(young), float(poisson), ctypes.byref(self.h)))
+        nodes = (ci * 3)()
+        n = ci(0)
+        _check(L.nrr_bm_fem_info(self.h, nodes, ctypes.byref(n)))
+        self.nodes, self.n_nodes = tuple(nodes), n.value
+
+    def solve(self, blocks, disp, ncc, weight=1.0, n_iter=1, tol=1e-12, max_cg=5000, allow_noconv=False):
+        blocks = np.ascontiguousarray(blocks, np.int32)
+        disp = np.ascontiguousarray(disp, np.int32)
+        ncc = np.ascontiguousarray(ncc, np.float32)
+        u = np.full((self.n_nodes, 3), np.nan)
+        iters = ctypes.c_int(0)
+        rc = lib().nrr_bm_fem_solve_host(self.h, blocks.ctypes.data, disp.ctypes.data, ncc.ctypes.data, len(blocks), float(weight),
+                                         int(n_iter), float(tol), int(max_cg), u.ctypes.data, ctypes.byref(iters))
+        if not (allow_noconv and rc == -13):
+            _check(rc)
+        return u, iters.value, rc
+
+    def dense_field(self, u):
+        nx, ny, nz = self.dims
+        out = np.empty((3, nz, ny, nx), np.float32)
+        u = np.ascontiguousarray(u, np.float64)
+        _check(lib().nrr_bm_fem_dense_field_host(self.h, u.ctypes.data, out.ctypes.data))
+        return out
+
+    def destroy(self):
+        if self.h:
+            _check(lib().nrr_bm_fem_destroy(self.h))
+            self.h = None

@@ -10,7 +10,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(os.path.dirname(HERE))
 CSRC = os.path.join(ROOT, "paper_2308_10868_b200", "csrc")
-SOURCES = ["nrr_api.cu", "nrr_select.cu", "nrr_boxstat.cu", "nrr_match.cu", "nrr_match_pair.cu", "nrr_plan.cu", "nrr_warp.cu"]   # not the FFMA microbenchmark
+SOURCES = ["nrr_api.cu", "nrr_select.cu", "nrr_boxstat.cu", "nrr_match.cu", "nrr_match_pair.cu", "nrr_plan.cu", "nrr_fem.cu", "nrr_warp.cu"]   # not the FFMA microbenchmark
 ASAN = os.environ.get("NRR_EMUL_ASAN", "0") == "1"      # AddressSanitizer build: LD_PRELOAD libasan when loading it
 LIB = os.path.join(HERE, "libnrr_bm_emul_asan.so" if ASAN else "libnrr_bm_emul.so")
 FLAGS = ["-std=c++17", "-O1", "-g", "-ffp-contract=off", "-fPIC", "-fvisibility=hidden", "-fno-strict-aliasing",

@@ -91,6 +91,16 @@ fake.nrr_bm_plan_match = plan_match
 fake.nrr_bm_plan_match_range = plan_match
 fake.nrr_bm_plan_match_host = lambda plan, moving, out_disp=None, out_ncc=None: plan.p.match_host(moving)
 fake.nrr_bm_plan_destroy = lambda plan: plan.p.destroy()
+class _Fem:
+    def __init__(self, f): self.f, self.nodes, self.n_nodes, self.dims = f, f.nodes, f.n_nodes, f.dims
+def fem_solve(fem, blocks, disp, ncc, weight=1.0, n_iter=1, tol=1e-10, max_cg=2000, out_u=None, stream=None):
+    u, it, _ = fem.f.solve(_np(blocks), _np(disp), _np(ncc), weight, n_iter, tol, max_cg)
+    return torch.from_numpy(u), it
+fake.nrr_bm_fem_create = lambda dims, spacing, young, poisson: _Fem(_emul.Fem(dims, spacing, young, poisson))
+fake.nrr_bm_fem_solve = fem_solve
+fake.nrr_bm_fem_solve_host = lambda fem, b, d, c, weight=1.0, n_iter=1, tol=1e-10, max_cg=2000: fem.f.solve(b, d, c, weight, n_iter, tol, max_cg)[:2]
+fake.nrr_bm_fem_dense_field = lambda fem, u, out_field=None, stream=None: torch.from_numpy(fem.f.dense_field(u.numpy()))
+fake.nrr_bm_fem_destroy = lambda fem: fem.f.destroy()
 fake.nrr_bm_register_batch = register_batch
 fake.nrr_bm_capacity_bound = _emul.capacity_bound
 fake.nrr_bm_select_blocks = select

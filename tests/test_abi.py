@@ -105,6 +105,15 @@ def test_argument_validation_happens_before_cuda(nrr):
     assert L.nrr_bm_plan_info(None, None, None) == -11 and L.nrr_bm_plan_destroy(None) == 0
     assert L.nrr_bm_register_batch(p, p, i3(8, 8, 8), None, None, 0, None, None, None, None, None, None) == 0       # nothing to do
     assert L.nrr_bm_register_batch(p, p, i3(8, 8, 8), None, None, 2, None, None, None, None, None, None) == -1
+    fh = ctypes.c_void_p()
+    assert L.nrr_bm_fem_create(i3(8, 8, 8), i3(2, 0, 2), 1.0, 0.3, ctypes.byref(fh)) == -4
+    assert L.nrr_bm_fem_create(i3(8, 8, 8), i3(2, 2, 2), -1.0, 0.3, ctypes.byref(fh)) == -11
+    assert L.nrr_bm_fem_create(i3(8, 8, 8), i3(2, 2, 2), 1.0, 0.5, ctypes.byref(fh)) == -11      # incompressible: lambda is infinite
+    assert L.nrr_bm_fem_create(i3(8, 8, 8), i3(2, 2, 2), 1.0, 0.3, None) == -1
+    assert not fh.value and L.nrr_bm_fem_destroy(None) == 0
+    assert L.nrr_bm_fem_solve(None, p, p, p, 1, 1.0, 1, 1e-10, 10, p, None, None) == -11
+    assert L.nrr_bm_fem_dense_field(None, p, p, None) == -11
+    assert nrr.lib().nrr_bm_status_string(-13) == b"NRR_E_NOCONV"
     st = (nrr.nrr_bm_setting * 1)()
     st[0].block[:] = [3, 3, 3]; st[0].stride[:] = [1, 1, 1]; st[0].window[:] = [1, 1, 1]; st[0].frac = 7.0
     one = (ctypes.c_void_p * 1)(p.value)
