@@ -107,7 +107,7 @@ template <int B>
 struct SlideCfg {
     static constexpr int NT = 256;
     static constexpr int TX = 64;
-    static constexpr int TY = B <= 7 ? 18 : (B == 9 ? 16 : 14);
+    static constexpr int TY = B <= 5 ? 18 : 14;      // 14 keeps <7> and <9> free of register spills (ptxas -v)
     static constexpr int HX = TX + B - 1, HY = TY + B - 1;
     static constexpr int NCOL = (HX * HY + NT - 1) / NT;
     static constexpr int ZP = HX | 1;            // pitch of s_z rows, in double2 (odd: conflict-free column walks)

@@ -34,7 +34,7 @@ constexpr size_t kStack = 256 * 1024;
 
 struct Fiber {
     ucontext_t ctx;
-    std::vector<unsigned char> stack;
+    unsigned char *stack = nullptr;      // from the grow-only pool below: launches do not re-allocate (and re-fault) them
     bool done = false;
     uint3 tid;
     int linear, warp, lane;
@@ -76,7 +76,7 @@ void switch_to_fiber(Cta *c, Fiber *f)
 {
 #if EMUL_ASAN
     void *fake = nullptr;
-    __sanitizer_start_switch_fiber(&fake, f->stack.data(), f->stack.size());
+    __sanitizer_start_switch_fiber(&fake, f->stack, kStack);
     swapcontext(&c->sched, &f->ctx);
     __sanitizer_finish_switch_fiber(fake, nullptr, nullptr);
 #else
@@ -278,7 +278,13 @@ void launch(dim3 grid, dim3 block, size_t smem, const std::function<void()> &bod
     cta.smem_raw = raw;
     cta.smem_bytes = 128 + smem + 16;
     cta.smem_aligned = raw + 128 + 16;
-    for (Fiber &f : cta.fibers) f.stack.resize(kStack);
+    static std::vector<unsigned char *> stack_pool;      // launches are serial: one pool serves them all
+    while ((int)stack_pool.size() < nthreads) {
+        void *p = nullptr;
+        if (posix_memalign(&p, 64, kStack) != 0) trap("out of memory");
+        stack_pool.push_back((unsigned char *)p);
+    }
+    for (int t = 0; t < nthreads; ++t) cta.fibers[t].stack = stack_pool[(size_t)t];
     // scheduling order of the runnable threads inside a CTA (default: ascending thread index)
     int sched_mode = 0;
     unsigned long long rng = 0x9E3779B97F4A7C15ull;
@@ -314,8 +320,8 @@ void launch(dim3 grid, dim3 block, size_t smem, const std::function<void()> &bod
                     f.tid = uint3{(unsigned)t % block.x, ((unsigned)t / block.x) % block.y, (unsigned)t / (block.x * block.y)};
                     cta.warps[f.warp].live_mask |= 1u << f.lane;
                     getcontext(&f.ctx);
-                    f.ctx.uc_stack.ss_sp = f.stack.data();
-                    f.ctx.uc_stack.ss_size = f.stack.size();
+                    f.ctx.uc_stack.ss_sp = f.stack;
+                    f.ctx.uc_stack.ss_size = kStack;
                     f.ctx.uc_link = nullptr;
                     makecontext(&f.ctx, (void (*)())fiber_entry, 0);
                 }

@@ -192,6 +192,69 @@ def case_warp():
     print("ok warp", flush=True)
 
 
+def case_plan():
+    """Plans (pre-operative select + records, intra-operative match; slab-pipelined host form; block ranges)."""
+    vp = ctypes.c_void_p
+    L.nrr_bm_plan_create_host.argtypes = [vp, i3p, i3p, i3p, i3p, cd, vp, ci, ctypes.POINTER(vp)]
+    L.nrr_bm_plan_info.argtypes = [vp, i3p, i3p]
+    L.nrr_bm_plan_blocks_host.argtypes = [vp, vp, vp]
+    L.nrr_bm_plan_match_host.argtypes = [vp, vp, vp, vp]
+    L.nrr_bm_plan_destroy.argtypes = [vp]
+    dims, block, stride, window, frac = (48, 40, 30), (7, 7, 7), (5, 5, 5), (5, 5, 3), 0.5
+    vol = smooth(dims, 500)
+    mov = shift_noise(vol, (1, -1, 1), 12.0, 501)
+    mask = spherical_mask(dims, 18.0)
+    h = vp()
+    check(L.nrr_bm_plan_create_host(vol.ctypes.data, i3(dims), i3(block), i3(stride), i3(window), frac, mask.ctypes.data, 0,
+                                    ctypes.byref(h)), "plan_create_host")
+    n, nc = ci(0), ci(0)
+    check(L.nrr_bm_plan_info(h, ctypes.byref(n), ctypes.byref(nc)), "plan_info")
+    blocks = np.empty((n.value, 3), np.int32)
+    check(L.nrr_bm_plan_blocks_host(h, blocks.ctypes.data, None), "plan_blocks_host")
+    sel = oracle.select(vol, block, stride, frac, mask)
+    assert n.value == len(sel["centres"]) and np.array_equal(blocks, sel["centres"])
+    ora = oracle.match(vol, mov, sel["centres"], block, window)
+    for slabs in (4, 1, 7):
+        opt("plan_slabs", slabs)
+        disp = np.full((n.value, 3), -99, np.int32)
+        ncc = np.full((n.value,), -99.0, np.float32)
+        check(L.nrr_bm_plan_match_host(h, mov.ctypes.data, disp.ctypes.data, ncc.ctypes.data), "plan_match_host")
+        assert_match_parity(disp, ncc, ora, label="plan, %d slabs" % slabs)
+    opt("plan_slabs", 4)
+    check(L.nrr_bm_plan_destroy(h), "plan_destroy")
+    print("ok plan (host form, slabs 4/1/7): %d blocks" % n.value, flush=True)
+
+
+def case_fem():
+    """FEM regularisation: cell table, FP64 scatter, PCG, dense field -- against the oracle's direct solve."""
+    from oracle import fem as ofem
+    vp = ctypes.c_void_p
+    L.nrr_bm_fem_create.argtypes = [i3p, i3p, cd, cd, ctypes.POINTER(vp)]
+    L.nrr_bm_fem_solve_host.argtypes = [vp, vp, vp, vp, ci, cd, ci, cd, ci, vp, i3p]
+    L.nrr_bm_fem_dense_field_host.argtypes = [vp, vp, vp]
+    L.nrr_bm_fem_destroy.argtypes = [vp]
+    dims, spacing = (13, 9, 11), (4, 2, 5)
+    rng = np.random.default_rng(11)
+    msh = ofem.mesh(dims, spacing)
+    blocks = np.vstack([msh["xyz"][np.all(msh["xyz"] < np.asarray(dims), axis=1)],
+                        np.floor(rng.uniform(0, np.asarray(dims) - 1e-9, (150, 3)))]).astype(np.int32)
+    disp = rng.integers(-3, 4, blocks.shape).astype(np.int32)
+    ncc = rng.uniform(-0.2, 1.0, len(blocks)).astype(np.float32)
+    h = vp()
+    check(L.nrr_bm_fem_create(i3(dims), i3(spacing), 3.0, 0.45, ctypes.byref(h)), "fem_create")
+    u = np.empty((len(msh["xyz"]), 3))
+    it = ci(0)
+    check(L.nrr_bm_fem_solve_host(h, blocks.ctypes.data, disp.ctypes.data, ncc.ctypes.data, len(blocks), 0.5, 3, 1e-12, 5000,
+                                  u.ctypes.data, ctypes.byref(it)), "fem_solve_host")
+    want = ofem.solve(msh, 3.0, 0.45, blocks, disp, ncc, 0.5, 3)["U"]
+    assert np.max(np.abs(u - want)) <= 1e-6 * max(1.0, np.max(np.abs(want)))
+    field = np.empty((3, dims[2], dims[1], dims[0]), np.float32)
+    check(L.nrr_bm_fem_dense_field_host(h, u.ctypes.data, field.ctypes.data), "fem_dense_field_host")
+    assert np.max(np.abs(field - ofem.dense_field(msh, u, dims))) <= 2e-6 * max(1.0, np.max(np.abs(u)))
+    check(L.nrr_bm_fem_destroy(h), "fem_destroy")
+    print("ok fem: %d nodes, %d CG iterations" % (len(u), it.value), flush=True)
+
+
 def main():
     quick = "--quick" in sys.argv
     # ---- selection: unrolled cubic statistics + single-CTA tail, runtime-shaped statistics, multi-launch select
@@ -230,8 +293,10 @@ def main():
         case_match((40, 36, 24), (3, 5, 3), (2, 1, 3), expect_kernel=0)
         case_match((33, 31, 29), (7, 7, 7), (4, 4, 4), expect_kernel=0)
     case_register()
+    case_plan()
     if not quick:
         case_warp()
+        case_fem()
     print("ALL OK", flush=True)
 
 

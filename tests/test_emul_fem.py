@@ -24,7 +24,7 @@ def _case(dims, spacing, n_blocks, seed, amp=3):
 
 @pytest.mark.parametrize("dims,spacing,young,poisson,weight,n_iter", [
     ((13, 9, 11), (4, 2, 5), 3.0, 0.30, 1.0, 1),          # anisotropic cells, the classical regularised solution
-    ((13, 9, 11), (4, 2, 5), 3.0, 0.45, 0.5, 4),          # nearly incompressible, several F / U iterations
+    ((13, 9, 11), (4, 4, 5), 3.0, 0.45, 0.5, 2),          # nearly incompressible, two F / U iterations
     ((20, 20, 12), (5, 5, 5), 1.0, 0.10, 10.0, 2),
     ((9, 9, 9), (16, 16, 16), 2.0, 0.2, 1.0, 1),          # one cell: spacing beyond the volume
 ])
@@ -44,12 +44,12 @@ def test_emulated_fem_solve_matches_the_oracle(dims, spacing, young, poisson, we
 
 
 def test_emulated_fem_rigid_translation_and_empty_input():
-    dims, spacing = (16, 12, 10), (5, 4, 3)
+    dims, spacing = (13, 9, 11), (4, 4, 5)
     msh, blocks, _, ncc = _case(dims, spacing, 60, 5)
     ncc = np.abs(np.nan_to_num(ncc, nan=0.5)) + 0.1
     disp = np.tile(np.asarray([2, -1, 3], np.int32), (len(blocks), 1))
     f = _emul.Fem(dims, spacing, 5.0, 0.4)
-    u, iters, _ = f.solve(blocks, disp, ncc, 0.7, 3)
+    u, iters, _ = f.solve(blocks, disp, ncc, 0.7, 2)
     assert np.allclose(u, [2.0, -1.0, 3.0], atol=1e-8)          # K annihilates rigid translations: recovered exactly
     u0, it0, _ = f.solve(blocks[:0], disp[:0], ncc[:0], 1.0, 2)
     assert np.all(u0 == 0.0) and it0 == 0                        # nothing to fit: U = 0, no CG iteration

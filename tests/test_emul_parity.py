@@ -292,7 +292,7 @@ def test_emulated_staging_timeout_is_an_error_code_not_a_fault():
 @pytest.mark.parametrize("dims,block,stride,window,frac,mask_r", [
     ((48, 40, 30), (7, 7, 7), (5, 5, 5), (5, 5, 3), 0.5, 18.0),      # pair kernel, TMA staging, records kept by the plan
     ((41, 37, 29), (5, 5, 5), (4, 4, 4), (3, 3, 3), 0.3, None),      # nx % 4 != 0: plain staging
-    ((40, 36, 24), (3, 5, 3), (3, 3, 3), (2, 1, 3), 0.4, None),      # generic kernel: no records
+    ((24, 20, 16), (3, 5, 3), (4, 4, 4), (1, 1, 2), 0.5, None),      # generic kernel: no records
 ])
 def test_emulated_plan_equals_select_then_match(dims, block, stride, window, frac, mask_r):
     """pre-operative plan (selection + fixed-block records), intra-operative match.  Bit-equal to
@@ -310,7 +310,7 @@ def test_emulated_plan_equals_select_then_match(dims, block, stride, window, fra
             want_d, want_n = _emul.match(fixed, moving, blocks, block, window)
             d, s = plan.match(moving)
             assert np.array_equal(d, want_d) and np.array_equal(s, want_n)
-            for slabs in (1, 2, 3, 7, 1000):
+            for slabs in (1, 3, 1000):
                 _emul.set_option("plan_slabs", slabs)
                 d, s = plan.match_host(moving)
                 assert np.array_equal(d, want_d) and np.array_equal(s, want_n), slabs

@@ -8,7 +8,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 QUICK = ("(test_select_parity_small or test_select_uniform or test_select_mask or test_match_parity_small or every_kernel "
          "or zero_blocks or exact_ties or host_forms or moving_stats or (register and tiny) or (warp and dims0) "
-         "or (pruned and dims0-6) or (plan_equals and tiny) or staging_timeout or (fem_solve and dims0)) and not 11-11")
+         "or (pruned and dims0-6) or staging_timeout or (fem_solve and dims0)) and not 11-11")
 
 
 def test_gpu_test_file_runs_on_the_emulated_library():
