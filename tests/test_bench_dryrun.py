@@ -25,8 +25,16 @@ class _Event:
 class _EmulNrr:
     """The subset of the binding bench.py uses, on CPU tensors."""
 
+    NrrError = RuntimeError
+    broken_default = False          # test hook: the default kernels give wrong displacements until the fallback is chosen
+
     def __init__(self):
         self.launches = 0
+        self.options = {}
+
+    def nrr_bm_set_option(self, name, value):
+        self.options[name] = value
+        _emul.set_option(name, value)
 
     def lib(self):
         return _emul.lib()
@@ -36,6 +44,8 @@ class _EmulNrr:
         n = min(len(b), capacity)
         out_blocks[:n] = torch.from_numpy(b[:n])
         out_disp[:n] = torch.from_numpy(d[:n])
+        if self.broken_default and not self.options.get("force_rows"):
+            out_disp[:n, 0] += 1
         out_ncc[:n] = torch.from_numpy(s[:n])
         out_n.fill_(len(b))
         self.launches += 5
@@ -164,3 +174,26 @@ def test_reference_arm_times_the_whole_oracle_step_and_agrees_with_cpu_baseline(
     assert cb["cores"] >= 1 and cb["threads_1_value"] > 0 and cb["matching_scaling_1_to_all_threads"] > 0
     assert "whole step" in cb["sample"]
     assert 0.25 < cb["value"] / ref["value"] < 4.0
+
+
+def test_bench_falls_back_to_the_round_1_kernels_when_parity_fails():
+    """Parity is the first gate: wrong results from the default kernels must not be timed.  The run switches, loudly,
+    to the kernels measured in round 1 (never to the CPU) and says so in the line."""
+    class Broken(_EmulNrr):
+        broken_default = True
+
+    class B(_Backend):
+        def __init__(self, local_rank):
+            super().__init__(local_rank)
+            self.nrr = Broken()
+
+    out = io.StringIO()
+    try:
+        with redirect_stdout(out):
+            bench.main(["--workload", "tiny", "--steps", "1", "--warmup", "3", "--e2e-steps", "1", "--no-cpu-baseline"], backend_factory=B)
+    finally:
+        for name in ("force_rows", "boxstat_generic", "select_generic"):
+            _emul.set_option(name, 0)
+    line = json.loads(out.getvalue().strip().splitlines()[-1])
+    assert line["kernel_fallback"] and "parity" in line["kernel_fallback"]
+    assert line["parity"]["ok"] and line["roofline"]["kernel"] == "match_rows_kernel"
