@@ -38,6 +38,8 @@ struct DevState {
     cudaStream_t host_stream = nullptr;    // stream of the *_host entry points
     cudaStream_t side_stream = nullptr;    // nrr_bm_register: moving statistics run beside the selection
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    cudaStream_t copy_stream = nullptr;    // nrr_bm_register_host: the intra-operative volume goes up beside the selection
+    cudaEvent_t ev_alloc = nullptr, ev_moving = nullptr;
     static constexpr int kSide = 4;
     cudaStream_t side[kSide] = {};         // nrr_bm_register_batch / plans: matching launches spread over streams
 };
@@ -203,8 +205,11 @@ int match_device(const float *fixed, const float *moving, const int dims[3], con
 // on K known on the host and read K itself from the selection state on the device.
 int register_device(const float *fixed, const float *moving, const int dims[3], const int block[3],
                     const int stride[3], const int window[3], double frac, const unsigned char *mask, int *out_blocks,
-                    int capacity, int *out_n_dev, int *out_disp, float *out_ncc, cudaStream_t stream)
+                    int capacity, int *out_n_dev, int *out_disp, float *out_ncc, cudaStream_t stream,
+                    cudaEvent_t moving_ready = nullptr)
 {
+    // moving_ready (nullable): `moving` is still being written on another stream; only the kernels that read it (the
+    // moving statistics, and through the join the matching kernels) wait for the event -- the selection does not.
     int rc = ensure_thread_state();
     if (rc) return rc;
     MatchPlan plan;
@@ -230,6 +235,7 @@ int register_device(const float *fixed, const float *moving, const int dims[3], 
         }
         NRR_CUDA(cudaEventRecord(t_ev_fork, stream));
         NRR_CUDA(cudaStreamWaitEvent(t_side_stream, t_ev_fork, 0));
+        if (moving_ready) NRR_CUDA(cudaStreamWaitEvent(t_side_stream, moving_ready, 0));
         Span s1(1, t_side_stream);
         rc = boxstat_enqueue(moving, i3(dims), i3(block), inv_sd, t_side_stream);
         s1.stop();
@@ -603,10 +609,24 @@ int nrr_bm_register_host(const float *fixed, const float *moving, const int dims
     cudaStream_t s;
     if ((rc = host_stream(&s))) return rc;
     const size_t nvox = (size_t)dims[0] * dims[1] * dims[2];
+    if ((rc = ensure_thread_state())) return rc;
     DevBuf d_fixed(s), d_moving(s), d_mask(s), d_blocks(s), d_disp(s), d_ncc(s);
+    // The pre-operative inputs go up first, on the compute stream: the selection needs nothing else.  The
+    // intra-operative volume follows on a copy stream, so that it is in flight while the selection kernels run; only
+    // the moving statistics and the matching kernels wait for it.
+    NRR_CUDA(d_moving.alloc(nvox * sizeof(float)));
+    DevState &d = ds();
+    if (!d.copy_stream) {
+        NRR_CUDA(cudaStreamCreateWithFlags(&d.copy_stream, cudaStreamNonBlocking));
+        NRR_CUDA(cudaEventCreateWithFlags(&d.ev_alloc, cudaEventDisableTiming));
+        NRR_CUDA(cudaEventCreateWithFlags(&d.ev_moving, cudaEventDisableTiming));
+    }
+    NRR_CUDA(cudaEventRecord(d.ev_alloc, s));                       // the allocation is ordered on s
     NRR_CUDA(d_fixed.upload(fixed, nvox * sizeof(float)));
     if (mask) NRR_CUDA(d_mask.upload(mask, nvox));
-    NRR_CUDA(d_moving.upload(moving, nvox * sizeof(float)));      // overlaps the selection kernels' queueing
+    NRR_CUDA(cudaStreamWaitEvent(d.copy_stream, d.ev_alloc, 0));
+    NRR_CUDA(cudaMemcpyAsync(d_moving.p, moving, nvox * sizeof(float), cudaMemcpyHostToDevice, d.copy_stream));
+    NRR_CUDA(cudaEventRecord(d.ev_moving, d.copy_stream));
     NRR_CUDA(d_blocks.alloc((size_t)capacity * 3 * sizeof(int)));
     DevBuf d_n(s);
     NRR_CUDA(d_n.alloc(sizeof(int)));
@@ -614,7 +634,9 @@ int nrr_bm_register_host(const float *fixed, const float *moving, const int dims
     NRR_CUDA(d_ncc.alloc((size_t)capacity * sizeof(float)));
     rc = register_device((const float *)d_fixed.p, (const float *)d_moving.p, dims, block, stride, window, frac,
                          (const unsigned char *)d_mask.p, (int *)d_blocks.p, capacity, (int *)d_n.p, (int *)d_disp.p,
-                         (float *)d_ncc.p, s);
+                         (float *)d_ncc.p, s, d.ev_moving);
+    // on every path the compute stream is ordered behind the upload before the buffer is released on it
+    if (cudaStreamWaitEvent(s, d.ev_moving, 0) != cudaSuccess && rc == NRR_OK) rc = fail(NRR_E_CUDA, "join of the copy stream failed");
     if (rc) return rc;
     int *h_n = (int *)((char *)t_pinned + 2048);
     NRR_CUDA(cudaMemcpyAsync(h_n, d_n.p, sizeof(int), cudaMemcpyDeviceToHost, s));
