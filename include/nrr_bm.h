@@ -236,6 +236,9 @@ NRR_BM_API int nrr_bm_plan_info(const nrr_bm_plan *plan, int *out_n, int *out_nc
 NRR_BM_API int nrr_bm_plan_blocks_host(const nrr_bm_plan *plan, int *out_blocks, double *out_var);
 /* DEVICE pointer to the plan's block centres [n][3] (owned by the plan, valid until nrr_bm_plan_destroy). */
 NRR_BM_API const int *nrr_bm_plan_blocks_device(const nrr_bm_plan *plan);
+/* Copies the block centres [n][3] (and, if out_var != NULL, the variances [n]) into caller-owned DEVICE buffers,
+ * asynchronously on `stream`. */
+NRR_BM_API int nrr_bm_plan_blocks(const nrr_bm_plan *plan, int *out_blocks, double *out_var, void *stream);
 NRR_BM_API int nrr_bm_plan_match(nrr_bm_plan *plan, const float *moving, int *out_disp, float *out_ncc, void *stream);
 NRR_BM_API int nrr_bm_plan_match_range(nrr_bm_plan *plan, const float *moving, int first, int count, int *out_disp,
                                        float *out_ncc, void *stream);

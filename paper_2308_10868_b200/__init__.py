@@ -9,7 +9,7 @@ from .binding import (  # noqa: F401
     nrr_bm_match_info, nrr_bm_pair_task_table, nrr_bm_profile_enable, nrr_bm_profile_read, nrr_bm_register_host, nrr_bm_select_blocks,
     nrr_bm_select_blocks_pruned,
     nrr_bm_select_blocks_host, nrr_bm_set_option, nrr_bm_version, nrr_bm_warp,
-    NrrPlan, nrr_bm_capacity_bound, nrr_bm_plan_blocks_host, nrr_bm_plan_create, nrr_bm_plan_create_host, nrr_bm_plan_destroy,
+    NrrPlan, nrr_bm_capacity_bound, nrr_bm_plan_blocks, nrr_bm_plan_blocks_host, nrr_bm_plan_create, nrr_bm_plan_create_host, nrr_bm_plan_destroy,
     NrrFem, nrr_bm_fem_create, nrr_bm_fem_dense_field, nrr_bm_fem_dense_field_host, nrr_bm_fem_destroy, nrr_bm_fem_solve,
     nrr_bm_fem_solve_host,
     nrr_bm_plan_info, nrr_bm_plan_match, nrr_bm_plan_match_host, nrr_bm_plan_match_range, nrr_bm_register_batch, nrr_bm_setting,

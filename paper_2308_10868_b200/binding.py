@@ -24,7 +24,7 @@ EXPORTS = [
     "nrr_bm_select_blocks_host", "nrr_bm_match_host", "nrr_bm_register_host",
     "nrr_bm_profile_enable", "nrr_bm_profile_read", "nrr_bm_launch_count", "nrr_bm_match_info",
     "nrr_bm_capacity_bound", "nrr_bm_plan_create", "nrr_bm_plan_create_host", "nrr_bm_plan_info", "nrr_bm_plan_blocks_host",
-    "nrr_bm_plan_blocks_device", "nrr_bm_plan_match", "nrr_bm_plan_match_range", "nrr_bm_plan_match_host", "nrr_bm_plan_destroy",
+    "nrr_bm_plan_blocks_device", "nrr_bm_plan_blocks", "nrr_bm_plan_match", "nrr_bm_plan_match_range", "nrr_bm_plan_match_host", "nrr_bm_plan_destroy",
     "nrr_bm_register_batch",
     "nrr_bm_fem_create", "nrr_bm_fem_info", "nrr_bm_fem_solve", "nrr_bm_fem_solve_host", "nrr_bm_fem_dense_field",
     "nrr_bm_fem_dense_field_host", "nrr_bm_fem_destroy",
@@ -89,6 +89,8 @@ def lib() -> ctypes.CDLL:
     L.nrr_bm_plan_info.argtypes = [vp, i3, i3]
     L.nrr_bm_plan_blocks_host.restype = ci
     L.nrr_bm_plan_blocks_host.argtypes = [vp, vp, vp]
+    L.nrr_bm_plan_blocks.restype = ci
+    L.nrr_bm_plan_blocks.argtypes = [vp, vp, vp, vp]
     L.nrr_bm_plan_blocks_device.restype = vp
     L.nrr_bm_plan_blocks_device.argtypes = [vp]
     L.nrr_bm_plan_match.restype = ci
@@ -392,6 +394,17 @@ def nrr_bm_plan_blocks_host(plan: NrrPlan, want_var: bool = False):
     blocks = np.empty((plan.n, 3), dtype=np.int32)
     var = np.empty((plan.n,), dtype=np.float64) if want_var else None
     _check(lib().nrr_bm_plan_blocks_host(plan.handle, blocks.ctypes.data, var.ctypes.data if want_var else None))
+    return (blocks, var) if want_var else blocks
+
+
+def nrr_bm_plan_blocks(plan: NrrPlan, device=None, want_var: bool = False, stream=None):
+    """The plan's block centres as a CUDA int32 tensor [n][3] (a copy), optionally with the variances (float64 [n])."""
+    import torch
+    dev = device if device is not None else torch.device("cuda", torch.cuda.current_device())
+    blocks = torch.empty((plan.n, 3), dtype=torch.int32, device=dev)
+    var = torch.empty((plan.n,), dtype=torch.float64, device=dev) if want_var else None
+    with torch.cuda.device(dev):
+        _check(lib().nrr_bm_plan_blocks(plan.handle, blocks.data_ptr(), var.data_ptr() if want_var else None, _stream_ptr(stream)))
     return (blocks, var) if want_var else blocks
 
 

@@ -262,6 +262,17 @@ int nrr_bm_plan_blocks_host(const nrr_bm_plan *plan, int *out_blocks, double *ou
     return NRR_OK;
 }
 
+int nrr_bm_plan_blocks(const nrr_bm_plan *plan, int *out_blocks, double *out_var, void *stream)
+{
+    int rc = plan_ok(plan);
+    if (rc) return rc;
+    if (plan->n > 0 && !out_blocks) return api_fail(NRR_E_NULL, "out_blocks is NULL");
+    if (plan->n == 0) return NRR_OK;
+    NRR_CUDA(cudaMemcpyAsync(out_blocks, plan->blocks, (size_t)plan->n * 3 * sizeof(int), cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+    if (out_var) NRR_CUDA(cudaMemcpyAsync(out_var, plan->var, (size_t)plan->n * sizeof(double), cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+    return NRR_OK;
+}
+
 const int *nrr_bm_plan_blocks_device(const nrr_bm_plan *plan)
 {
     if (!plan || plan->magic != kPlanMagic) { api_fail(NRR_E_ARG, "not a live nrr_bm_plan"); return nullptr; }

@@ -87,6 +87,7 @@ fake.nrr_bm_plan_create = plan_create
 fake.nrr_bm_plan_create_host = plan_create_host
 fake.nrr_bm_plan_info = lambda plan: (plan.n, plan.ncand)
 fake.nrr_bm_plan_blocks_host = lambda plan, want_var=False: plan.p.blocks() if want_var else plan.p.blocks()[0]
+fake.nrr_bm_plan_blocks = lambda plan, device=None, want_var=False, stream=None: torch.from_numpy(plan.p.blocks()[0])
 fake.nrr_bm_plan_match = plan_match
 fake.nrr_bm_plan_match_range = plan_match
 fake.nrr_bm_plan_match_host = lambda plan, moving, out_disp=None, out_ncc=None: plan.p.match_host(moving)

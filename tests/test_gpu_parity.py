@@ -420,6 +420,7 @@ def test_plan_equals_select_then_match(name):
     plan = nrr.nrr_bm_plan_create(f, cfg.block, cfg.stride, cfg.window, cfg.frac, k)
     assert nrr.nrr_bm_plan_info(plan) == (n, ncand)
     assert np.array_equal(nrr.nrr_bm_plan_blocks_host(plan), blocks.cpu().numpy())
+    assert torch.equal(nrr.nrr_bm_plan_blocks(plan), blocks)
     for _ in range(2):                                               # a plan serves many intra-operative volumes
         pd, pn = nrr.nrr_bm_plan_match(plan, m)
         nrr.nrr_bm_check_async_error()
