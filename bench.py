@@ -525,27 +525,32 @@ def main(argv=None, backend_factory=CudaBackend):
            "call": "torch pinned copies + nrr_bm_register_batch" if is_batch else "nrr_bm_register_host (pre- and intra-operative work, both volumes uploaded)"}
     # plan form: the pre-operative half is done once; a step uploads the intra-operative volume only
     if not is_batch:
-        hplan = nrr.nrr_bm_plan_create_host(fixed_p, block, stride, window, frac, mask_p)
-        pd = be.pin(torch.empty((hplan.n, 3), dtype=torch.int32))
-        pn = be.pin(torch.empty((hplan.n,), dtype=torch.float32))
-        for _ in range(3):
-            nrr.nrr_bm_plan_match_host(hplan, moving_p, pd, pn)
-        barrier()
-        t_plan = 0.0
-        for _ in range(e2e_steps):
-            flush.zero_()
-            be.sync()
-            t0 = time.perf_counter()
-            nrr.nrr_bm_plan_match_host(hplan, moving_p, pd, pn)
-            t_plan += time.perf_counter() - t0
-        barrier()
-        assert np.array_equal(np.asarray(pd), res[0][1]), "plan and register forms disagree"
-        t_plan_max, plan_blocks = reduce_over_ranks(t_plan, float(hplan.n) * e2e_steps, world, dev, dist)
-        e2e["plan"] = {"value": plan_blocks / t_plan_max, "unit": UNIT, "ms_per_step": 1e3 * t_plan_max / e2e_steps,
-                       "h2d_bytes_per_step": moving_h.nbytes, "d2h_bytes_per_step": int(hplan.n) * 16,
-                       "call": "nrr_bm_plan_match_host (intra-operative work only; selection and fixed-block records "
-                               "were made by nrr_bm_plan_create_host before the timed region)"}
-        nrr.nrr_bm_plan_destroy(hplan)
+        try:      # a secondary leg: on one GPU its failure is reported in the line, it does not cost the line
+            hplan = nrr.nrr_bm_plan_create_host(fixed_p, block, stride, window, frac, mask_p)
+            pd = be.pin(torch.empty((hplan.n, 3), dtype=torch.int32))
+            pn = be.pin(torch.empty((hplan.n,), dtype=torch.float32))
+            for _ in range(3):
+                nrr.nrr_bm_plan_match_host(hplan, moving_p, pd, pn)
+            barrier()
+            t_plan = 0.0
+            for _ in range(e2e_steps):
+                flush.zero_()
+                be.sync()
+                t0 = time.perf_counter()
+                nrr.nrr_bm_plan_match_host(hplan, moving_p, pd, pn)
+                t_plan += time.perf_counter() - t0
+            barrier()
+            assert np.array_equal(np.asarray(pd), res[0][1]), "plan and register forms disagree"
+            t_plan_max, plan_blocks = reduce_over_ranks(t_plan, float(hplan.n) * e2e_steps, world, dev, dist)
+            e2e["plan"] = {"value": plan_blocks / t_plan_max, "unit": UNIT, "ms_per_step": 1e3 * t_plan_max / e2e_steps,
+                           "h2d_bytes_per_step": moving_h.nbytes, "d2h_bytes_per_step": int(hplan.n) * 16,
+                           "call": "nrr_bm_plan_match_host (intra-operative work only; selection and fixed-block records "
+                                   "were made by nrr_bm_plan_create_host before the timed region)"}
+            nrr.nrr_bm_plan_destroy(hplan)
+        except Exception as e:
+            if world > 1:
+                raise
+            e2e["plan"] = {"error": repr(e)}
     if plan is not None:
         nrr.nrr_bm_plan_destroy(plan)
 
