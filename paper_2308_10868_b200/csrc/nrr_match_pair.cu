@@ -537,11 +537,34 @@ struct PairGeom {
     int pair_lanes_per_block, single_lanes_per_block;
     int union_stride;
     size_t smem;
-    double efficiency;          // useful candidate rows / issued row slots
+    double efficiency;          // useful candidate rows / row slots of the busiest warp scheduler x 4
     int ctas_per_sm;
+    int sched_max;              // row-units on the busiest scheduler (a two-row warp is 2 units, a one-row warp 1)
 };
 
 constexpr size_t kMaxSmemPerCta = 227 * 1024, kSmemPerSm = 228 * 1024;
+
+// Warp w of a CTA issues from scheduler w % 4.  A two-row warp carries 2 units of work per lane, a one-row warp 1: which
+// warp slots should the n_single one-row warps take so that the busiest scheduler has as little as possible?
+int balance_single_warps(int n_pair_warps, int n_single_warps, std::vector<int> *best_slots)
+{
+    const int nw = n_pair_warps + n_single_warps;
+    std::vector<int> slots((size_t)n_single_warps);
+    int best_max = 1 << 30;
+    std::function<void(int, int)> rec = [&](int k, int from) {
+        if (k == n_single_warps) {
+            int load[4] = {0, 0, 0, 0};
+            for (int w = 0; w < nw; ++w) load[w & 3] += 2;
+            for (int sl : slots) load[sl & 3] -= 1;
+            const int mx = std::max(std::max(load[0], load[1]), std::max(load[2], load[3]));
+            if (mx < best_max) { best_max = mx; if (best_slots) *best_slots = slots; }
+            return;
+        }
+        for (int sl = from; sl < nw; ++sl) { slots[(size_t)k] = sl; rec(k + 1, sl + 1); }
+    };
+    rec(0, 0);
+    return best_max;
+}
 
 template <int B, int R>
 bool pair_geometry(int rz, int bz, int G, PairGeom *out)
@@ -558,7 +581,11 @@ bool pair_geometry(int rz, int bz, int G, PairGeom *out)
     g.union_stride = (int)align_up(sizeof(float) * (size_t)UZ * C::UX * C::PITCH, 128);
     g.smem = (size_t)G * g.union_stride + (size_t)G * C::rec_bytes(bz) + align_up(sizeof(PairCtrl), 16) + 128;
     if (g.threads > kPairMaxThreads || g.smem > kMaxSmemPerCta) return false;
-    g.efficiency = (double)G * C::W * WZ / 32.0 / (2.0 * g.n_pair_warps + g.n_single_warps);
+    // The CTA is done when its busiest scheduler is: efficiency counts the other three schedulers' idle slots too
+    // (round 1c counted issued row slots only and preferred groupings whose warps do not divide evenly over the four
+    // schedulers, e.g. 7 warps for 7^3 / +-5 with rz = 3).
+    g.sched_max = balance_single_warps(g.n_pair_warps, g.n_single_warps, nullptr);
+    g.efficiency = (double)G * C::W * WZ / 32.0 / (4.0 * g.sched_max);
     const int by_smem = (int)(kSmemPerSm / (g.smem + 1024));
     const int by_regs = 65536 / (g.threads * 112);
     g.ctas_per_sm = by_smem < by_regs ? by_smem : by_regs;
@@ -568,8 +595,12 @@ bool pair_geometry(int rz, int bz, int G, PairGeom *out)
 }
 
 template <int B, int R>
-bool pair_plan(int rz, int bz, PairGeom *best)
+bool pair_plan(int rz, int bz, PairGeom *best, int n = 0)
 {
+    // n > 0: the number of blocks of this launch.  CTAs are handed to SMs as they free up, so the launch ends when the
+    // SM with the most CTAs does: with nCTA CTAs over the device's SMs the last round is only partly filled.  For small
+    // block lists (config 2: 1,215 blocks) this term decides; for config 3 (2,053 CTAs over 148 SMs) it is 0.99.
+    constexpr int kSms = 148;
     bool found = false;
     double best_score = 0.0;
     for (int G = 1; G <= kGMax; ++G) {
@@ -577,8 +608,13 @@ bool pair_plan(int rz, int bz, PairGeom *best)
         PairGeom g;
         if (!pair_geometry<B, R>(rz, bz, G, &g)) continue;
         // a lone CTA per SM cannot overlap its staging with another CTA's arithmetic
-        const double score = g.efficiency * (g.ctas_per_sm >= 2 ? 1.0 : 0.85);
-        if (!found || score > best_score + 1e-9) { found = true; best_score = score; *best = g; }
+        double score = g.efficiency * (g.ctas_per_sm >= 2 ? 1.0 : 0.85);
+        if (n > 0) {
+            const int ctas = (n + G - 1) / G, rounds = (ctas + kSms - 1) / kSms;
+            score *= (double)ctas / ((double)rounds * kSms);
+        }
+        // a larger group must be better by more than the model's resolution (1 %) to be taken
+        if (!found || score > best_score * 1.01) { found = true; best_score = score; *best = g; }
     }
     return found;
 }
@@ -631,23 +667,9 @@ std::vector<uint32_t> build_task_table(int rz, const PairGeom &g)
         for (int d = 0; d < C::W; ++d) { dy.push_back(d); p.push_back(0); res.push_back((P4 * d + PLANE4 * (WZ - 1)) & 7); }
         place_tasks(tab, g.n_pair_warps * 32 + blk * g.single_lanes_per_block, g.single_lanes_per_block, blk, dy, p, res);
     }
-    // Warp w issues from scheduler w % 4.  A pair warp carries two rows of work per lane, a single-row warp one:
-    // choose which warp slots the single-row warps take so that the four schedulers get equal work.
     const int nw = g.n_pair_warps + g.n_single_warps;
-    std::vector<int> best_slots, slots(g.n_single_warps);
-    int best_max = 1 << 30;
-    std::function<void(int, int)> rec = [&](int k, int from) {
-        if (k == g.n_single_warps) {
-            int load[4] = {0, 0, 0, 0};
-            for (int w = 0; w < nw; ++w) load[w & 3] += 2;
-            for (int s : slots) load[s & 3] -= 1;
-            const int mx = std::max(std::max(load[0], load[1]), std::max(load[2], load[3]));
-            if (mx < best_max) { best_max = mx; best_slots = slots; }
-            return;
-        }
-        for (int s = from; s < nw; ++s) { slots[k] = s; rec(k + 1, s + 1); }
-    };
-    rec(0, 0);
+    std::vector<int> best_slots;
+    balance_single_warps(g.n_pair_warps, g.n_single_warps, &best_slots);
     std::vector<char> is_single(nw, 0);
     for (int s : best_slots) is_single[s] = 1;
     std::vector<uint32_t> out((size_t)g.threads, 0u);
@@ -707,7 +729,7 @@ int launch_pair(const MatchCall &c, MatchPlan *plan_only, bool *handled)
     cudaStream_t stream = c.stream;
     *handled = false;
     PairGeom g;
-    if (bz < 1 || bz > kMaxBZ || !pair_plan<B, R>(rz, bz, &g)) return NRR_OK;
+    if (bz < 1 || bz > kMaxBZ || !pair_plan<B, R>(rz, bz, &g, plan_only ? 0 : n)) return NRR_OK;
     if (plan_only) {
         *handled = true;
         plan_only->fast = 2;
