@@ -572,7 +572,7 @@ def main(argv=None, backend_factory=CudaBackend):
         micro = nrr.nrr_bm_fp32_microbench() if hasattr(nrr, "nrr_bm_fp32_microbench") else None
     except Exception as e:  # pragma: no cover
         print("fp32 microbenchmark failed: %s" % e, file=sys.stderr)
-    info = nrr.nrr_bm_match_info(dims, block, window)
+    info = nrr.nrr_bm_match_info(dims, block, window, int(len(res[0][0])))
     kernel_name = {2: "match_pair_kernel", 1: "match_rows_kernel", 0: "match_generic_kernel"}[info["kernel"]]
     traffic, traffic_file = traffic_for(kernel_name, args.workload)
     roofline = {

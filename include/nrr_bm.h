@@ -354,6 +354,9 @@ NRR_BM_API int nrr_bm_profile_enable(int on);
 NRR_BM_API int nrr_bm_profile_read(double ms[4], int calls[4]);
 NRR_BM_API long long nrr_bm_launch_count(int reset);
 NRR_BM_API int nrr_bm_match_info(const int dims[3], const int block[3], const int window[3], int info[6]);
+/*  nrr_bm_match_info_n: the same for a launch of n blocks (the pair kernel groups blocks into CTAs so that the last round
+ *      of CTAs over the SMs is well filled; nrr_bm_match_info answers for a long block list). */
+NRR_BM_API int nrr_bm_match_info_n(const int dims[3], const int block[3], const int window[3], int n, int info[6]);
 NRR_BM_API int nrr_bm_fp32_peak(double *out_tflops, void *stream);
 /*  nrr_bm_fp32_microbench: the FP32 microbenchmarks behind the matching kernel's design, TFLOP/s:
  *      out[0] FFMA register chain, out[1] FFMA register tile, out[2] FFMA2 (fma.rn.f32x2) packed x packed,

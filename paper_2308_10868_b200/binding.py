@@ -22,7 +22,7 @@ NRR_E_CAPACITY, NRR_E_BOUNDS, NRR_E_SMEM, NRR_E_CUDA, NRR_E_ARG, NRR_E_DEVICE, N
 EXPORTS = [
     "nrr_bm_select_blocks", "nrr_bm_select_blocks_pruned", "nrr_bm_select_blocks_pruned_host", "nrr_bm_match", "nrr_bm_register", "nrr_bm_check_async_error", "nrr_bm_moving_stats", "nrr_bm_moving_stats_host", "nrr_bm_warp", "nrr_bm_warp_host",
     "nrr_bm_select_blocks_host", "nrr_bm_match_host", "nrr_bm_register_host",
-    "nrr_bm_profile_enable", "nrr_bm_profile_read", "nrr_bm_launch_count", "nrr_bm_match_info",
+    "nrr_bm_profile_enable", "nrr_bm_profile_read", "nrr_bm_launch_count", "nrr_bm_match_info", "nrr_bm_match_info_n",
     "nrr_bm_capacity_bound", "nrr_bm_plan_create", "nrr_bm_plan_create_host", "nrr_bm_plan_info", "nrr_bm_plan_blocks_host",
     "nrr_bm_plan_blocks_device", "nrr_bm_plan_blocks", "nrr_bm_plan_match", "nrr_bm_plan_match_range", "nrr_bm_plan_match_host", "nrr_bm_plan_destroy",
     "nrr_bm_register_batch",
@@ -125,6 +125,8 @@ def lib() -> ctypes.CDLL:
     L.nrr_bm_launch_count.argtypes = [ci]
     L.nrr_bm_match_info.restype = ci
     L.nrr_bm_match_info.argtypes = [i3, i3, i3, i3]
+    L.nrr_bm_match_info_n.restype = ci
+    L.nrr_bm_match_info_n.argtypes = [i3, i3, i3, ci, i3]
     L.nrr_bm_pair_task_table.restype = ci
     L.nrr_bm_pair_task_table.argtypes = [i3, i3, vp, ci, ctypes.POINTER(ci)]
     L.nrr_bm_fp32_peak.restype = ci
@@ -630,9 +632,10 @@ def nrr_bm_launch_count(reset: bool = False) -> int:
     return int(lib().nrr_bm_launch_count(1 if reset else 0))
 
 
-def nrr_bm_match_info(dims, block, window):
+def nrr_bm_match_info(dims, block, window, n: int = 0):
+    """Which matching kernel (and launch shape) a (dims, block, window) triple dispatches to, for a launch of n blocks."""
     info = (ctypes.c_int * 6)()
-    _check(lib().nrr_bm_match_info(_i3(dims), _i3(block), _i3(window), info))
+    _check(lib().nrr_bm_match_info_n(_i3(dims), _i3(block), _i3(window), int(n), info))
     return {"fast": bool(info[0]), "kernel": info[0], "threads": info[1], "smem_bytes": info[2], "tma": bool(info[3]),
             "candidates": info[4], "blocks_per_cta": info[5]}
 

@@ -698,6 +698,22 @@ int nrr_bm_match_info(const int dims[3], const int block[3], const int window[3]
     return NRR_OK;
 }
 
+int nrr_bm_match_info_n(const int dims[3], const int block[3], const int window[3], int n, int info[6])
+{
+    if (!info || !window) return fail(NRR_E_NULL, "info/window is NULL");
+    int rc = check_dims_block(dims, block);
+    if (rc) return rc;
+    for (int a = 0; a < 3; ++a)
+        if (window[a] < 0) return fail(NRR_E_WINDOW, "window[%d] = %d < 0", a, window[a]);
+    if (n < 0) return fail(NRR_E_ARG, "n = %d < 0", n);
+    MatchPlan plan;
+    memset(&plan, 0, sizeof(plan));
+    rc = match_plan(i3(dims), i3(block), i3(window), nullptr, nullptr, &plan, n);
+    if (rc) return rc;
+    info[0] = plan.fast; info[1] = plan.threads; info[2] = plan.smem_bytes; info[3] = plan.tma; info[4] = plan.candidates; info[5] = plan.blocks_per_cta;
+    return NRR_OK;
+}
+
 int nrr_bm_pair_task_table(const int block[3], const int window[3], unsigned int *out_table, int capacity, int info[6])
 {
     if (!block || !window || !info || (capacity > 0 && !out_table)) return fail(NRR_E_NULL, "block/window/info/out_table is NULL");

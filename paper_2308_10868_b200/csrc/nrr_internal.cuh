@@ -121,8 +121,9 @@ struct MatchPlan {
     int candidates;
     int blocks_per_cta;
 };
+// n: the number of blocks the launch will have (0: unknown / large) -- the pair kernel's grouping depends on it
 int match_plan(Int3 dims, Int3 block, Int3 window, const void *moving_ptr, const void *fixed_ptr,
-               MatchPlan *plan);
+               MatchPlan *plan, int n = 0);
 
 // One matching launch sequence.  The pair kernel works from per-block RECORDS of the fixed image (centred block, pair
 // table, 1/sqrt(SS_f): everything that needs only the pre-operative image); a caller that keeps

@@ -506,9 +506,10 @@ int dispatch(const MatchCall &c, MatchPlan *plan_only)
 
 }  // namespace
 
-int match_plan(Int3 dims, Int3 block, Int3 window, const void *moving_ptr, const void *fixed_ptr, MatchPlan *plan)
+int match_plan(Int3 dims, Int3 block, Int3 window, const void *moving_ptr, const void *fixed_ptr, MatchPlan *plan, int n)
 {
     MatchCall c;
+    c.n = n;
     c.fixed = (const float *)fixed_ptr;
     c.moving = (const float *)moving_ptr;
     c.dims = dims; c.block = block; c.window = window;

@@ -729,7 +729,7 @@ int launch_pair(const MatchCall &c, MatchPlan *plan_only, bool *handled)
     cudaStream_t stream = c.stream;
     *handled = false;
     PairGeom g;
-    if (bz < 1 || bz > kMaxBZ || !pair_plan<B, R>(rz, bz, &g, plan_only ? 0 : n)) return NRR_OK;
+    if (bz < 1 || bz > kMaxBZ || !pair_plan<B, R>(rz, bz, &g, n)) return NRR_OK;
     if (plan_only) {
         *handled = true;
         plan_only->fast = 2;

@@ -99,7 +99,7 @@ class _EmulNrr:
         v, self.launches = self.launches, 0 if reset else self.launches
         return v
 
-    def nrr_bm_match_info(self, dims, block, window):
+    def nrr_bm_match_info(self, dims, block, window, n=0):
         i = _emul.match_info(dims, block, window)
         return {"fast": bool(i["kernel"]), "kernel": i["kernel"], "threads": i["threads"], "smem_bytes": i["smem_bytes"],
                 "tma": bool(i["tma"]), "candidates": i["candidates"], "blocks_per_cta": 0}
