@@ -255,18 +255,29 @@ int register_device(const float *fixed, const float *moving, const int dims[3], 
     rc = select_enqueue(fixed, i3(dims), i3(block), i3(stride), g, frac, mask, out_blocks, capacity, nullptr, sel_buf.p,
                         &st, stream);
     span.stop();
+    // The fixed-block records need the selection only: they are made BEFORE the join, beside the moving statistics
+    // that still run on the side stream; only the matching kernel waits for both.
+    AsyncScratch rec_buf(stream);
+    MatchCall c;
+    c.fixed = fixed; c.moving = moving; c.inv_sd = inv_sd; c.dims = i3(dims); c.block = i3(block); c.window = i3(window);
+    c.blocks = out_blocks; c.n = n_cap; c.n_dev = st ? &st->k : nullptr; c.out_disp = out_disp; c.out_ncc = out_ncc;
+    c.err_flag = t_err_flag; c.stream = stream;
+    const size_t rec_bytes = n_cap > 0 ? match_records_bytes(c.block, c.window, n_cap) : 0;
+    if (rc == NRR_OK && rec_bytes > 0) {
+        if (rec_buf.alloc(rec_bytes) != cudaSuccess) rc = fail(NRR_E_CUDA, "cudaMallocAsync of the block records failed");
+        else {
+            c.records = (float *)rec_buf.p;
+            c.phase = kMatchPrepOnly;
+            rc = match_enqueue(c);
+            c.phase = kMatchKernelOnly;
+        }
+    }
     const int jrc = join();
     if (rc == NRR_OK) rc = jrc;
     if (rc == NRR_OK && out_n_dev)
         rc = cudaMemcpyAsync(out_n_dev, &st->k, sizeof(int), cudaMemcpyDeviceToDevice, stream) == cudaSuccess
                  ? NRR_OK : fail(NRR_E_CUDA, "copy of K failed");
-    if (rc == NRR_OK && n_cap > 0) {
-        MatchCall c;
-        c.fixed = fixed; c.moving = moving; c.inv_sd = inv_sd; c.dims = i3(dims); c.block = i3(block); c.window = i3(window);
-        c.blocks = out_blocks; c.n = n_cap; c.n_dev = &st->k; c.out_disp = out_disp; c.out_ncc = out_ncc;
-        c.err_flag = t_err_flag; c.stream = stream;
-        rc = match_enqueue(c);
-    }
+    if (rc == NRR_OK && n_cap > 0) rc = match_enqueue(c);
     return rc;
 }
 
