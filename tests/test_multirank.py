@@ -96,3 +96,38 @@ def test_two_ranks_shard_one_block_list_and_gather(tmp_path):
     assert r[0]["first"] == 0 and r[0]["count"] == r[1]["first"] and r[1]["first"] + r[1]["count"] == r[0]["n"]
     assert r[0]["equal"] and r[1]["equal"]                       # gathered result == single-rank result, bit for bit
     assert np.array_equal(np.load(tmp_path / "disp0.npy"), np.load(tmp_path / "disp1.npy"))
+
+
+def _bench_worker(rank, world, port, outdir, shard):
+    """bench.py's own main() under torch.distributed (gloo, 2 ranks) on the emulated library: the whole N > 1 host path --
+    rendezvous, per-rank step, the pre-timing parity gate, barriers, MAX/SUM reduction, rank 0's JSON line."""
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE=str(world))
+    sys.path.insert(0, ROOT)
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    import io
+    from contextlib import redirect_stdout
+    import bench
+    from test_bench_dryrun import _Backend
+    out = io.StringIO()
+    with redirect_stdout(out):
+        bench.main(["--gpus", str(world), "--workload", "tiny", "--steps", "1", "--warmup", "3", "--e2e-steps", "1", "--shard", shard],
+                   backend_factory=_Backend)
+    with open(os.path.join(outdir, "bench_%s_%d.txt" % (shard, rank)), "w") as f:
+        f.write(out.getvalue())
+
+
+@pytest.mark.parametrize("shard", ["blocks", "pairs"])
+def test_bench_main_on_two_ranks(tmp_path, shard):
+    import torch.multiprocessing as mp
+    port = _free_port()
+    mp.spawn(_bench_worker, args=(2, port, str(tmp_path), shard), nprocs=2, join=True)
+    out0 = open(tmp_path / ("bench_%s_0.txt" % shard)).read().strip()
+    assert open(tmp_path / ("bench_%s_1.txt" % shard)).read().strip() == ""          # rank 0 alone prints
+    line = json.loads(out0.splitlines()[-1])
+    assert line["n_gpus"] == 2 and line["value"] > 0 and line["parity"]["ok"] and line["kernel_fallback"] is None
+    if shard == "blocks":
+        # ONE block list of 259 blocks, split 129 + 130, gathered: parity is checked on the gathered result
+        assert line["scaling"] == "strong" and line["config"]["blocks_per_pair"] == 259
+        assert line["parity"]["blocks_checked"] == 259 and "all-gather" in line["config"]["parallelism"]
+    else:
+        assert line["scaling"] == "weak" and line["cpu_baseline"] is None
