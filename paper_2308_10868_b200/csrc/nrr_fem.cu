@@ -14,9 +14,11 @@
 //            by fem_cell_kernel; K u at a node is the sum over its <= 8 cells of table blocks times neighbour values.
 //   H^T S H  = W (x) I_3 with the scalar stencil W[node][27] = sum_k s_k w_k w_k^T; H^T S D = sum_k s_k w_k d_k^T:
 //            one thread per block scatters its 4 x 4 + 4 x 3 contributions with FP64 atomics (fem_accumulate_kernel).
-//   solve    Jacobi-preconditioned conjugate gradients in FP64, three kernels per iteration, no host round trip inside
-//            an iteration: dot products are reduced per CTA in a fixed order and finished by the last CTA to arrive
-//            (ticket), which also updates alpha / beta / the convergence flag on the device.
+//   solve    Jacobi-preconditioned conjugate gradients in FP64, TWO kernels per iteration (the direction update
+//            p = z + beta p_old is fused into the operator application: a neighbour's p is formed on the fly from z
+//            and p_old, the directions ping-pong between two buffers), no host round trip inside an iteration: dot
+//            products are reduced per CTA in a fixed order and finished by the last CTA to arrive (ticket), which
+//            also updates alpha / beta / the convergence flag on the device.
 #include <math.h>
 #include <string.h>
 
@@ -138,8 +140,16 @@ fem_accumulate_kernel(FemGeom g, const int *__restrict__ blocks, const int *__re
 }
 
 // ---- operator application at one node: y = [K u] (with_k) + [W u] (with_w)
+// The operand is u, or u + beta * u2 when u2 != NULL (the search direction p = z + beta p_old formed on the fly, with the
+// same explicitly fused operation wherever it is formed, so every thread sees the same bits for a given node).
+__device__ __forceinline__ double operand(const double *__restrict__ u, const double *__restrict__ u2, double beta, size_t e)
+{
+    return u2 ? fma(beta, u2[e], u[e]) : u[e];
+}
+
 __device__ __forceinline__ void apply_node(const FemGeom &g, const double *__restrict__ kcell, const double *__restrict__ wst,
-                                           const double *__restrict__ u, int i, int j, int k, bool with_k, bool with_w, double y[3])
+                                           const double *__restrict__ u, int i, int j, int k, bool with_k, bool with_w, double y[3],
+                                           const double *__restrict__ u2 = nullptr, double beta = 0.0)
 {
     y[0] = y[1] = y[2] = 0.0;
     if (with_k) {
@@ -153,10 +163,11 @@ __device__ __forceinline__ void apply_node(const FemGeom &g, const double *__res
                     for (int vb = 0; vb < 8; ++vb) {
                         const int nb = node_of(g, ci + (vb & 1), cj + ((vb >> 1) & 1), ck + (vb >> 2));
                         const double *kb = kcell + (va * 8 + vb) * 9;
-                        const double u0 = u[(size_t)nb * 3], u1 = u[(size_t)nb * 3 + 1], u2 = u[(size_t)nb * 3 + 2];
-                        y[0] += kb[0] * u0 + kb[1] * u1 + kb[2] * u2;
-                        y[1] += kb[3] * u0 + kb[4] * u1 + kb[5] * u2;
-                        y[2] += kb[6] * u0 + kb[7] * u1 + kb[8] * u2;
+                        const double v0 = operand(u, u2, beta, (size_t)nb * 3), v1 = operand(u, u2, beta, (size_t)nb * 3 + 1),
+                                     v2 = operand(u, u2, beta, (size_t)nb * 3 + 2);
+                        y[0] += kb[0] * v0 + kb[1] * v1 + kb[2] * v2;
+                        y[1] += kb[3] * v0 + kb[4] * v1 + kb[5] * v2;
+                        y[2] += kb[6] * v0 + kb[7] * v1 + kb[8] * v2;
                     }
                 }
     }
@@ -168,9 +179,9 @@ __device__ __forceinline__ void apply_node(const FemGeom &g, const double *__res
                     const double wv = wr[(di + 1) + 3 * (dj + 1) + 9 * (dk + 1)];
                     if (wv == 0.0) continue;            // also skips neighbours outside the grid (never written)
                     const int nb = node_of(g, i + di, j + dj, k + dk);
-                    y[0] += wv * u[(size_t)nb * 3];
-                    y[1] += wv * u[(size_t)nb * 3 + 1];
-                    y[2] += wv * u[(size_t)nb * 3 + 2];
+                    y[0] += wv * operand(u, u2, beta, (size_t)nb * 3);
+                    y[1] += wv * operand(u, u2, beta, (size_t)nb * 3 + 1);
+                    y[2] += wv * operand(u, u2, beta, (size_t)nb * 3 + 2);
                 }
     }
 }
@@ -275,31 +286,36 @@ pcg_init_kernel(FemGeom g, const double *__restrict__ kcell, const double *__res
     if (finish_sums<3>(part, parts, st, tot) && threadIdx.x == 0) {
         st->rz = tot[0]; st->rr = tot[1]; st->bb = tot[2];
         st->tol2 = tol * tol;
+        st->beta = 0.0;                                   // the first direction is z itself
         st->iters = 0;
         st->done = tot[1] <= tol * tol * tot[2] ? 1 : 0;
     }
 }
 
-// q = A p;  pq = p . q;  alpha = rz / pq
+// p = z + beta p_old (written to the OTHER buffer: neighbours still read p_old);  q = A p;  pq = p . q;  alpha = rz / pq.
+// The direction update is fused into the operator application: p at a neighbour is formed on the fly from z and p_old.
 __global__ void __launch_bounds__(kFemThreads)
-pcg_apply_kernel(FemGeom g, const double *__restrict__ kcell, const double *__restrict__ wst, const double *__restrict__ p,
-                 double *q, double *parts, PcgState *st)
+pcg_apply_kernel(FemGeom g, const double *__restrict__ kcell, const double *__restrict__ wst, const double *__restrict__ z,
+                 const double *__restrict__ p_old, double *__restrict__ p_new, double *q, double *parts, PcgState *st)
 {
     __shared__ double s_red[kFemThreads / 32];
     if (st->done) return;                                 // uniform over the grid: written by an earlier launch
+    const double beta = st->beta;
     const int node = blockIdx.x * kFemThreads + threadIdx.x;
     double pq = 0.0;
     if (node < g.n) {
         int i, j, k;
         node_ijk(g, node, i, j, k);
         double y[3], yw[3];
-        apply_node(g, kcell, wst, p, i, j, k, true, false, y);
-        apply_node(g, kcell, wst, p, i, j, k, false, true, yw);
+        apply_node(g, kcell, wst, z, i, j, k, true, false, y, p_old, beta);
+        apply_node(g, kcell, wst, z, i, j, k, false, true, yw, p_old, beta);
         for (int a = 0; a < 3; ++a) {
             const size_t e = (size_t)node * 3 + a;
+            const double pv = operand(z, p_old, beta, e);
             const double qv = y[a] + yw[a];
+            p_new[e] = pv;
             q[e] = qv;
-            pq += p[e] * qv;
+            pq += pv * qv;
         }
     }
     const double part[1] = {cta_sum(pq, s_red)};
@@ -341,15 +357,6 @@ pcg_update_kernel(FemGeom g, const double *__restrict__ diag, const double *__re
     }
 }
 
-// p = z + beta p   (skipped once converged: the flag was set by the update kernel of this iteration)
-__global__ void __launch_bounds__(kFemThreads)
-pcg_direction_kernel(int n3, const double *__restrict__ z, double *p, const PcgState *st)
-{
-    if (st->done) return;
-    const int e = blockIdx.x * kFemThreads + threadIdx.x;
-    if (e < n3) p[e] = z[e] + st->beta * p[e];
-}
-
 // field[c][voxel] = sum_a w_a U[node_a][c]  (fp32: what nrr_bm_warp takes)
 __global__ void __launch_bounds__(256)
 fem_dense_field_kernel(FemGeom g, const double *__restrict__ u, float *__restrict__ field)
@@ -376,7 +383,7 @@ struct nrr_bm_fem {
     FemGeom g{};
     double young = 0.0, poisson = 0.0;
     double *kcell = nullptr, *wst = nullptr, *rhs0 = nullptr, *diag = nullptr;
-    double *x = nullptr, *b = nullptr, *r = nullptr, *z = nullptr, *p = nullptr, *q = nullptr, *parts = nullptr;
+    double *x = nullptr, *b = nullptr, *r = nullptr, *z = nullptr, *p = nullptr, *p2 = nullptr, *q = nullptr, *parts = nullptr;
     PcgState *st = nullptr;
 };
 
@@ -387,7 +394,7 @@ constexpr unsigned int kFemMagic = 0x4e524646u;      // "NRFF"
 void fem_free(nrr_bm_fem *f)
 {
     if (!f) return;
-    void *bufs[] = {f->kcell, f->wst, f->rhs0, f->diag, f->x, f->b, f->r, f->z, f->p, f->q, f->parts, f->st};
+    void *bufs[] = {f->kcell, f->wst, f->rhs0, f->diag, f->x, f->b, f->r, f->z, f->p, f->p2, f->q, f->parts, f->st};
     for (void *p : bufs)
         if (p) cudaFree(p);
     f->magic = 0;
@@ -430,17 +437,18 @@ int fem_solve_device(nrr_bm_fem *f, const int *blocks, const int *disp, const fl
         NRR_LAUNCH(pcg_init_kernel, ctas, kFemThreads, 0, stream, g, f->kcell, f->wst, f->rhs0, f->diag, f->x, f->b, f->r, f->z,
                    f->p, f->parts, f->st, tol);
         NRR_LAUNCH_CHECK("pcg_init_kernel");
-        int it = 0;
+        int it = 0, cur = 0;                               // pcg_init_kernel wrote the first direction into pbuf[0]
+        double *pbuf[2] = {f->p, f->p2};
         bool done = false;
         while (!done && it < max_cg) {
             const int batch = max_cg - it < 16 ? max_cg - it : 16;      // one host poll per 16 iterations
-            for (int s = 0; s < batch; ++s) {
-                NRR_LAUNCH(pcg_apply_kernel, ctas, kFemThreads, 0, stream, g, f->kcell, f->wst, f->p, f->q, f->parts, f->st);
+            for (int s = 0; s < batch; ++s) {      // two launches per iteration; the direction ping-pongs between two buffers
+                double *p_old = pbuf[cur], *p_new = pbuf[cur ^ 1];
+                NRR_LAUNCH(pcg_apply_kernel, ctas, kFemThreads, 0, stream, g, f->kcell, f->wst, f->z, p_old, p_new, f->q, f->parts, f->st);
                 NRR_LAUNCH_CHECK("pcg_apply_kernel");
-                NRR_LAUNCH(pcg_update_kernel, ctas, kFemThreads, 0, stream, g, f->diag, f->p, f->q, f->x, f->r, f->z, f->parts, f->st);
+                NRR_LAUNCH(pcg_update_kernel, ctas, kFemThreads, 0, stream, g, f->diag, p_new, f->q, f->x, f->r, f->z, f->parts, f->st);
                 NRR_LAUNCH_CHECK("pcg_update_kernel");
-                NRR_LAUNCH(pcg_direction_kernel, (n3 + kFemThreads - 1) / kFemThreads, kFemThreads, 0, stream, n3, f->z, f->p, f->st);
-                NRR_LAUNCH_CHECK("pcg_direction_kernel");
+                cur ^= 1;
             }
             it += batch;
             NRR_CUDA(cudaMemcpyAsync(h, f->st, sizeof(PcgState), cudaMemcpyDeviceToHost, stream));
@@ -504,7 +512,7 @@ int nrr_bm_fem_create(const int dims[3], const int spacing[3], double young, dou
     auto fail_with = [&](int code) { fem_free(f); return code; };
     if (cudaGetDevice(&f->device) != cudaSuccess) return fail_with(api_fail(NRR_E_CUDA, "no CUDA device"));
     const size_t n3 = 3 * (size_t)g.n;
-    double **vecs[] = {&f->rhs0, &f->diag, &f->x, &f->b, &f->r, &f->z, &f->p, &f->q};
+    double **vecs[] = {&f->rhs0, &f->diag, &f->x, &f->b, &f->r, &f->z, &f->p, &f->p2, &f->q};
     bool ok = cudaMalloc((void **)&f->kcell, sizeof(double) * 8 * 8 * 9) == cudaSuccess &&
               cudaMalloc((void **)&f->wst, sizeof(double) * 27 * (size_t)g.n) == cudaSuccess &&
               cudaMalloc((void **)&f->parts, sizeof(double) * 3 * kMaxParts) == cudaSuccess &&
