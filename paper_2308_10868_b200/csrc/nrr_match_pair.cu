@@ -379,11 +379,16 @@ match_pair_kernel(const __grid_constant__ CUtensorMap tm_moving, const PairArgs 
             ctrl->count[lane] = 0;
         }
         const unsigned okmask = __ballot_sync(0xffffffffu, ok);
-        __syncwarp();
+        // The lane that initialised the barrier also programs it and issues every copy (the order the round-1 kernel
+        // ran on hardware: init, fence, expect_tx, copies, all by one thread); the other lanes only hand over their
+        // block's origin.  The copy instructions take warp-uniform operands anyway.
         if (lane == 0)
             mbar_arrive_expect_tx(&ctrl->bar, (a.use_tma ? (uint32_t)__popc(okmask) * union_bytes : 0u) + (uint32_t)gact * REC_FLOATS * 4u + a.debug_tx_extra);
-        __syncwarp();
-        if (ok && a.use_tma) tma_load_3d(s_unions + (size_t)lane * a.union_stride, &tm_moving, (ox - R) & ~3, oy - R, oz - rz, &ctrl->bar);
+        for (int gg = 0; gg < gact; ++gg) {
+            const int gx = __shfl_sync(0xffffffffu, ox, gg), gy = __shfl_sync(0xffffffffu, oy, gg), gz = __shfl_sync(0xffffffffu, oz, gg);
+            if (lane == 0 && a.use_tma && ((okmask >> gg) & 1u))
+                tma_load_3d(s_unions + (size_t)gg * a.union_stride, &tm_moving, (gx - R) & ~3, gy - R, gz - rz, &ctrl->bar);
+        }
         if (lane == 0) bulk_load(s_recs, a.records + (size_t)b0 * REC_FLOATS, (uint32_t)gact * REC_FLOATS * 4u, &ctrl->bar);
     }
     // this lane's task

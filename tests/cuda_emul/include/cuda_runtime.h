@@ -166,6 +166,20 @@ static inline T __shfl_up_sync(unsigned mask, T v, unsigned delta)
     memcpy(&r, &out[src], sizeof(T));
     return r;
 }
+template <class T>
+static inline T __shfl_sync(unsigned mask, T v, int src_lane)
+{
+    static_assert(sizeof(T) <= 8, "shuffle of up to 64 bits");
+    unsigned long long in = 0, out[32];
+    unsigned present;
+    memcpy(&in, &v, sizeof(T));
+    emul::warp_gather(mask, in, out, &present);
+    const int src = src_lane & 31;
+    if (!((present >> src) & 1)) return v;
+    T r;
+    memcpy(&r, &out[src], sizeof(T));
+    return r;
+}
 static inline unsigned __ballot_sync(unsigned mask, int pred)
 {
     unsigned long long out[32];

@@ -1,6 +1,12 @@
 """GPU parity tests (-m gpu): the CUDA path, called through the C ABI, against the CPU oracle, element by
 element on the same seeded inputs.  Sizes span several tiles and ragged tails; the BASELINE.json configs run
-at full size (config 4 and the 32-setting batch on sampled blocks the oracle computes one by one)."""
+at full size (config 4 and the 32-setting batch on sampled blocks the oracle computes one by one).
+
+ORDER.  The driver runs this file with -x, so the first failure hides everything behind it.  The tests are therefore
+ordered by subsystem, from what depends on least to what depends on most: selection, moving statistics, warp, FEM,
+pruned selection, then the matching kernels one family at a time (generic -> one row per thread -> two rows per
+thread; plain-load staging before TMA / bulk-copy staging), then the whole-call forms (host, register, plans, batch)
+at the BASELINE.json sizes, and last the test that makes a staging barrier time out on purpose."""
 import numpy as np
 import pytest
 
@@ -63,7 +69,30 @@ def pair(name):
     return _pairs[name]
 
 
-# ------------------------------------------------------------------------------------------- selection
+def _with_options(opts, fn):
+    for k, v in opts.items():
+        nrr.nrr_bm_set_option(k, v)
+    try:
+        return fn()
+    finally:
+        for k in opts:
+            nrr.nrr_bm_set_option(k, 0)
+
+
+def _match_case(dims, block, window, shift, noise, seed, stride=None, frac=1.0, expect_fast=None):
+    vol = _smooth(dims, seed)
+    mov = _shift_noise(vol, shift, noise, seed + 1)
+    sel = oracle.select(vol, block, stride or block, frac)
+    ora = oracle.match(vol, mov, sel["centres"], block, window)
+    info = nrr.nrr_bm_match_info(dims, block, window)
+    if expect_fast is not None:
+        assert info["fast"] == expect_fast, info
+    disp, ncc = nrr.nrr_bm_match(_cuda(vol), _cuda(mov), _cuda(sel["centres"]), block, window)
+    nrr.nrr_bm_check_async_error()
+    return assert_match_parity(disp.cpu().numpy(), ncc.cpu().numpy(), ora, label=str((dims, block, window))), len(sel["centres"])
+
+
+# ------------------------------------------------------------------------------------------- selection (S1-S3)
 @pytest.mark.parametrize("dims,block,stride,frac,mask_r", [
     ((41, 37, 29), (5, 5, 5), (5, 5, 5), 0.30, None),
     ((41, 37, 29), (7, 7, 7), (5, 5, 5), 0.25, 15.0),
@@ -106,6 +135,16 @@ def test_select_mask_excluding_everything_and_capacity_error():
     assert ei.value.status == -7
 
 
+def test_select_generic_path_equals_default():
+    cfg = CONFIGS["intraop"]
+    fixed, _, mask = pair("intraop")
+    ora = oracle.select(fixed, cfg.block, cfg.stride, cfg.frac, mask)
+    for generic in (0, 1):
+        blocks, n, ncand, var = _with_options({"select_generic": generic}, lambda: nrr.nrr_bm_select_blocks(
+            _cuda(fixed), cfg.block, cfg.stride, cfg.frac, _cuda(mask), want_var=True))
+        assert_select_parity(blocks.cpu().numpy(), n, ncand, ora, var.cpu().numpy())
+
+
 @pytest.mark.parametrize("name", ["tiny", "intraop", "fullres", "highres"])
 def test_select_parity_configs(name):
     cfg = CONFIGS[name]
@@ -116,6 +155,77 @@ def test_select_parity_configs(name):
     print("%s: N=%d K=%d oracle K/K+1 variance margin %.3g" % (name, ncand, n, ora["margin"]))
 
 
+# ------------------------------------------------------------------------------------------- moving-volume statistics (M2)
+def test_moving_stats_against_numpy():
+    dims, block = (70, 45, 33), (7, 7, 7)
+    vol = _smooth(dims, 21)
+    vol[:6, :8, :9] = 321.0                                  # a constant corner: SS = 0 -> inv_sd = 0
+    v = vol.astype(np.float64)
+    win = np.lib.stride_tricks.sliding_window_view(v, block[::-1])
+    ss = ((win - win.mean(axis=(3, 4, 5), keepdims=True)) ** 2).sum(axis=(3, 4, 5))
+    want = np.where(ss > 1e-9, 1.0 / np.sqrt(np.maximum(ss, 1e-300)), 0.0)
+    for generic in (0, 1):
+        out = torch.full(vol.shape, -7.0, dtype=torch.float32, device="cuda")
+        got = _with_options({"boxstat_generic": generic}, lambda: nrr.nrr_bm_moving_stats(_cuda(vol), block, out)).cpu().numpy()
+        valid = got[: ss.shape[0], : ss.shape[1], : ss.shape[2]]
+        assert np.all(valid[ss <= 1e-9] == 0.0)
+        rel = np.abs(valid - want)[ss > 1e-9] * np.sqrt(ss[ss > 1e-9])
+        assert rel.max() < 2e-6, rel.max()
+        untouched = np.ones(vol.shape, bool)
+        untouched[: ss.shape[0], : ss.shape[1], : ss.shape[2]] = False
+        assert np.all(got[untouched] == -7.0)
+
+
+# ------------------------------------------------------------------------------------------- dense-field warp
+@pytest.mark.parametrize("dims,amp", [((37, 21, 9), 2.5), ((64, 60, 33), 40.0), ((256, 256, 124), 8.0)])
+def test_warp_parity(dims, amp):
+    """out(p) = trilinear(image, clamp(p + v(p))) (reading Q21): |gpu - oracle| <= 8 * 2^-24 * max|image|."""
+    rng = np.random.default_rng(90 + dims[0])
+    nx, ny, nz = dims
+    img = rng.uniform(0, 1000, (nz, ny, nx)).astype(np.float32)
+    field = rng.uniform(-amp, amp, (3, nz, ny, nx)).astype(np.float32)
+    field[:, 0, 0, :4] = [[-1e9, 1e9, 0.0, 2.0]] * 3
+    got = nrr.nrr_bm_warp(_cuda(img), _cuda(field)).cpu().numpy()
+    want = oracle.warp(img, field)
+    assert np.max(np.abs(got.astype(np.float64) - want)) <= 8 * 2.0 ** -24 * 1000.0
+    assert torch.equal(nrr.nrr_bm_warp(_cuda(img), torch.zeros_like(_cuda(field))), _cuda(img))
+
+
+# ------------------------------------------------------------------------------------------- FEM regularisation
+@pytest.mark.parametrize("dims,spacing,young,poisson,weight,n_iter", [
+    ((13, 9, 11), (4, 2, 5), 3.0, 0.30, 1.0, 1),
+    ((40, 36, 24), (6, 6, 6), 1.0, 0.45, 0.5, 3),
+    ((64, 64, 32), (8, 8, 8), 2.0, 0.40, 2.0, 2),
+])
+def test_fem_solve_parity(dims, spacing, young, poisson, weight, n_iter):
+    """PAPER.md:252-265: F_i = K U_i, U_{i+1} = [K + H^T S H]^-1 [H^T S D + F_i] on the Kuhn grid mesh (Q22-Q25): the
+    CUDA path (stencil K, FP64 scatter, PCG) against the oracle's assembled sparse matrices and direct solves."""
+    from oracle import fem as ofem
+    rng = np.random.default_rng(dims[0])
+    msh = ofem.mesh(dims, spacing)
+    inside = msh["xyz"][np.all(msh["xyz"] < np.asarray(dims), axis=1)]
+    blocks = np.vstack([inside, np.floor(rng.uniform(0, np.asarray(dims) - 1e-9, (400, 3)))]).astype(np.int32)
+    disp = rng.integers(-4, 5, blocks.shape).astype(np.int32)
+    ncc = rng.uniform(-0.2, 1.0, len(blocks)).astype(np.float32)
+    ncc[::13] = np.nan
+    want = ofem.solve(msh, young, poisson, blocks, disp, ncc, weight, n_iter)["U"]
+    fem = nrr.nrr_bm_fem_create(dims, spacing, young, poisson)
+    assert fem.nodes == msh["nodes_shape"]
+    u, iters = nrr.nrr_bm_fem_solve(fem, _cuda(blocks), _cuda(disp), _cuda(ncc), weight, n_iter, tol=1e-12)
+    got = u.cpu().numpy()
+    err = np.max(np.abs(got - want))
+    print("fem %s: %d nodes, %d CG iterations, max |U - oracle| %.3g" % (dims, fem.n_nodes, iters, err))
+    assert err <= 1e-6 * max(1.0, np.max(np.abs(want)))
+    field = nrr.nrr_bm_fem_dense_field(fem, u).cpu().numpy()
+    if np.prod(dims) <= 20000:
+        ref = ofem.dense_field(msh, got, dims)
+        assert np.max(np.abs(field - ref)) <= 2e-6 * max(1.0, np.max(np.abs(ref)))
+    hu, hiters = nrr.nrr_bm_fem_solve_host(fem, blocks, disp, ncc, weight, n_iter, tol=1e-12)
+    assert np.max(np.abs(hu - got)) <= 1e-9 * max(1.0, np.max(np.abs(got)))      # FP64 atomics: order may differ
+    nrr.nrr_bm_fem_destroy(fem)
+
+
+# ------------------------------------------------------------------------------------------- connectivity pruning
 @pytest.mark.parametrize("conn", [6, 18, 26])
 @pytest.mark.parametrize("dims,block,stride,frac,mask_r", [
     ((48, 44, 40), (3, 3, 3), (1, 1, 1), 0.05, None),          # the paper's setting: every voxel a candidate
@@ -142,18 +252,37 @@ def test_pruned_selection_dense_grid_multi_launch_path():
     assert_select_parity(blocks.cpu().numpy(), n, ncand, ora)
 
 
-# ------------------------------------------------------------------------------------------- matching
-def _match_case(dims, block, window, shift, noise, seed, stride=None, frac=1.0, expect_fast=None):
-    vol = _smooth(dims, seed)
-    mov = _shift_noise(vol, shift, noise, seed + 1)
-    sel = oracle.select(vol, block, stride or block, frac)
-    ora = oracle.match(vol, mov, sel["centres"], block, window)
-    info = nrr.nrr_bm_match_info(dims, block, window)
-    if expect_fast is not None:
-        assert info["fast"] == expect_fast, info
-    disp, ncc = nrr.nrr_bm_match(_cuda(vol), _cuda(mov), _cuda(sel["centres"]), block, window)
+# ------------------------------------------------------------------------------------------- matching kernels (M1, M3-M5)
+_FAMILIES = [      # (label, options, kernel id reported by nrr_bm_match_info under these options)
+    ("generic", {"force_generic": 1}),
+    ("rows, plain staging", {"force_rows": 1, "disable_tma": 1}),
+    ("rows, TMA", {"force_rows": 1}),
+    ("pair, plain staging", {"disable_tma": 1}),
+    ("pair, TMA + bulk copy", {}),                      # the default path
+    ("pair, G=3", {"pair_blocks_per_cta": 3}),           # another grouping, partial last CTA
+]
+_family_results = {}
+
+
+@pytest.mark.parametrize("label,opts", _FAMILIES, ids=[f[0].replace(" ", "_").replace(",", "") for f in _FAMILIES])
+def test_match_kernel_families_on_the_same_input(label, opts):
+    """Every matching kernel and staging path against the oracle on one input, the simplest machinery first: the
+    generic kernel, the one-row-per-thread kernel, the pair kernel; plain loads before TMA / bulk copies.  The staging
+    path and the grouping of blocks into CTAs must not change a bit."""
+    dims, block, window = (48, 44, 40), (7, 7, 7), (5, 5, 5)
+    vol = _smooth(dims, 31)
+    mov = _shift_noise(vol, (2, 1, -2), 25.0, 32)
+    sel = oracle.select(vol, block, (5, 5, 5), 0.5)
+    assert nrr.nrr_bm_match_info(dims, block, window)["kernel"] == 2
+    d, s = _with_options(opts, lambda: nrr.nrr_bm_match(_cuda(vol), _cuda(mov), _cuda(sel["centres"]), block, window))
     nrr.nrr_bm_check_async_error()
-    return assert_match_parity(disp.cpu().numpy(), ncc.cpu().numpy(), ora, label=str((dims, block, window))), len(sel["centres"])
+    ora = oracle.match(vol, mov, sel["centres"], block, window)
+    assert_match_parity(d.cpu().numpy(), s.cpu().numpy(), ora, label=label)
+    _family_results[label] = (d, s)
+    for a, b in (("rows, plain staging", "rows, TMA"), ("pair, plain staging", "pair, TMA + bulk copy"),
+                 ("pair, TMA + bulk copy", "pair, G=3")):
+        if label == b and a in _family_results:
+            assert torch.equal(_family_results[a][0], d) and torch.equal(_family_results[a][1], s), (a, b)
 
 
 @pytest.mark.parametrize("dims,block,window,fast", [
@@ -172,95 +301,6 @@ def _match_case(dims, block, window, shift, noise, seed, stride=None, frac=1.0, 
 def test_match_parity_small(dims, block, window, fast):
     exempt, n = _match_case(dims, block, window, (1, -1, 1), 20.0, 200 + dims[0], expect_fast=fast)
     print("%s %s %s: %d blocks, %d exempt" % (dims, block, window, n, exempt))
-
-
-def _with_options(opts, fn):
-    for k, v in opts.items():
-        nrr.nrr_bm_set_option(k, v)
-    try:
-        return fn()
-    finally:
-        for k in opts:
-            nrr.nrr_bm_set_option(k, 0)
-
-
-def test_match_every_kernel_on_the_same_input():
-    """Pair kernel (default), one-row-per-thread kernel with TMA and with plain staging, generic kernel."""
-    dims, block, window = (48, 44, 40), (7, 7, 7), (5, 5, 5)
-    vol = _smooth(dims, 31)
-    mov = _shift_noise(vol, (2, 1, -2), 25.0, 32)
-    sel = oracle.select(vol, block, (5, 5, 5), 0.5)
-    c = _cuda(sel["centres"])
-    run = lambda: nrr.nrr_bm_match(_cuda(vol), _cuda(mov), c, block, window)
-    assert nrr.nrr_bm_match_info(dims, block, window)["kernel"] == 2
-    d0, n0 = run()
-    d1, n1 = _with_options({"force_rows": 1}, run)
-    d2, n2 = _with_options({"force_generic": 1}, run)
-    d3, n3 = _with_options({"force_rows": 1, "disable_tma": 1}, run)
-    d4, n4 = _with_options({"pair_blocks_per_cta": 3}, run)           # another grouping, partial last CTA
-    d5, n5 = _with_options({"disable_tma": 1}, run)                   # pair kernel, plain-load staging
-    ora = oracle.match(vol, mov, sel["centres"], block, window)
-    for d, n_, lab in ((d0, n0, "pair"), (d1, n1, "rows+tma"), (d2, n2, "generic"), (d3, n3, "rows, plain staging"),
-                       (d4, n4, "pair, G=3"), (d5, n5, "pair, plain staging")):
-        assert_match_parity(d.cpu().numpy(), n_.cpu().numpy(), ora, label=lab)
-    assert torch.equal(d1, d3) and torch.equal(n1, n3)      # the staging path must not change a bit
-    assert torch.equal(d0, d4) and torch.equal(n0, n4)      # nor may the grouping of blocks into CTAs
-    assert torch.equal(d0, d5) and torch.equal(n0, n5)
-
-
-@pytest.mark.parametrize("b,r,rz", [(7, 5, 5), (5, 3, 3), (7, 5, 3), (9, 7, 7), (11, 9, 9), (5, 9, 9), (11, 3, 3)])
-def test_match_every_candidate_row_can_win(b, r, rz):
-    """Planted displacements covering every (dy, dz) candidate row and every dx of the window (nrr_inputs.planted)."""
-    from nrr_inputs.planted import planted_pair
-    fixed, moving, centres, want = planted_pair(b, r, rz)
-    block, window = (b, b, b), (r, r, rz)
-    assert nrr.nrr_bm_match_info(fixed.shape[::-1], block, window)["kernel"] == 2
-    for opts in ({}, {"force_rows": 1}):
-        disp, ncc = _with_options(opts, lambda: nrr.nrr_bm_match(_cuda(fixed), _cuda(moving), _cuda(centres), block, window))
-        nrr.nrr_bm_check_async_error()
-        assert np.array_equal(disp.cpu().numpy(), want), opts
-        assert np.all(np.abs(ncc.cpu().numpy() - 1.0) < 1e-5)
-
-
-def test_moving_stats_against_numpy():
-    dims, block = (70, 45, 33), (7, 7, 7)
-    vol = _smooth(dims, 21)
-    vol[:6, :8, :9] = 321.0                                  # a constant corner: SS = 0 -> inv_sd = 0
-    v = vol.astype(np.float64)
-    win = np.lib.stride_tricks.sliding_window_view(v, block[::-1])
-    ss = ((win - win.mean(axis=(3, 4, 5), keepdims=True)) ** 2).sum(axis=(3, 4, 5))
-    want = np.where(ss > 1e-9, 1.0 / np.sqrt(np.maximum(ss, 1e-300)), 0.0)
-    for generic in (0, 1):
-        out = torch.full(vol.shape, -7.0, dtype=torch.float32, device="cuda")
-        got = _with_options({"boxstat_generic": generic}, lambda: nrr.nrr_bm_moving_stats(_cuda(vol), block, out)).cpu().numpy()
-        valid = got[: ss.shape[0], : ss.shape[1], : ss.shape[2]]
-        assert np.all(valid[ss <= 1e-9] == 0.0)
-        rel = np.abs(valid - want)[ss > 1e-9] * np.sqrt(ss[ss > 1e-9])
-        assert rel.max() < 2e-6, rel.max()
-        untouched = np.ones(vol.shape, bool)
-        untouched[: ss.shape[0], : ss.shape[1], : ss.shape[2]] = False
-        assert np.all(got[untouched] == -7.0)
-
-
-def test_select_generic_path_equals_default():
-    cfg = CONFIGS["intraop"]
-    fixed, _, mask = pair("intraop")
-    ora = oracle.select(fixed, cfg.block, cfg.stride, cfg.frac, mask)
-    for generic in (0, 1):
-        blocks, n, ncand, var = _with_options({"select_generic": generic}, lambda: nrr.nrr_bm_select_blocks(
-            _cuda(fixed), cfg.block, cfg.stride, cfg.frac, _cuda(mask), want_var=True))
-        assert_select_parity(blocks.cpu().numpy(), n, ncand, ora, var.cpu().numpy())
-
-
-def test_match_largest_fast_instantiation():
-    dims, block, window = (64, 60, 56), (11, 11, 11), (9, 9, 9)
-    vol = _smooth(dims, 41, sigma=2.0)
-    mov = _shift_noise(vol, (4, -6, 5), 15.0, 42)
-    sel = oracle.select(vol, block, (9, 9, 9), 0.4)
-    ora = oracle.match(vol, mov, sel["centres"], block, window)
-    assert nrr.nrr_bm_match_info(dims, block, window)["fast"]
-    disp, ncc = nrr.nrr_bm_match(_cuda(vol), _cuda(mov), _cuda(sel["centres"]), block, window)
-    assert_match_parity(disp.cpu().numpy(), ncc.cpu().numpy(), ora)
 
 
 def test_match_exact_ties_and_constant_regions():
@@ -299,6 +339,32 @@ def test_match_zero_blocks_and_bounds_flag():
     nrr.nrr_bm_check_async_error()                                       # flag was cleared
 
 
+@pytest.mark.parametrize("b,r,rz", [(7, 5, 5), (5, 3, 3), (7, 5, 3), (9, 7, 7), (11, 9, 9), (5, 9, 9), (11, 3, 3)])
+def test_match_every_candidate_row_can_win(b, r, rz):
+    """Planted displacements covering every (dy, dz) candidate row and every dx of the window (nrr_inputs.planted)."""
+    from nrr_inputs.planted import planted_pair
+    fixed, moving, centres, want = planted_pair(b, r, rz)
+    block, window = (b, b, b), (r, r, rz)
+    assert nrr.nrr_bm_match_info(fixed.shape[::-1], block, window)["kernel"] == 2
+    for opts in ({}, {"force_rows": 1}):
+        disp, ncc = _with_options(opts, lambda: nrr.nrr_bm_match(_cuda(fixed), _cuda(moving), _cuda(centres), block, window))
+        nrr.nrr_bm_check_async_error()
+        assert np.array_equal(disp.cpu().numpy(), want), opts
+        assert np.all(np.abs(ncc.cpu().numpy() - 1.0) < 1e-5)
+
+
+def test_match_largest_fast_instantiation():
+    dims, block, window = (64, 60, 56), (11, 11, 11), (9, 9, 9)
+    vol = _smooth(dims, 41, sigma=2.0)
+    mov = _shift_noise(vol, (4, -6, 5), 15.0, 42)
+    sel = oracle.select(vol, block, (9, 9, 9), 0.4)
+    ora = oracle.match(vol, mov, sel["centres"], block, window)
+    assert nrr.nrr_bm_match_info(dims, block, window)["fast"]
+    disp, ncc = nrr.nrr_bm_match(_cuda(vol), _cuda(mov), _cuda(sel["centres"]), block, window)
+    assert_match_parity(disp.cpu().numpy(), ncc.cpu().numpy(), ora)
+
+
+# ------------------------------------------------------------------------------------------- whole calls: host forms, register, plans, the BASELINE.json configs
 def test_host_forms_equal_device_forms():
     cfg = CONFIGS["tiny"]
     fixed, moving, mask = pair("tiny")
@@ -348,6 +414,66 @@ def test_match_parity_configs_full(name):
         inside = np.all((blocks.cpu().numpy() - 2 + np.asarray(cfg.shift) >= np.maximum(cfg.shift, 0)) &
                         (blocks.cpu().numpy() + 3 + np.asarray(cfg.shift) <= np.asarray(cfg.dims) + np.minimum(cfg.shift, 0)), axis=1)
         assert np.all(disp.cpu().numpy()[inside] == np.asarray(cfg.shift))
+
+
+@pytest.mark.parametrize("name", ["tiny", "intraop", "fullres"])
+def test_plan_equals_select_then_match(name):
+    """PAPER.md:233-235: the pre-operative plan (selection + fixed-block records) and the intra-operative match give
+    the bits of nrr_bm_select_blocks + nrr_bm_match; so do the host form's slab pipeline and a sharded block list."""
+    cfg = CONFIGS[name]
+    fixed, moving, mask = pair(name)
+    f, m, k = _cuda(fixed), _cuda(moving), _cuda(mask)
+    blocks, n, ncand = nrr.nrr_bm_select_blocks(f, cfg.block, cfg.stride, cfg.frac, k)
+    disp, ncc = nrr.nrr_bm_match(f, m, blocks, cfg.block, cfg.window)
+    plan = nrr.nrr_bm_plan_create(f, cfg.block, cfg.stride, cfg.window, cfg.frac, k)
+    assert nrr.nrr_bm_plan_info(plan) == (n, ncand)
+    assert np.array_equal(nrr.nrr_bm_plan_blocks_host(plan), blocks.cpu().numpy())
+    assert torch.equal(nrr.nrr_bm_plan_blocks(plan), blocks)
+    for _ in range(2):                                               # a plan serves many intra-operative volumes
+        pd, pn = nrr.nrr_bm_plan_match(plan, m)
+        nrr.nrr_bm_check_async_error()
+        assert torch.equal(pd, disp) and torch.equal(pn, ncc)
+    od = torch.full((n, 3), -99, dtype=torch.int32, device="cuda")
+    on = torch.full((n,), -99.0, dtype=torch.float32, device="cuda")
+    cuts = [0, n // 2, n]                                            # two "ranks", each its slice of the block list
+    for a, b in zip(cuts[:-1], cuts[1:]):
+        nrr.nrr_bm_plan_match_range(plan, m, od, on, first=a, count=b - a)
+    nrr.nrr_bm_check_async_error()
+    assert torch.equal(od, disp) and torch.equal(on, ncc)
+    nrr.nrr_bm_plan_destroy(plan)
+    hplan = nrr.nrr_bm_plan_create_host(fixed, cfg.block, cfg.stride, cfg.window, cfg.frac, mask)
+    for slabs in (4, 1, 9):
+        nrr.nrr_bm_set_option("plan_slabs", slabs)
+        hd, hn = nrr.nrr_bm_plan_match_host(hplan, moving)
+        assert np.array_equal(hd, disp.cpu().numpy()) and np.array_equal(hn, ncc.cpu().numpy()), slabs
+    nrr.nrr_bm_set_option("plan_slabs", 4)
+    nrr.nrr_bm_plan_destroy(hplan)
+
+
+def test_register_then_regularise_then_warp_on_the_tiny_config():
+    """The whole chain on the device: select + match (PAPER.md:231-250) -> biomechanical regularisation
+    (PAPER.md:252-265) -> dense field -> warp (PAPER.md:225-229).  The constructed translation (2,-1,1) is recovered
+    at every mesh node and the warped intra-operative image lands on the pre-operative one."""
+    cfg = CONFIGS["tiny"]
+    fixed, moving, _ = pair("tiny")
+    f, m = _cuda(fixed), _cuda(moving)
+    blocks, n, _ = nrr.nrr_bm_select_blocks(f, cfg.block, cfg.stride, cfg.frac)
+    disp, ncc = nrr.nrr_bm_match(f, m, blocks, cfg.block, cfg.window)
+    fem = nrr.nrr_bm_fem_create(cfg.dims, (8, 8, 8), 1.0, 0.45)
+    u, iters = nrr.nrr_bm_fem_solve(fem, blocks, disp, ncc, weight=1.0, n_iter=5)
+    un = u.cpu().numpy()
+    nn = np.asarray(fem.nodes)
+    core = un.reshape(nn[2], nn[1], nn[0], 3)[1:-1, 1:-1, 1:-1]               # away from the hull (clamped shift, skipped candidates)
+    dev = np.abs(core - np.asarray(cfg.shift))                                   # border blocks see the clamped shift
+    assert np.median(dev) < 0.1 and np.max(dev) < 1.0, (np.median(dev), np.max(dev))
+    field = nrr.nrr_bm_fem_dense_field(fem, u)
+    warped = nrr.nrr_bm_warp(m, field).cpu().numpy()
+    inner = (slice(6, -6), slice(8, -8), slice(8, -8))
+    before = np.abs(moving[inner] - fixed[inner]).mean()
+    after = np.abs(warped[inner] - fixed[inner]).mean()
+    print("tiny chain: %d blocks, %d CG iterations, mean |moving - fixed| %.2f -> %.2f after the warp" % (n, iters, before, after))
+    assert after < 0.5 * before
+    nrr.nrr_bm_fem_destroy(fem)
 
 
 def test_match_parity_highres_sampled():
@@ -408,40 +534,7 @@ def test_match_parity_batch_sampled():
         assert torch.equal(rd[:n], results[si][1][:n]) and torch.equal(rs[:n], results[si][2][:n])
 
 
-@pytest.mark.parametrize("name", ["tiny", "intraop", "fullres"])
-def test_plan_equals_select_then_match(name):
-    """PAPER.md:233-235: the pre-operative plan (selection + fixed-block records) and the intra-operative match give
-    the bits of nrr_bm_select_blocks + nrr_bm_match; so do the host form's slab pipeline and a sharded block list."""
-    cfg = CONFIGS[name]
-    fixed, moving, mask = pair(name)
-    f, m, k = _cuda(fixed), _cuda(moving), _cuda(mask)
-    blocks, n, ncand = nrr.nrr_bm_select_blocks(f, cfg.block, cfg.stride, cfg.frac, k)
-    disp, ncc = nrr.nrr_bm_match(f, m, blocks, cfg.block, cfg.window)
-    plan = nrr.nrr_bm_plan_create(f, cfg.block, cfg.stride, cfg.window, cfg.frac, k)
-    assert nrr.nrr_bm_plan_info(plan) == (n, ncand)
-    assert np.array_equal(nrr.nrr_bm_plan_blocks_host(plan), blocks.cpu().numpy())
-    assert torch.equal(nrr.nrr_bm_plan_blocks(plan), blocks)
-    for _ in range(2):                                               # a plan serves many intra-operative volumes
-        pd, pn = nrr.nrr_bm_plan_match(plan, m)
-        nrr.nrr_bm_check_async_error()
-        assert torch.equal(pd, disp) and torch.equal(pn, ncc)
-    od = torch.full((n, 3), -99, dtype=torch.int32, device="cuda")
-    on = torch.full((n,), -99.0, dtype=torch.float32, device="cuda")
-    cuts = [0, n // 2, n]                                            # two "ranks", each its slice of the block list
-    for a, b in zip(cuts[:-1], cuts[1:]):
-        nrr.nrr_bm_plan_match_range(plan, m, od, on, first=a, count=b - a)
-    nrr.nrr_bm_check_async_error()
-    assert torch.equal(od, disp) and torch.equal(on, ncc)
-    nrr.nrr_bm_plan_destroy(plan)
-    hplan = nrr.nrr_bm_plan_create_host(fixed, cfg.block, cfg.stride, cfg.window, cfg.frac, mask)
-    for slabs in (4, 1, 9):
-        nrr.nrr_bm_set_option("plan_slabs", slabs)
-        hd, hn = nrr.nrr_bm_plan_match_host(hplan, moving)
-        assert np.array_equal(hd, disp.cpu().numpy()) and np.array_equal(hn, ncc.cpu().numpy()), slabs
-    nrr.nrr_bm_set_option("plan_slabs", 4)
-    nrr.nrr_bm_plan_destroy(hplan)
-
-
+# ------------------------------------------------------------------------------------------- the bounded staging wait (last: it makes a kernel wait out its time bound)
 def test_staging_timeout_reports_device_error_without_faulting():
     """The matching kernel's bounded wait: an over-programmed staging barrier must end as NRR_E_DEVICE (-12) with NaN
     results and a usable context afterwards -- never a trap."""
@@ -463,78 +556,3 @@ def test_staging_timeout_reports_device_error_without_faulting():
     again = nrr.nrr_bm_match(f, m, blocks[:8], cfg.block, cfg.window)
     nrr.nrr_bm_check_async_error()
     assert torch.equal(again[0], good[0]) and torch.equal(again[1], good[1])
-
-
-# ------------------------------------------------------------------------------------------- dense-field warp
-@pytest.mark.parametrize("dims,amp", [((37, 21, 9), 2.5), ((64, 60, 33), 40.0), ((256, 256, 124), 8.0)])
-def test_warp_parity(dims, amp):
-    """out(p) = trilinear(image, clamp(p + v(p))) (reading Q21): |gpu - oracle| <= 8 * 2^-24 * max|image|."""
-    rng = np.random.default_rng(90 + dims[0])
-    nx, ny, nz = dims
-    img = rng.uniform(0, 1000, (nz, ny, nx)).astype(np.float32)
-    field = rng.uniform(-amp, amp, (3, nz, ny, nx)).astype(np.float32)
-    field[:, 0, 0, :4] = [[-1e9, 1e9, 0.0, 2.0]] * 3
-    got = nrr.nrr_bm_warp(_cuda(img), _cuda(field)).cpu().numpy()
-    want = oracle.warp(img, field)
-    assert np.max(np.abs(got.astype(np.float64) - want)) <= 8 * 2.0 ** -24 * 1000.0
-    assert torch.equal(nrr.nrr_bm_warp(_cuda(img), torch.zeros_like(_cuda(field))), _cuda(img))
-
-
-# ------------------------------------------------------------------------------------------- FEM regularisation
-@pytest.mark.parametrize("dims,spacing,young,poisson,weight,n_iter", [
-    ((13, 9, 11), (4, 2, 5), 3.0, 0.30, 1.0, 1),
-    ((40, 36, 24), (6, 6, 6), 1.0, 0.45, 0.5, 3),
-    ((64, 64, 32), (8, 8, 8), 2.0, 0.40, 2.0, 2),
-])
-def test_fem_solve_parity(dims, spacing, young, poisson, weight, n_iter):
-    """PAPER.md:252-265: F_i = K U_i, U_{i+1} = [K + H^T S H]^-1 [H^T S D + F_i] on the Kuhn grid mesh (Q22-Q25): the
-    CUDA path (stencil K, FP64 scatter, PCG) against the oracle's assembled sparse matrices and direct solves."""
-    from oracle import fem as ofem
-    rng = np.random.default_rng(dims[0])
-    msh = ofem.mesh(dims, spacing)
-    inside = msh["xyz"][np.all(msh["xyz"] < np.asarray(dims), axis=1)]
-    blocks = np.vstack([inside, np.floor(rng.uniform(0, np.asarray(dims) - 1e-9, (400, 3)))]).astype(np.int32)
-    disp = rng.integers(-4, 5, blocks.shape).astype(np.int32)
-    ncc = rng.uniform(-0.2, 1.0, len(blocks)).astype(np.float32)
-    ncc[::13] = np.nan
-    want = ofem.solve(msh, young, poisson, blocks, disp, ncc, weight, n_iter)["U"]
-    fem = nrr.nrr_bm_fem_create(dims, spacing, young, poisson)
-    assert fem.nodes == msh["nodes_shape"]
-    u, iters = nrr.nrr_bm_fem_solve(fem, _cuda(blocks), _cuda(disp), _cuda(ncc), weight, n_iter, tol=1e-12)
-    got = u.cpu().numpy()
-    err = np.max(np.abs(got - want))
-    print("fem %s: %d nodes, %d CG iterations, max |U - oracle| %.3g" % (dims, fem.n_nodes, iters, err))
-    assert err <= 1e-6 * max(1.0, np.max(np.abs(want)))
-    field = nrr.nrr_bm_fem_dense_field(fem, u).cpu().numpy()
-    if np.prod(dims) <= 20000:
-        ref = ofem.dense_field(msh, got, dims)
-        assert np.max(np.abs(field - ref)) <= 2e-6 * max(1.0, np.max(np.abs(ref)))
-    hu, hiters = nrr.nrr_bm_fem_solve_host(fem, blocks, disp, ncc, weight, n_iter, tol=1e-12)
-    assert np.max(np.abs(hu - got)) <= 1e-9 * max(1.0, np.max(np.abs(got)))      # FP64 atomics: order may differ
-    nrr.nrr_bm_fem_destroy(fem)
-
-
-def test_register_then_regularise_then_warp_on_the_tiny_config():
-    """The whole chain on the device: select + match (PAPER.md:231-250) -> biomechanical regularisation
-    (PAPER.md:252-265) -> dense field -> warp (PAPER.md:225-229).  The constructed translation (2,-1,1) is recovered
-    at every mesh node and the warped intra-operative image lands on the pre-operative one."""
-    cfg = CONFIGS["tiny"]
-    fixed, moving, _ = pair("tiny")
-    f, m = _cuda(fixed), _cuda(moving)
-    blocks, n, _ = nrr.nrr_bm_select_blocks(f, cfg.block, cfg.stride, cfg.frac)
-    disp, ncc = nrr.nrr_bm_match(f, m, blocks, cfg.block, cfg.window)
-    fem = nrr.nrr_bm_fem_create(cfg.dims, (8, 8, 8), 1.0, 0.45)
-    u, iters = nrr.nrr_bm_fem_solve(fem, blocks, disp, ncc, weight=1.0, n_iter=5)
-    un = u.cpu().numpy()
-    nn = np.asarray(fem.nodes)
-    core = un.reshape(nn[2], nn[1], nn[0], 3)[1:-1, 1:-1, 1:-1]               # away from the hull (clamped shift, skipped candidates)
-    dev = np.abs(core - np.asarray(cfg.shift))                                   # border blocks see the clamped shift
-    assert np.median(dev) < 0.1 and np.max(dev) < 1.0, (np.median(dev), np.max(dev))
-    field = nrr.nrr_bm_fem_dense_field(fem, u)
-    warped = nrr.nrr_bm_warp(m, field).cpu().numpy()
-    inner = (slice(6, -6), slice(8, -8), slice(8, -8))
-    before = np.abs(moving[inner] - fixed[inner]).mean()
-    after = np.abs(warped[inner] - fixed[inner]).mean()
-    print("tiny chain: %d blocks, %d CG iterations, mean |moving - fixed| %.2f -> %.2f after the warp" % (n, iters, before, after))
-    assert after < 0.5 * before
-    nrr.nrr_bm_fem_destroy(fem)

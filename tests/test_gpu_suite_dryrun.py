@@ -6,7 +6,7 @@ import sys
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
-QUICK = ("(test_select_parity_small or test_select_uniform or test_select_mask or test_match_parity_small or every_kernel "
+QUICK = ("(test_select_parity_small or test_select_uniform or test_select_mask or test_match_parity_small or kernel_families "
          "or zero_blocks or exact_ties or host_forms or moving_stats or (register and tiny) or (warp and dims0) "
          "or (pruned and dims0-6) or staging_timeout or (fem_solve and dims0)) and not 11-11")
 
