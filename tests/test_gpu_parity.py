@@ -102,11 +102,15 @@ def _match_case(dims, block, window, shift, noise, seed, stride=None, frac=1.0, 
     ((130, 3, 3), (3, 3, 3), (1, 1, 1), 0.10, None),         # degenerate thin volume
     ((9, 9, 9), (9, 9, 9), (1, 1, 1), 1.00, None),           # a single candidate
 ])
-def test_select_parity_small(dims, block, stride, frac, mask_r):
+@pytest.mark.parametrize("generic", [1, 0], ids=["round1_kernels", "default_kernels"])
+def test_select_parity_small(generic, dims, block, stride, frac, mask_r):
+    """generic = 1: the runtime-shaped statistics kernel and the multi-launch radix select that ran on hardware in
+    round 1 (first, so that a failure of the default kernels is told apart from a failure of the method)."""
     vol = _smooth(dims, 100 + dims[0])
     mask = None if mask_r is None else spherical_mask(dims, mask_r)
     ora = oracle.select(vol, block, stride, frac, mask)
-    blocks, n, ncand, var = nrr.nrr_bm_select_blocks(_cuda(vol), block, stride, frac, _cuda(mask), want_var=True)
+    blocks, n, ncand, var = _with_options({"select_generic": generic}, lambda: nrr.nrr_bm_select_blocks(
+        _cuda(vol), block, stride, frac, _cuda(mask), want_var=True))
     assert_select_parity(blocks.cpu().numpy(), n, ncand, ora, var.cpu().numpy())
 
 
@@ -156,7 +160,8 @@ def test_select_parity_configs(name):
 
 
 # ------------------------------------------------------------------------------------------- moving-volume statistics (M2)
-def test_moving_stats_against_numpy():
+@pytest.mark.parametrize("generic", [1, 0], ids=["round1_kernel", "sliding_kernel"])
+def test_moving_stats_against_numpy(generic):
     dims, block = (70, 45, 33), (7, 7, 7)
     vol = _smooth(dims, 21)
     vol[:6, :8, :9] = 321.0                                  # a constant corner: SS = 0 -> inv_sd = 0
@@ -164,16 +169,15 @@ def test_moving_stats_against_numpy():
     win = np.lib.stride_tricks.sliding_window_view(v, block[::-1])
     ss = ((win - win.mean(axis=(3, 4, 5), keepdims=True)) ** 2).sum(axis=(3, 4, 5))
     want = np.where(ss > 1e-9, 1.0 / np.sqrt(np.maximum(ss, 1e-300)), 0.0)
-    for generic in (0, 1):
-        out = torch.full(vol.shape, -7.0, dtype=torch.float32, device="cuda")
-        got = _with_options({"boxstat_generic": generic}, lambda: nrr.nrr_bm_moving_stats(_cuda(vol), block, out)).cpu().numpy()
-        valid = got[: ss.shape[0], : ss.shape[1], : ss.shape[2]]
-        assert np.all(valid[ss <= 1e-9] == 0.0)
-        rel = np.abs(valid - want)[ss > 1e-9] * np.sqrt(ss[ss > 1e-9])
-        assert rel.max() < 2e-6, rel.max()
-        untouched = np.ones(vol.shape, bool)
-        untouched[: ss.shape[0], : ss.shape[1], : ss.shape[2]] = False
-        assert np.all(got[untouched] == -7.0)
+    out = torch.full(vol.shape, -7.0, dtype=torch.float32, device="cuda")
+    got = _with_options({"boxstat_generic": generic}, lambda: nrr.nrr_bm_moving_stats(_cuda(vol), block, out)).cpu().numpy()
+    valid = got[: ss.shape[0], : ss.shape[1], : ss.shape[2]]
+    assert np.all(valid[ss <= 1e-9] == 0.0)
+    rel = np.abs(valid - want)[ss > 1e-9] * np.sqrt(ss[ss > 1e-9])
+    assert rel.max() < 2e-6, rel.max()
+    untouched = np.ones(vol.shape, bool)
+    untouched[: ss.shape[0], : ss.shape[1], : ss.shape[2]] = False
+    assert np.all(got[untouched] == -7.0)
 
 
 # ------------------------------------------------------------------------------------------- dense-field warp
