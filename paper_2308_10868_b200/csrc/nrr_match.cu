@@ -179,7 +179,7 @@ __global__ void __launch_bounds__(kFastMaxThreads) match_rows_kernel(const __gri
     }
 
     if (use_tma) {
-        if (!mbar_wait(&sm->bar_union, 0)) sm->stage_failed = 1;
+        if (!mbar_wait(&sm->bar_union, 0, err_flag)) sm->stage_failed = 1;
         if (xoff != 0) {                      // uniform over the CTA
             const int nstaged = UZ * C::UX;   // rows that are read later: (z, y < UX)
             for (int r = tid; r < nstaged; r += blockDim.x) {

@@ -21,7 +21,7 @@ __device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count) { emul:
 __device__ __forceinline__ void mbar_fence_init() {}
 __device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t *bar, uint32_t bytes) { emul::mbar_arrive_expect_tx(bar, bytes); }
 __device__ __forceinline__ bool mbar_try_wait(uint64_t *bar, uint32_t parity) { return emul::mbar_try_wait(bar, parity); }
-__device__ __forceinline__ bool mbar_wait(uint64_t *bar, uint32_t parity)
+__device__ __forceinline__ bool mbar_wait(uint64_t *bar, uint32_t parity, const unsigned int *)
 {
     for (int spin = 0; spin < 3; ++spin)
         if (mbar_try_wait(bar, parity)) return true;
@@ -66,13 +66,21 @@ __device__ __forceinline__ uint64_t global_timer_ns()
 // not completed after kMbarTimeoutNs of wall time (bounded by time, not by polls: time-slicing, a debugger or a long
 // TMA queue must not fire it on a healthy copy); the caller then reports NRR_E_DEVICE through the sticky error
 // flag and leaves the kernel in an orderly way -- no __trap(), no Xid.
+// Fail fast once one CTA has given up: a wait that has lasted kMbarPeekNs (a healthy copy lands in microseconds) also
+// looks at the sticky error flag, so the CTAs behind the first time-out leave after a millisecond each instead of
+// holding the GPU for the full bound round after round (19,757 CTAs of config 4 would be 134 rounds x 4 s).
 constexpr uint64_t kMbarTimeoutNs = 4000000000ull;
-__device__ __forceinline__ bool mbar_wait(uint64_t *bar, uint32_t parity)
+constexpr uint64_t kMbarPeekNs = 1000000ull;
+__device__ __forceinline__ bool mbar_wait(uint64_t *bar, uint32_t parity, const unsigned int *err_flag)
 {
     if (mbar_try_wait(bar, parity)) return true;
     const uint64_t t0 = global_timer_ns();
-    while (!mbar_try_wait(bar, parity))
-        if (global_timer_ns() - t0 > kMbarTimeoutNs) return false;
+    while (!mbar_try_wait(bar, parity)) {
+        const uint64_t dt = global_timer_ns() - t0;
+        if (dt <= kMbarPeekNs) continue;
+        if (dt > kMbarTimeoutNs) return false;
+        if (err_flag && (*(const volatile unsigned int *)err_flag & 2u /* kErrStaging */)) return false;
+    }
     return true;
 }
 __device__ __forceinline__ void tma_load_3d(void *dst, const CUtensorMap *map, int x, int y, int z, uint64_t *bar)

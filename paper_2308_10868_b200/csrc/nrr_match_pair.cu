@@ -414,7 +414,7 @@ match_pair_kernel(const __grid_constant__ CUtensorMap tm_moving, const PairArgs 
             ((float *)(s_unions + (size_t)gg * a.union_stride))[((size_t)zz * UX + yy) * PITCH + xx] = v;
         }
     }
-    if (!mbar_wait(&ctrl->bar, 0)) ctrl->stage_failed = 1;
+    if (!mbar_wait(&ctrl->bar, 0, a.err_flag)) ctrl->stage_failed = 1;
     // ---- undo the TMA alignment slack: shift every staged row left by its block's 0..3 floats
     if (a.use_tma) {
         const int rows_per_block = UZ * UX;
