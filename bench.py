@@ -56,7 +56,20 @@ def parse_args(argv=None):
     ap.add_argument("--e2e-steps", type=int, default=None, help="steps of the host-buffer (end-to-end) legs")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-parity", action="store_true", help="skip the oracle comparison reported under 'parity'")
+    ap.add_argument("--option", action="append", default=[], metavar="NAME=VALUE",
+                    help="library option for this run (nrr_bm_set_option), e.g. pair_blocks_per_cta=2, force_rows=1, "
+                         "disable_tma=1: the A/B runs and sweeps behind DESIGN.md 6.3; recorded under config.options")
     return ap.parse_args(argv)
+
+
+def parse_options(pairs):
+    out = {}
+    for item in pairs:
+        name, sep, value = item.partition("=")
+        if not sep or not name:
+            raise SystemExit("--option wants NAME=VALUE, got %r" % item)
+        out[name] = float(value)
+    return out
 
 
 def valid_candidates(blocks: np.ndarray, dims, block, window) -> np.ndarray:
@@ -343,6 +356,9 @@ def main(argv=None, backend_factory=CudaBackend):
 
     be = backend_factory(local_rank)
     nrr, dev = be.nrr, be.dev
+    options = parse_options(args.option)
+    for name, value in options.items():
+        nrr.nrr_bm_set_option(name, value)
     if world > 1:
         dist.init_process_group(be.collective_backend, device_id=dev if dev.type == "cuda" else None)
     shard_blocks = args.shard == "blocks" and world > 1
@@ -628,7 +644,7 @@ def main(argv=None, backend_factory=CudaBackend):
         "dtype": "f32", "data": "synthetic",
         "config": dict(config_of(args.workload, cfg, settings), blocks_per_pair=int(n),
                        candidates_per_block=cfg.n_candidates if not is_batch else "343..6859",
-                       l2="flushed between steps (256 MB write)",
+                       l2="flushed between steps (256 MB write)", options=options,
                        parallelism=("block list sharded over ranks + all-gather of 16 B/block" if shard_blocks else "independent pairs per GPU")),
         "cand_evals_per_sec": evals * args.steps * (1 if shard_blocks else world) / (total_ms_max * 1e-3),
         # only matching is time-critical: the two halves are reported separately and summed

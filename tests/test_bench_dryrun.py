@@ -8,6 +8,7 @@ import time
 from contextlib import redirect_stdout
 
 import numpy as np
+import pytest
 import torch
 
 import _emul
@@ -155,6 +156,23 @@ def test_bench_main_runs_end_to_end_on_the_emulated_library():
     e2e = line["e2e"]
     assert e2e["h2d_bytes_per_step"] == 2 * 64 * 64 * 32 * 4 and e2e["d2h_bytes_per_step"] == 259 * 28 + 4
     assert line["gpu_launches"] == 10 and line["value"] > 0 and e2e["value"] > 0
+    assert line["config"]["options"] == {}
+
+
+def test_bench_option_flag_reaches_the_library_and_the_line():
+    """--option NAME=VALUE (the A/B runs of DESIGN.md 6.3): force_rows=1 must time the one-row-per-thread kernel."""
+    out = io.StringIO()
+    try:
+        with redirect_stdout(out):
+            bench.main(["--workload", "tiny", "--steps", "1", "--warmup", "3", "--e2e-steps", "1", "--no-cpu-baseline",
+                        "--option", "force_rows=1"], backend_factory=_Backend)
+    finally:
+        _emul.set_option("force_rows", 0)
+    line = json.loads(out.getvalue().strip().splitlines()[-1])
+    assert line["config"]["options"] == {"force_rows": 1.0}
+    assert line["roofline"]["kernel"] == "match_rows_kernel" and line["parity"]["ok"]
+    with pytest.raises(SystemExit):
+        bench.parse_options(["force_rows"])
 
 
 def test_reference_arm_times_the_whole_oracle_step_and_agrees_with_cpu_baseline():
