@@ -365,9 +365,10 @@ NRR_BM_API int nrr_bm_fp32_peak(double *out_tflops, void *stream);
  *      out[4] one candidate row per thread with FFMA, out[5] two rows with FFMA, out[6] two rows with FFMA2. */
 NRR_BM_API int nrr_bm_fp32_microbench(double out_tflops[7], void *stream);
 /*  nrr_bm_pair_task_table: the host-built lane -> task table of the pair matching kernel for a cubic block and a
- *      window (wx == wy), one word per thread of a CTA: bit 31 = lane has a task, bit 30 = one-row warp,
- *      bits 16..23 = block of the CTA's group, bits 8..15 = dy index, bits 0..7 = pair index p (rows dz = 2p, 2p+1;
- *      a one-row task has dz = 2*wz).  info[0] = threads per CTA (= words written), info[1] = blocks per CTA,
+ *      window (wx == wy), one word per thread of a CTA: bit 31 = lane has a task, bit 30 = y-pair warp (the last
+ *      candidate plane), bits 16..23 = block of the CTA's group, bits 8..15 = dy index, bits 0..7 = p: a z-pair task
+ *      owns the rows (dy, dz = 2p) and (dy, 2p+1); a y-pair task owns (dy, dz = 2*wz) and, if p = 1, (dy+1, 2*wz).
+ *      info[0] = threads per CTA (= words written), info[1] = blocks per CTA,
  *      info[2] = staged row pitch (floats), info[3] = staged rows per plane, info[4] = bytes between the unions of
  *      consecutive blocks in shared memory, info[5] = dynamic shared memory bytes.  No device needed. */
 NRR_BM_API int nrr_bm_pair_task_table(const int block[3], const int window[3], unsigned int *out_table, int capacity,

@@ -27,7 +27,9 @@
 //                 second, so one FFMA2 (fma.rn.f32x2: scalar moving voxel x pair of fixed voxels from the pair
 //                 table) does two useful FMAs per issue slot and halves the shared-memory traffic per FMA.
 //                 The two end planes touch one row only and use plain FFMA on one half of the pair.  The
-//                 odd plane of candidates (dz = 2rz) is handled by separate warps with one row per thread.
+//                 odd plane of candidates (dz = 2rz) is handled by separate warps whose threads own two rows
+//                 adjacent in y, (dy, 2rz) and (dy+1, 2rz) (plain FFMA; one row per block stays alone), so that
+//                 every warp of the CTA carries two candidate rows per lane.
 //                 Which lane takes which (block, dy, p) comes from a host-built table that packs the tasks of
 //                 the G blocks into full warps and keeps the LDS.128 of each quarter-warp on distinct banks.
 //    M4 argmax  : NCC in registers; per-block maximum through a warp reduction and one 64-bit shared atomicMax
@@ -39,7 +41,6 @@
 #include <math.h>
 #include <string.h>
 
-#include <functional>
 #include <map>
 #include <mutex>
 #include <vector>
@@ -292,28 +293,54 @@ __device__ __forceinline__ void pair_rows(const float *urow, const float *rec, i
     }
 }
 
-// One candidate row per thread (the odd last plane of candidates).
+// The odd last plane of candidates (dz = 2 rz): two candidate rows adjacent in y per thread, (dy, 2rz) and (dy+1, 2rz).
+// Row vy of the union meets fixed row vy for the first candidate row and vy-1 for the second, so every moving row
+// loaded feeds both (plain FFMA on two sets of accumulators: a packed form would need a second pair table).  The
+// first union row of a plane touches the first candidate row only, the row after the last the second only.  `second`
+// is false for the one task per block whose row has no partner (W is odd): its rb is never used.
 template <int B, int R>
-__device__ __forceinline__ void single_row(const float *urow, const float *rec, int bz, float (&ra)[2 * R + 1])
+__device__ __forceinline__ void ypair_rows(const float *urow, const float *rec, int bz, bool second, float (&ra)[2 * R + 1], float (&rb)[2 * R + 1])
 {
     using C = PairCfg<B, R>;
     constexpr int NVX = C::NV;
     constexpr int W = C::W, PITCH = C::PITCH, PLANE = C::UX * C::PITCH;
 #pragma unroll
-    for (int j = 0; j < W; ++j) ra[j] = 0.f;
+    for (int j = 0; j < W; ++j) { ra[j] = 0.f; rb[j] = 0.f; }
 #pragma unroll 1
     for (int vz = 0; vz < bz; ++vz) {
         const float *up = urow + vz * PLANE;
         const float *fp = rec + vz * B * C::FP;
-#pragma unroll 1
-        for (int vy = 0; vy < B; ++vy) {
+        {   // union row 0: first candidate row only, fixed row 0
             float m[NVX * 4], f[C::FP];
-            load_row<NVX>(m, up + vy * PITCH);
-            load_row<C::NF>(f, fp + vy * C::FP);
+            load_row<NVX>(m, up);
+            load_row<C::NF>(f, fp);
 #pragma unroll
             for (int vx = 0; vx < B; ++vx)
 #pragma unroll
                 for (int j = 0; j < W; ++j) ra[j] = fmaf(f[vx], m[j + vx], ra[j]);
+        }
+#pragma unroll 1
+        for (int vy = 1; vy < B; ++vy) {
+            float m[NVX * 4], fa[C::FP], fb[C::FP];
+            load_row<NVX>(m, up + vy * PITCH);
+            load_row<C::NF>(fa, fp + vy * C::FP);
+            load_row<C::NF>(fb, fp + (vy - 1) * C::FP);
+#pragma unroll
+            for (int vx = 0; vx < B; ++vx)
+#pragma unroll
+                for (int j = 0; j < W; ++j) {
+                    ra[j] = fmaf(fa[vx], m[j + vx], ra[j]);
+                    rb[j] = fmaf(fb[vx], m[j + vx], rb[j]);
+                }
+        }
+        if (second) {   // union row B: second candidate row only, fixed row B-1 (a row without a partner has no such union row)
+            float m[NVX * 4], f[C::FP];
+            load_row<NVX>(m, up + B * PITCH);
+            load_row<C::NF>(f, fp + (B - 1) * C::FP);
+#pragma unroll
+            for (int vx = 0; vx < B; ++vx)
+#pragma unroll
+                for (int j = 0; j < W; ++j) rb[j] = fmaf(f[vx], m[j + vx], rb[j]);
         }
     }
 }
@@ -322,7 +349,7 @@ __device__ __forceinline__ void single_row(const float *urow, const float *rec, 
 struct PairArgs {
     const float *fixed, *moving, *inv_sd, *records;
     const int *blocks;
-    const uint32_t *task_tab;      // [threads]: valid << 31 | single-row warp << 30 | g << 16 | dy << 8 | p
+    const uint32_t *task_tab;      // [threads]: valid << 31 | y-pair warp << 30 | g << 16 | dy << 8 | p (z-pair: plane pair; y-pair: 1 = the row dy+1 belongs to the task)
     const unsigned int *n_dev;     // nullable: the number of blocks is min(n, *n_dev)
     int *out_disp;
     float *out_ncc;
@@ -440,9 +467,12 @@ match_pair_kernel(const __grid_constant__ CUtensorMap tm_moving, const PairArgs 
     float ra[W], rb[W];
     const float *urow = (const float *)(s_unions + (size_t)g * a.union_stride) + (size_t)dzA * PLANE + dyi * PITCH;
     const float *rec = s_recs + (size_t)g * REC_FLOATS;
+    // second candidate row of the task: one plane further (z-pair) or one row further (y-pair, unless the row is alone)
+    const bool has_b = is_pair || p != 0;
+    const int dyB = is_pair ? dyi : dyi + 1, dzB = is_pair ? dzA + 1 : dzA;
     if (active) {
         if (is_pair) pair_rows<B, R>(urow, rec, bz, ra, rb);
-        else single_row<B, R>(urow, rec, bz, ra);
+        else ypair_rows<B, R>(urow, rec, bz, has_b, ra, rb);
     }
 
     // ---- M4: NCC and the per-block arg-max
@@ -465,16 +495,16 @@ match_pair_kernel(const __grid_constant__ CUtensorMap tm_moving, const PairArgs 
                 if (v > bv) { bv = v; bi = (dzA * W + dyi) * W + j; }
             }
         }
-        if (is_pair) {
-            const int pz = org.z + dzA + 1 - rz;
-            const bool row_ok = y_ok && pz >= 0 && pz + bz <= dims.z;
-            const float *ip = a.inv_sd + ((size_t)pz * dims.y + py) * dims.x + org.x - R;
+        if (has_b) {
+            const int pyb = org.y + dyB - R, pz = org.z + dzB - rz;
+            const bool row_ok = pyb >= 0 && pyb + B <= dims.y && pz >= 0 && pz + bz <= dims.z;
+            const float *ip = a.inv_sd + ((size_t)pz * dims.y + pyb) * dims.x + org.x - R;
 #pragma unroll
             for (int j = 0; j < W; ++j) {
                 const bool ok = row_ok && j >= jlo && j <= jhi;
                 const float v = ok ? rb[j] * __ldg(ip + j) * isd_f : -INFINITY;
                 rb[j] = v;
-                if (v > bv) { bv = v; bi = ((dzA + 1) * W + dyi) * W + j; }
+                if (v > bv) { bv = v; bi = (dzB * W + dyB) * W + j; }
             }
         }
     }
@@ -503,10 +533,10 @@ match_pair_kernel(const __grid_constant__ CUtensorMap tm_moving, const PairArgs 
             const int idx = (dzA * W + dyi) * W + j;
             if (ra[j] >= thr && idx != big) s_list[atomicAdd(&ctrl->count[g], 1)] = idx;
         }
-        if (is_pair) {
+        if (has_b) {
 #pragma unroll
             for (int j = 0; j < W; ++j) {
-                const int idx = ((dzA + 1) * W + dyi) * W + j;
+                const int idx = (dzB * W + dyB) * W + j;
                 if (rb[j] >= thr && idx != big) s_list[atomicAdd(&ctrl->count[g], 1)] = idx;
             }
         }
@@ -538,38 +568,16 @@ match_pair_kernel(const __grid_constant__ CUtensorMap tm_moving, const PairArgs 
 
 // ------------------------------------------------------------------------------------------ host side
 struct PairGeom {
-    int G, n_pair_warps, n_single_warps, threads;
-    int pair_lanes_per_block, single_lanes_per_block;
+    int G, n_pair_warps, n_ypair_warps, threads;
+    int pair_lanes_per_block, ypair_lanes_per_block;
     int union_stride;
     size_t smem;
     double efficiency;          // useful candidate rows / row slots of the busiest warp scheduler x 4
     int ctas_per_sm;
-    int sched_max;              // row-units on the busiest scheduler (a two-row warp is 2 units, a one-row warp 1)
+    int sched_max;              // row-units on the busiest scheduler (every warp carries two candidate rows per lane)
 };
 
 constexpr size_t kMaxSmemPerCta = 227 * 1024, kSmemPerSm = 228 * 1024;
-
-// Warp w of a CTA issues from scheduler w % 4.  A two-row warp carries 2 units of work per lane, a one-row warp 1: which
-// warp slots should the n_single one-row warps take so that the busiest scheduler has as little as possible?
-int balance_single_warps(int n_pair_warps, int n_single_warps, std::vector<int> *best_slots)
-{
-    const int nw = n_pair_warps + n_single_warps;
-    std::vector<int> slots((size_t)n_single_warps);
-    int best_max = 1 << 30;
-    std::function<void(int, int)> rec = [&](int k, int from) {
-        if (k == n_single_warps) {
-            int load[4] = {0, 0, 0, 0};
-            for (int w = 0; w < nw; ++w) load[w & 3] += 2;
-            for (int sl : slots) load[sl & 3] -= 1;
-            const int mx = std::max(std::max(load[0], load[1]), std::max(load[2], load[3]));
-            if (mx < best_max) { best_max = mx; if (best_slots) *best_slots = slots; }
-            return;
-        }
-        for (int sl = from; sl < nw; ++sl) { slots[(size_t)k] = sl; rec(k + 1, sl + 1); }
-    };
-    rec(0, 0);
-    return best_max;
-}
 
 template <int B, int R>
 bool pair_geometry(int rz, int bz, int G, PairGeom *out)
@@ -579,17 +587,17 @@ bool pair_geometry(int rz, int bz, int G, PairGeom *out)
     PairGeom g;
     g.G = G;
     g.pair_lanes_per_block = (C::W * NP + 7) / 8 * 8;
-    g.single_lanes_per_block = (C::W + 7) / 8 * 8;
+    g.ypair_lanes_per_block = ((C::W + 1) / 2 + 7) / 8 * 8;      // the last plane: (W-1)/2 pairs of rows and one row alone
     g.n_pair_warps = (G * g.pair_lanes_per_block + 31) / 32;
-    g.n_single_warps = (G * g.single_lanes_per_block + 31) / 32;
-    g.threads = (g.n_pair_warps + g.n_single_warps) * 32;
+    g.n_ypair_warps = (G * g.ypair_lanes_per_block + 31) / 32;
+    g.threads = (g.n_pair_warps + g.n_ypair_warps) * 32;
     g.union_stride = (int)align_up(sizeof(float) * (size_t)UZ * C::UX * C::PITCH, 128);
     g.smem = (size_t)G * g.union_stride + (size_t)G * C::rec_bytes(bz) + align_up(sizeof(PairCtrl), 16) + 128;
     if (g.threads > kPairMaxThreads || g.smem > kMaxSmemPerCta) return false;
-    // The CTA is done when its busiest scheduler is: efficiency counts the other three schedulers' idle slots too
-    // (round 1c counted issued row slots only and preferred groupings whose warps do not divide evenly over the four
-    // schedulers, e.g. 7 warps for 7^3 / +-5 with rz = 3).
-    g.sched_max = balance_single_warps(g.n_pair_warps, g.n_single_warps, nullptr);
+    // The CTA is done when its busiest scheduler is (warp w issues from scheduler w % 4): efficiency counts the other
+    // three schedulers' idle slots too.  Every warp carries two candidate rows per lane, so the busiest scheduler is the
+    // one with the most warps.
+    g.sched_max = 2 * ((g.n_pair_warps + g.n_ypair_warps + 3) / 4);
     g.efficiency = (double)G * C::W * WZ / 32.0 / (4.0 * g.sched_max);
     const int by_smem = (int)(kSmemPerSm / (g.smem + 1024));
     const int by_regs = 65536 / (g.threads * 112);
@@ -657,6 +665,17 @@ void place_tasks(std::vector<uint32_t> &tab, int lane0, int lanes, int g, const 
         }
 }
 
+// Start rows of the y-pair tasks of the last candidate plane: rows are paired from 0 up to a pivot row that stays
+// alone, then from pivot + 1 on, so that the starts run through even and then odd values -- with an odd row pitch (in
+// 16-byte units) up to eight of them fall on distinct bank groups (W = 7, 11, 15: all of them).
+inline void ypair_starts(int W, std::vector<int> *dy, std::vector<int> *has_partner)
+{
+    const int pivot = W - 1 < 6 ? W - 1 : 6;          // even, <= W - 1 (W is odd)
+    for (int d = 0; d < pivot; d += 2) { dy->push_back(d); has_partner->push_back(1); }
+    dy->push_back(pivot); has_partner->push_back(0);
+    for (int d = pivot + 1; d + 1 < W; d += 2) { dy->push_back(d); has_partner->push_back(1); }
+}
+
 template <int B, int R>
 std::vector<uint32_t> build_task_table(int rz, const PairGeom &g)
 {
@@ -669,21 +688,13 @@ std::vector<uint32_t> build_task_table(int rz, const PairGeom &g)
             for (int d = 0; d < C::W; ++d) { dy.push_back(d); p.push_back(pp); res.push_back((P4 * d + PLANE4 * 2 * pp) & 7); }
         place_tasks(tab, blk * g.pair_lanes_per_block, g.pair_lanes_per_block, blk, dy, p, res);
         dy.clear(); p.clear(); res.clear();
-        for (int d = 0; d < C::W; ++d) { dy.push_back(d); p.push_back(0); res.push_back((P4 * d + PLANE4 * (WZ - 1)) & 7); }
-        place_tasks(tab, g.n_pair_warps * 32 + blk * g.single_lanes_per_block, g.single_lanes_per_block, blk, dy, p, res);
+        ypair_starts(C::W, &dy, &p);
+        for (int d : dy) res.push_back((P4 * d + PLANE4 * (WZ - 1)) & 7);
+        place_tasks(tab, g.n_pair_warps * 32 + blk * g.ypair_lanes_per_block, g.ypair_lanes_per_block, blk, dy, p, res);
     }
-    const int nw = g.n_pair_warps + g.n_single_warps;
-    std::vector<int> best_slots;
-    balance_single_warps(g.n_pair_warps, g.n_single_warps, &best_slots);
-    std::vector<char> is_single(nw, 0);
-    for (int s : best_slots) is_single[s] = 1;
-    std::vector<uint32_t> out((size_t)g.threads, 0u);
-    int vp = 0, vs = g.n_pair_warps;                 // next virtual pair / single warp
-    for (int w = 0; w < nw; ++w) {
-        const int v = is_single[w] ? vs++ : vp++;
-        for (int l = 0; l < 32; ++l) out[(size_t)w * 32 + l] = tab[(size_t)v * 32 + l] | (is_single[w] ? 0x40000000u : 0u);
-    }
-    return out;
+    for (int w = g.n_pair_warps; w < g.n_pair_warps + g.n_ypair_warps; ++w)
+        for (int l = 0; l < 32; ++l) tab[(size_t)w * 32 + l] |= 0x40000000u;      // role bit, uniform over the warp
+    return tab;
 }
 
 std::mutex g_tab_mutex;

@@ -105,7 +105,7 @@ def _grid_blocks(dims, block, stride):
     ((32, 30, 26), 7, 5, 5, (9, 11, 9), 3),       # a group size that leaves a partial last CTA
     ((32, 30, 24), 7, 5, 3, (12, 11, 8), 0),      # the config-2 shape: anisotropic window (5,5,3)
     ((36, 34, 30), 9, 7, 7, (13, 12, 10), 0),     # the config-4 shape
-    ((28, 28, 24), 5, 5, 0, (11, 11, 9), 0),      # rz = 0: only the single-row warps work
+    ((28, 28, 24), 5, 5, 0, (11, 11, 9), 0),      # rz = 0: only the y-pair warps of the last (only) candidate plane work
     ((32, 30, 30), 11, 3, 3, (10, 9, 9), 0),
     ((29, 27, 25), 5, 3, 3, (6, 7, 8), 0),        # nx not a multiple of 4: TMA cannot address it, plain staging
     ((32, 30, 20), (7, 3), 5, 2, (9, 11, 5), 0),  # thick-slice block 7 x 7 x 3

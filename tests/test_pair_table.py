@@ -1,7 +1,8 @@
 """Host logic of the pair matching kernel (no GPU): the lane -> task table must give every candidate row of every
-block of a CTA's group to exactly one lane, keep one-row warps and two-row warps apart, spread the work evenly
-over the four warp schedulers of an SM, and keep the LDS.128 row addresses of a quarter-warp on distinct 16-byte
-bank groups where the counts allow it (paper_2308_10868_b200/csrc/nrr_match_pair.cu)."""
+block of a CTA's group to exactly one lane, keep the z-pair warps (rows (dy, 2p), (dy, 2p+1)) and the y-pair warps of
+the last candidate plane (rows (dy, 2rz), (dy+1, 2rz); one row per block alone) apart, and keep the LDS.128 row
+addresses of a quarter-warp on distinct 16-byte bank groups where the counts allow it
+(paper_2308_10868_b200/csrc/nrr_match_pair.cu)."""
 import numpy as np
 import pytest
 
@@ -13,7 +14,7 @@ SHAPES = [(b, r, rz) for b in (5, 7, 9, 11) for r in (3, 5, 7, 9) for rz in (r,)
 
 def _decode(tab):
     valid = (tab >> 31) & 1
-    single = (tab >> 30) & 1
+    single = (tab >> 30) & 1          # y-pair warp: the last candidate plane, p = 1 if the row dy+1 belongs to the task
     g = (tab >> 16) & 0xFF
     dy = (tab >> 8) & 0xFF
     p = tab & 0xFF
@@ -34,7 +35,11 @@ def test_every_candidate_row_has_exactly_one_lane(b, r, rz):
             continue
         assert gg < info["blocks_per_cta"] and d < w
         if s:
+            assert pp in (0, 1)
             rows.append((gg, d, wz - 1))
+            if pp:
+                assert d + 1 < w
+                rows.append((gg, d + 1, wz - 1))
         else:
             assert 2 * pp + 1 <= wz - 2 + 1 and 2 * pp + 1 < wz
             rows += [(gg, d, 2 * pp), (gg, d, 2 * pp + 1)]
@@ -52,15 +57,13 @@ def test_schedulers_are_balanced_and_quarter_warps_mostly_conflict_free(b, r, rz
     valid, single, g, dy, p = _decode(tab)
     nw = len(tab) // 32
     wz = 2 * rz + 1
-    load = [0, 0, 0, 0]                                           # warp w issues from scheduler w % 4
-    for wi in range(nw):
-        load[wi % 4] += 1 if single[wi * 32] else 2
-    n_single = sum(1 for wi in range(nw) if single[wi * 32])
-    # no choice of warp slots for the one-row warps gives a smaller maximum (brute force over the slot sets)
-    import itertools
-    best = min(max(sum((1 if wi in sl else 2) for wi in range(nw) if wi % 4 == s) for s in range(4))
-               for sl in map(set, itertools.combinations(range(nw), n_single)))
-    assert max(load) == best
+    # every warp carries two candidate rows per lane, whatever its role: at most one row per block is without a partner
+    for gg in range(info["blocks_per_cta"]):
+        alone = [i for i in range(len(tab)) if valid[i] and single[i] and g[i] == gg and p[i] == 0]
+        assert len(alone) == 1
+    # the y-pair warps come last, so that the z-pair warps fill the scheduler slots first (warp w issues from w % 4)
+    roles = [bool(single[wi * 32]) for wi in range(nw)]
+    assert roles == sorted(roles)
     # shared-memory wavefronts of one LDS.128 of moving voxels: per quarter-warp, the largest number of lanes whose
     # row address falls into the same 16-byte bank group (address in 16-byte units: base + P4*dy + PLANE4*dz)
     p4 = info["pitch"] // 4
@@ -80,7 +83,10 @@ def test_schedulers_are_balanced_and_quarter_warps_mostly_conflict_free(b, r, rz
 def test_config3_numbers_quoted_in_design_md():
     tab, info = nrr.nrr_bm_pair_task_table((7, 7, 7), (5, 5, 5))
     valid, single, g, dy, p = _decode(tab)
-    assert info["blocks_per_cta"] == 4 and info["threads"] == 288 and info["pitch"] == 20
+    assert info["blocks_per_cta"] == 4 and info["threads"] == 256 and info["pitch"] == 20
     assert 2 * (info["smem_bytes"] + 1024) <= 228 * 1024          # two CTAs per SM
-    assert int(valid.sum()) == 4 * (55 + 11)
-    assert [wi for wi in range(9) if single[wi * 32]] == [0, 4]    # two of scheduler 0's three slots: 4 units each
+    assert int(valid.sum()) == 4 * (55 + 6)                       # 55 z-pairs and 5 y-pairs + 1 row alone per block
+    assert [wi for wi in range(8) if single[wi * 32]] == [7]       # 8 warps of 2 row-units: two per scheduler
+    # the six y-pair tasks of a block start at rows 0, 2, 4, 6 (alone), 7, 9: distinct bank groups for pitch 5 x 16 B
+    ys = sorted((int(dy[i]), int(p[i])) for i in range(len(tab)) if valid[i] and single[i] and g[i] == 0)
+    assert ys == [(0, 1), (2, 1), (4, 1), (6, 0), (7, 1), (9, 1)]
