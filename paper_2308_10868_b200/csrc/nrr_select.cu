@@ -403,13 +403,26 @@ select_small_kernel(const double *__restrict__ var, long long ngrid, Int3 block,
         } else {
             if (tid == 0) s_nlist = 0u;
             __syncthreads();
-            for (long long g = tid; g < ngrid; g += kSmallThreads) {
-                const unsigned long long key = key_of(var[g]);
-                if ((key & mask) == prefix) {
-                    atomicAdd(&s_hist[digit_of(key, pass)], 1u);
-                    if (mask != 0ull) {        // with no digit decided yet everything matches: not worth listing
-                        const unsigned int slot = atomicAdd(&s_nlist, 1u);
-                        if (slot < (unsigned int)kSmallList) s_list[slot] = key;
+            // One CTA cannot hide the latency of one load per thread and trip: kScanAhead independent loads are issued
+            // before the first key is used (a full scan of config 3's 60,000 keys is 59 keys per thread).
+            constexpr int kScanAhead = 8;
+            for (long long g0 = tid; g0 < ngrid; g0 += (long long)kSmallThreads * kScanAhead) {
+                double v[kScanAhead];
+#pragma unroll
+                for (int u = 0; u < kScanAhead; ++u) {
+                    const long long g = g0 + (long long)u * kSmallThreads;
+                    v[u] = g < ngrid ? var[g] : -1.0;
+                }
+#pragma unroll
+                for (int u = 0; u < kScanAhead; ++u) {
+                    if (g0 + (long long)u * kSmallThreads >= ngrid) break;
+                    const unsigned long long key = key_of(v[u]);
+                    if ((key & mask) == prefix) {
+                        atomicAdd(&s_hist[digit_of(key, pass)], 1u);
+                        if (mask != 0ull) {        // with no digit decided yet everything matches: not worth listing
+                            const unsigned int slot = atomicAdd(&s_nlist, 1u);
+                            if (slot < (unsigned int)kSmallList) s_list[slot] = key;
+                        }
                     }
                 }
             }
@@ -425,7 +438,7 @@ select_small_kernel(const double *__restrict__ var, long long ngrid, Int3 block,
     const unsigned int ties = st->k_remaining;
     if (tid == 0) s_carry = 0ull;
     __syncthreads();
-    constexpr int IPT = 4;
+    constexpr int IPT = 8;      // consecutive keys per thread and trip: eight independent loads, half the block scans of four
     for (long long start = 0; start < ngrid; start += (long long)kSmallThreads * IPT) {
         const long long base = start + (long long)tid * IPT;
         unsigned long long keys[IPT];
