@@ -588,13 +588,16 @@ def main(argv=None, backend_factory=CudaBackend):
         micro = nrr.nrr_bm_fp32_microbench() if hasattr(nrr, "nrr_bm_fp32_microbench") else None
     except Exception as e:  # pragma: no cover
         print("fp32 microbenchmark failed: %s" % e, file=sys.stderr)
-    info = nrr.nrr_bm_match_info(dims, block, window, int(len(res[0][0])))
+    # the launch shape depends on the number of blocks the launch is SIZED for: this rank's slice (--shard blocks), or
+    # the capacity bound of nrr_bm_register (K is known only on the device; CTAs beyond K exit at once)
+    launch_n = count if shard_blocks else (int(len(res[0][0])) if is_batch else cap)
+    info = nrr.nrr_bm_match_info(dims, block, window, int(launch_n))
     kernel_name = {2: "match_pair_kernel", 1: "match_rows_kernel", 0: "match_generic_kernel"}[info["kernel"]]
     traffic, traffic_file = traffic_for(kernel_name, args.workload)
     roofline = {
         "bound": "alu", "kernel": kernel_name if not is_batch else "match_pair_kernel (32 launches, all shapes)",
         "launch": {"threads": info["threads"], "smem_bytes": info["smem_bytes"],
-                   "blocks_per_cta": info["blocks_per_cta"], "tma": info["tma"]},
+                   "blocks_per_cta": info["blocks_per_cta"], "tma": info["tma"], "sized_for_blocks": int(launch_n)},
         "achieved": achieved_tflops, "peak": FP32_PEAK_TFLOPS,
         "unit": "TFLOP/s", "frac": achieved_tflops / FP32_PEAK_TFLOPS,
         "peak_source": "derived: 148 SMs x 128 FP32 lanes x 2 x 1.965 GHz (MEASURED_PEAKS.json has no FP32 figure)",
