@@ -140,11 +140,14 @@ template <int B>
 __device__ double block_variance_cubic(const float *__restrict__ fixed, Int3 dims, int ox, int oy, int oz)
 {
     constexpr int RY = B <= 7 ? B : (B == 9 ? 5 : 4);      // rows loaded ahead of the additions (<= 49 values)
+    // Planes unrolled into one basic block, so that the loads of the next plane are scheduled under the additions of
+    // this one (with one plane per trip every plane exposed a full load latency: 14 per block).
+    constexpr int ZUNROLL = B <= 7 ? B : 2;
     const double nvox = (double)(B * B * B);
     const size_t plane = (size_t)dims.x * dims.y;
     const float *org = fixed + ((size_t)oz * dims.y + oy) * dims.x + ox;
     double s = 0.0;
-#pragma unroll 1
+#pragma unroll(ZUNROLL)
     for (int z = 0; z < B; ++z) {
 #pragma unroll
         for (int y0 = 0; y0 < B; y0 += RY) {
@@ -163,7 +166,7 @@ __device__ double block_variance_cubic(const float *__restrict__ fixed, Int3 dim
     }
     const double mean = __ddiv_rn(s, nvox);
     double q = 0.0;
-#pragma unroll 1
+#pragma unroll(ZUNROLL)
     for (int z = 0; z < B; ++z) {
 #pragma unroll
         for (int y0 = 0; y0 < B; y0 += RY) {
