@@ -274,10 +274,12 @@ int register_device(const float *fixed, const float *moving, const int dims[3], 
     }
     const int jrc = join();
     if (rc == NRR_OK) rc = jrc;
+    if (rc == NRR_OK && n_cap > 0) rc = match_enqueue(c);
+    // K goes out BEHIND the matching kernel: a copy node in front of it would only delay the time-critical launch
+    // (the selection state lives in call scratch that is released, in stream order, after this copy)
     if (rc == NRR_OK && out_n_dev)
         rc = cudaMemcpyAsync(out_n_dev, &st->k, sizeof(int), cudaMemcpyDeviceToDevice, stream) == cudaSuccess
                  ? NRR_OK : fail(NRR_E_CUDA, "copy of K failed");
-    if (rc == NRR_OK && n_cap > 0) rc = match_enqueue(c);
     return rc;
 }
 
